@@ -1,0 +1,372 @@
+"""Pins for the FP64 oracle: every check compares `oracle/` with something that is NOT the oracle --
+a library routine, a closed form, a hand-built case, brute force, or numerical quadrature of Eq. 8.
+(CPU only; `-m "not gpu"`.)  Citations: P:<line> of PAPER.md, R<k> of DESIGN.md section 3."""
+import math
+
+import numpy as np
+import pytest
+
+import oracle
+import bioem_workloads as W
+from bioem_workloads import simulate
+
+RNG = np.random.default_rng(20161)
+
+
+# ------------------------------------------------------------------ DFT (Eqs. 2-3, R3)
+@pytest.mark.parametrize("N", [6, 8, 14])
+def test_dft2_matches_library_fft(N):
+    x = RNG.normal(size=(N, N)) + 1j * RNG.normal(size=(N, N))
+    assert np.allclose(oracle.dft2(x, -1), np.fft.fft2(x), atol=1e-11)
+    assert np.allclose(oracle.dft2(x, +1, 1.0 / N ** 2), np.fft.ifft2(x), atol=1e-12)
+
+
+def test_plancherel():
+    # C_oo ~ sum |F(I)|^2
+    x = RNG.normal(size=(12, 12))
+    F = oracle.dft2(x)
+    assert math.isclose((x ** 2).sum(), (np.abs(F) ** 2).sum() / x.size, rel_tol=1e-12)
+
+
+def test_dft3_matches_library():
+    rho = RNG.normal(size=(6, 6, 6))
+    assert np.allclose(oracle.dft3(rho), np.fft.fftn(rho), atol=1e-10)
+
+
+# ------------------------------------------------------------------ cross-correlation (Eq. 7 / 11 / 12; R4, R5)
+def test_cross_corr_delta_images_pin_the_shift_sign():
+    # I_obs = delta at (j0,k0), I1 = delta at (j1,k1):  C_co(d) = sum_r I_obs(r) I1(r+d) = 1 iff r0 + d == r1 (mod N)
+    N, D = 8, 3
+    a = np.zeros((N, N)); b = np.zeros((N, N))
+    j0, k0, j1, k1 = 2, 5, 4, 3            # x = j (fast index), y = k
+    a[k0, j0] = 1.0; b[k1, j1] = 1.0
+    C = oracle.cross_corr_direct(a, b, D)
+    want = np.zeros((2 * D + 1, 2 * D + 1)); want[(k1 - k0) + D, (j1 - j0) + D] = 1.0     # dy = -2, dx = +2
+    assert np.array_equal(C, want)
+    # wrap-around (R5): delta near the border
+    a[:] = 0; b[:] = 0; a[7, 7] = 1.0; b[1, 0] = 1.0     # dx = 0-7 = +1 (mod 8), dy = 1-7 = +2 (mod 8)
+    C = oracle.cross_corr_direct(a, b, D)
+    assert C[2 + D, 1 + D] == 1.0 and C.sum() == 1.0
+
+
+@pytest.mark.parametrize("N,D", [(8, 3), (6, 2), (7, 3)])
+def test_direct_sum_equals_naive_dft_eq12(N, D):
+    # north_star check 1: the FFT-free correlation equals a naive DFT evaluation of Eq. 12 on tiny images
+    a, b = RNG.normal(size=(N, N)), RNG.normal(size=(N, N))
+    C = oracle.cross_corr_direct(a, b, D)
+    assert np.allclose(C, oracle.cross_corr_eq12(a, b, D), atol=1e-12)
+    assert np.allclose(C, oracle.cross_corr_dft(a, b, D), atol=1e-12)                      # tier B
+    # library routine: irfft2(conj(A) B)[dy mod N, dx mod N]
+    lib = np.fft.ifft2(np.conj(np.fft.fft2(a)) * np.fft.fft2(b)).real
+    idx = np.arange(-D, D + 1) % N
+    assert np.allclose(C, lib[np.ix_(idx, idx)], atol=1e-12)
+
+
+def test_tier_b_matches_direct_on_a_real_pair():
+    wl = W.build_workload("tiny_mini")
+    s = wl["spec"]
+    I1 = oracle.calc_image(wl["models"][0], wl["quats"][1], wl["ctfs"][2], s.n_pix, s.pixel_A)
+    img = wl["images"][0].astype(np.float64)
+    A, B = oracle.cross_corr_direct(img, I1, s.max_shift), oracle.cross_corr_dft(img, I1, s.max_shift)
+    assert np.abs(A - B).max() <= 1e-9 * np.abs(A).max()
+
+
+def test_shift_of_observed_image_moves_the_map():
+    # d <-> rolling I_obs: I_obs'(r) = I_obs(r - e)  =>  C'(d) = C(d - e)... checked on the unpruned map
+    N, D = 8, 4
+    a, b = RNG.normal(size=(N, N)), RNG.normal(size=(N, N))
+    C = oracle.cross_corr_direct(a, b, D)
+    a2 = np.roll(a, shift=(1, 2), axis=(0, 1))         # a2[k][j] = a[k-1][j-2]
+    C2 = oracle.cross_corr_direct(a2, b, D)
+    # sum_r a(r - e) b(r + d) = sum_r a(r) b(r + d + e)  =>  C2(d) = C(d + e), e = (ex=2, ey=1)
+    assert np.allclose(C2[0:2 * D, 0:2 * D - 1], C[1:2 * D + 1, 2:2 * D + 1], atol=1e-12)
+
+
+# ------------------------------------------------------------------ closed form (stands in for Eq. S8; R1)
+def _sums(obs, cal):
+    return obs.size, obs.sum(), (obs ** 2).sum(), cal.sum(), (cal ** 2).sum(), (obs * cal).sum()
+
+
+def _quadrature_log_marginal(obs, cal):
+    """log of int dN dmu dlambda of Eq. 8 with I_cal = N*cal - mu (Eq. 7) and unit priors.
+    The integrand is the raw sum of squares at every node; the completed squares only centre the grids."""
+    n = obs.size
+    Co, Coo, Cc, Ccc, Cco = obs.sum(), (obs ** 2).sum(), cal.sum(), (cal ** 2).sum(), (obs * cal).sum()
+    A, B, Dd = Ccc - Cc ** 2 / n, Cco - Co * Cc / n, Coo - Co ** 2 / n
+    E = Dd - B ** 2 / A
+    Nstar = B / A
+    u = np.linspace(math.log(2e-3 * math.sqrt(E / n)), math.log(5e2 * math.sqrt(E / n)), 1201)
+    K = 161
+    t = np.linspace(-12.0, 12.0, K)
+    vals = np.empty_like(u)
+    for i, lam in enumerate(np.exp(u)):
+        Ng = Nstar + t * lam / math.sqrt(A)                               # [K]
+        mustar = (Ng * Cc - Co) / n
+        mug = mustar[:, None] + t[None, :] * lam / math.sqrt(n)           # [K_N][K_mu]
+        resid = obs[None, None, :] - Ng[:, None, None] * cal[None, None, :] + mug[:, :, None]
+        logL = -(resid ** 2).sum(-1) / (2 * lam * lam) - 0.5 * n * math.log(2 * math.pi * lam * lam)
+        ref = logL.max()
+        w = np.exp(logL - ref)
+        inner = np.trapezoid(w, dx=(t[1] - t[0]) * lam / math.sqrt(n), axis=1)
+        outer = np.trapezoid(inner, dx=(t[1] - t[0]) * lam / math.sqrt(A))
+        vals[i] = math.log(outer) + ref + u[i]                            # d lambda = lambda du
+    ref = vals.max()
+    return math.log(np.trapezoid(np.exp(vals - ref), dx=u[1] - u[0])) + ref
+
+
+@pytest.mark.parametrize("n", [9, 12, 16])
+def test_closed_form_equals_quadrature_of_eq8(n):
+    # north_star check 3
+    rng = np.random.default_rng(100 + n)
+    obs = rng.normal(size=n) * 1.7 + 0.4
+    cal = rng.normal(size=n) * 0.6 - 0.2
+    obs = obs + 0.8 * cal                      # some correlation
+    c1 = oracle.log_post_c1(*_sums(obs, cal))
+    c2 = oracle.log_post_c2(*_sums(obs, cal))
+    quad = _quadrature_log_marginal(obs, cal)
+    assert abs(c1 - c2) < 1e-10
+    assert abs(c1 - quad) < 2e-7, (c1, quad)
+
+
+def test_eq8_function_matches_its_definition():
+    rng = np.random.default_rng(5)
+    obs, cal = rng.normal(size=10), rng.normal(size=10)
+    Nn, mu, lam = 1.3, -0.2, 0.7
+    want = -((obs - (Nn * cal - mu)) ** 2).sum() / (2 * lam ** 2) - 5 * math.log(2 * math.pi * lam ** 2)
+    assert math.isclose(oracle.log_lik_eq8(obs, cal, Nn, mu, lam), want, rel_tol=1e-13)
+
+
+def test_const_n_closed_form():
+    # const(n) = -((n-2)/2) log 2pi + ((n-5)/2) log 2 + lgamma((n-3)/2); n = 5 -> lgamma(1) = 0
+    assert math.isclose(oracle.const_n(5), -1.5 * math.log(2 * math.pi), rel_tol=1e-14)
+    assert math.isclose(oracle.const_n(7), -2.5 * math.log(2 * math.pi) + math.log(2.0), rel_tol=1e-14)   # lgamma(2)=0
+
+
+def test_closed_form_invariances():
+    rng = np.random.default_rng(77)
+    n = 64
+    obs, cal = rng.normal(size=n) + 2.0, rng.normal(size=n)
+    base = oracle.log_post_c1(*_sums(obs, cal))
+    al, be, ga, de = 3.7, -11.0, -0.25, 5.0
+    # I_obs -> alpha I_obs + beta : log P shifts by -(n-3) log|alpha|
+    assert math.isclose(oracle.log_post_c1(*_sums(al * obs + be, cal)), base - (n - 3) * math.log(abs(al)), abs_tol=1e-9)
+    # I1 -> gamma I1 + delta : log P shifts by -log|gamma|   (N < 0 allowed, R1)
+    assert math.isclose(oracle.log_post_c1(*_sums(obs, ga * cal + de)), base - math.log(abs(ga)), abs_tol=1e-9)
+    # joint permutation of pixels (e.g. a joint circular shift) changes nothing
+    p = rng.permutation(n)
+    assert math.isclose(oracle.log_post_c1(*_sums(obs[p], cal[p])), base, abs_tol=1e-10)
+
+
+def test_c1_c2_agree_at_workload_scale():
+    wl = W.build_workload("tiny_mini")
+    s = wl["spec"]
+    I1 = oracle.calc_image(wl["models"][0], wl["quats"][0], wl["ctfs"][0], s.n_pix, s.pixel_A)
+    img = wl["images"][0].astype(np.float64)
+    n, Co, Coo, Cc, Ccc, _ = _sums(img.ravel(), I1.ravel())
+    C = oracle.cross_corr_direct(img, I1, 2)
+    for cco in C.ravel():
+        assert abs(oracle.log_post_c1(n, Co, Coo, Cc, Ccc, cco) - oracle.log_post_c2(n, Co, Coo, Cc, Ccc, cco)) < 1e-8
+
+
+# ------------------------------------------------------------------ projection (Eq. 1; R10-R12)
+def test_projection_total_mass_converges_to_sum_of_weights():
+    rng = np.random.default_rng(3)
+    xyz = rng.uniform(-20, 20, size=(50, 3)); rad = rng.uniform(1.0, 2.0, 50); wt = rng.uniform(1, 8, 50)
+    q = np.array([0.3, -0.5, 0.2, 0.78]); q /= np.linalg.norm(q)
+    m4 = oracle.project_atoms(xyz, rad, wt, q, 64, 1.0, 4).sum()
+    m32 = oracle.project_atoms(xyz, rad, wt, q, 64, 1.0, 32).sum()
+    assert abs(m4 / wt.sum() - 1) < 0.04
+    assert abs(m32 / wt.sum() - 1) < 2e-3
+
+
+def test_projection_single_sphere_values():
+    # sphere inside one pixel: that pixel holds all the mass; big sphere: centre pixel ~ chord * px^2 * density
+    N, px = 16, 4.0
+    I0 = oracle.project_atoms([[0.3, -0.2, 5.0]], [1.0], [2.5], [1, 0, 0, 0], N, px, 64)
+    assert abs(I0[N // 2, N // 2] - 2.5) < 5e-3 and abs(I0.sum() - I0[N // 2, N // 2]) < 1e-12
+    R = 30.0
+    I0 = oracle.project_atoms([[0.0, 0.0, 0.0]], [R], [1.0], [1, 0, 0, 0], 64, 1.0, 8)
+    assert math.isclose(I0[32, 32], 2 * R / (4 / 3 * math.pi * R ** 3), rel_tol=2e-4)
+    # 4-fold symmetric footprint about pixel (N/2, N/2) (R11)
+    assert np.allclose(I0[32 - 5:32 + 6, 32 - 5:32 + 6], I0[32 - 5:32 + 6, 32 - 5:32 + 6].T, atol=1e-15)
+    assert np.allclose(I0[32 - 5:32 + 6, 32 - 5:32 + 6], I0[32 - 5:32 + 6, 32 - 5:32 + 6][::-1, ::-1], atol=1e-15)
+
+
+def test_projection_rotations():
+    rng = np.random.default_rng(4)
+    xyz = rng.uniform(-10, 10, size=(30, 3)); rad = np.full(30, 1.5); wt = np.ones(30)
+    N, px = 32, 2.0
+    I_id = oracle.project_atoms(xyz, rad, wt, [1, 0, 0, 0], N, px)
+    # 180 deg about z: (x,y) -> (-x,-y): I0(j,k) -> I0(N-j, N-k)  (indices mod N; atoms are away from the border)
+    I_z180 = oracle.project_atoms(xyz, rad, wt, [0, 0, 0, 1], N, px)
+    idx = (-np.arange(N)) % N
+    assert np.allclose(I_z180, I_id[np.ix_(idx, idx)], atol=1e-13)
+    # active rotation (R12): +90 deg about z sends x -> y.  An atom at (+6,0,0) must land at y = +6 -> k = N/2 + 3
+    I = oracle.project_atoms([[6.0, 0, 0]], [1.0], [1.0], [math.cos(math.pi / 4), 0, 0, math.sin(math.pi / 4)], N, px)
+    k, j = np.unravel_index(np.argmax(I), I.shape)
+    assert (j, k) == (N // 2, N // 2 + 3)
+    # projection along z' : rotating about x by +90 deg sends y -> z (drops out) and z -> -y
+    I = oracle.project_atoms([[0, 0, 8.0]], [1.0], [1.0], [math.cos(math.pi / 4), math.sin(math.pi / 4), 0, 0], N, px)
+    k, j = np.unravel_index(np.argmax(I), I.shape)
+    assert (j, k) == (N // 2, N // 2 - 4)
+    # quaternion -> matrix against the Euler ZYZ product R = Rz(a) Ry(b) Rz(g)
+    a, b, g = 0.4, 1.1, -2.0
+    def rz(t): return np.array([[math.cos(t), -math.sin(t), 0], [math.sin(t), math.cos(t), 0], [0, 0, 1]])
+    def ry(t): return np.array([[math.cos(t), 0, math.sin(t)], [0, 1, 0], [-math.sin(t), 0, math.cos(t)]])
+    assert np.allclose(oracle.quat_to_matrix(W.euler_zyz_to_quat(a, b, g)), rz(a) @ ry(b) @ rz(g), atol=1e-14)
+
+
+# ------------------------------------------------------------------ CTF (Eqs. 4-6; R8, R9)
+def test_ctf_special_cases():
+    rng = np.random.default_rng(8)
+    I0 = rng.normal(size=(8, 8))
+    # "CTF-free" (a=0, A=1, b=0): CTF Env == -1  ->  I1 = -I0  (R9)
+    assert np.allclose(oracle.apply_ctf(I0, 1.5, 0.0, 1.0, 0.0), -I0, atol=1e-13)
+    # A = 0: pure sine, zeros at a s^2/2 = m pi
+    a = 31.0
+    for m in (1, 2, 3):
+        assert abs(oracle.ctf_env(2 * m * math.pi / a, a, 0.0, 0.0)) < 1e-13
+    # s = 0: CTF = -A
+    assert math.isclose(oracle.ctf_env(0.0, a, 0.1, 0.7), -0.1)
+    # envelope
+    assert math.isclose(oracle.ctf_env(3.0, 0.0, 1.0, 0.4), -math.exp(-0.6), rel_tol=1e-14)
+
+
+def test_eq5_equals_eq6_psf_convolution():
+    rng = np.random.default_rng(9)
+    I0 = rng.normal(size=(8, 8))
+    a, A, b = 9.0, 0.2, 0.8
+    assert np.allclose(oracle.apply_ctf(I0, 1.5, a, A, b), oracle.apply_psf_realspace(I0, 1.5, a, A, b), atol=1e-12)
+
+
+def test_ctf_matches_library_fft_route():
+    rng = np.random.default_rng(10)
+    N, px = 12, 1.5
+    I0 = rng.normal(size=(N, N))
+    a, A, b = 31.3, 0.1, 0.63
+    want = np.fft.irfft2(np.fft.rfft2(I0) * simulate.ctf_image(N, px, a, A, b), s=(N, N))
+    assert np.allclose(oracle.apply_ctf(I0, px, a, A, b), want, atol=1e-12)
+
+
+def test_defocus_constants_r8_r9():
+    # lambda_e(300 kV) = 0.019687 A; 1 um -> a = 31.33 A^2; B = 50 A^2 -> b = 0.633 A^2
+    assert abs(W.generate.electron_wavelength_A(300.0) - 0.019687) < 1e-6
+    a, b = W.ctf_from_defocus(1.0, 50.0, 300.0)
+    assert abs(a - 31.33) < 5e-3 and abs(b - 0.6333) < 1e-4
+
+
+# ------------------------------------------------------------------ density model / Fourier slice (R21)
+def _blob_map(n, vox, centres, sig):
+    ax = (np.arange(n) - n // 2) * vox
+    Z, Y, X = np.meshgrid(ax, ax, ax, indexing="ij")
+    rho = np.zeros((n, n, n))
+    for c in centres:
+        rho += np.exp(-0.5 * ((X - c[0]) ** 2 + (Y - c[1]) ** 2 + (Z - c[2]) ** 2) / sig ** 2)
+    return rho
+
+
+def test_fourier_slice_identity_is_dft_of_z_sum():
+    n, vox = 16, 1.5
+    rho = _blob_map(n, vox, [[2.0, -1.0, 3.0], [-3.0, 2.5, -1.0]], 2.0)
+    F = oracle.fourier_slice(oracle.dft3(rho), vox, [1, 0, 0, 0])
+    want = np.fft.fft2(rho.sum(0) * vox)
+    h = n // 2
+    keep = np.ones((n, n), bool); keep[h, :] = False; keep[:, h] = False
+    assert np.allclose(F[keep], want[keep], atol=1e-10)
+    assert np.all(F[~keep] == 0)
+
+
+def test_fourier_slice_axis_rotation_is_index_permutation():
+    n, vox = 16, 1.0
+    rho = _blob_map(n, vox, [[2.0, -1.0, 3.0], [-3.0, 2.0, -1.0], [0.5, 3.0, 2.0]], 1.5)
+    V = oracle.dft3(rho)
+    # +90 deg about z, active: rho'(x,y,z) = rho(y,-x,z).  Projection image I'(x,y) = I(y,-x).
+    q = [math.cos(math.pi / 4), 0, 0, math.sin(math.pi / 4)]
+    F_rot, F_id = oracle.fourier_slice(V, vox, q), oracle.fourier_slice(V, vox, [1, 0, 0, 0])
+    # I'(x,y) = I(y,-x)  =>  F'(l', m') = F(m', -l')   (arrays are [y-frequency][x-frequency]).
+    # sqrt(1/2) is not exact, so bins with |l'| or |m'| = n/2 - 1 may fall just outside the |k_i| <= n/2 - 1 rule: skip them
+    h = n // 2
+    for ls in range(-h + 2, h - 1):
+        for ms in range(-h + 2, h - 1):
+            assert abs(F_rot[ms % n, ls % n] - F_id[(-ls) % n, ms % n]) < 1e-9
+
+
+def test_fourier_slice_general_orientation_vs_analytic_blobs():
+    # loose pin (interpolation error, not a parity bound): projected Gaussians at actively rotated centres (R12)
+    n, vox, sig = 32, 1.5, 3.0
+    centres = np.array([[5.0, -3.0, 4.0], [-6.0, 2.0, -2.0], [1.0, 7.0, 3.0]])
+    rho = _blob_map(n, vox, centres, sig)
+    q = W.euler_zyz_to_quat(0.7, 1.0, -0.4)
+    img = -oracle.apply_ctf_spectrum(oracle.fourier_slice(oracle.dft3(rho), vox, q), vox, 0.0, 1.0, 0.0)
+    R = oracle.quat_to_matrix(q)
+    rc = centres @ R.T
+    ax = (np.arange(n) - n // 2) * vox
+    Y, X = np.meshgrid(ax, ax, indexing="ij")
+    want = np.zeros((n, n))
+    for c in rc:
+        want += math.sqrt(2 * math.pi) * sig * np.exp(-0.5 * ((X - c[0]) ** 2 + (Y - c[1]) ** 2) / sig ** 2)
+    assert np.corrcoef(img.ravel(), want.ravel())[0, 1] > 0.99
+    # the transposed (passive) convention must NOT fit
+    wrong = np.zeros((n, n))
+    for c in centres @ R:
+        wrong += math.sqrt(2 * math.pi) * sig * np.exp(-0.5 * ((X - c[0]) ** 2 + (Y - c[1]) ** 2) / sig ** 2)
+    assert np.corrcoef(img.ravel(), wrong.ravel())[0, 1] < 0.9
+
+
+# ------------------------------------------------------------------ Eq. 9 on the grid (R7, R15, R16)
+def test_planted_truth_is_the_argmax():
+    # north_star check 2: a noiseless, CTF-free image at a grid orientation and shift scores its maximum exactly there
+    spec = W.get_spec("tiny")
+    model = W.make_atom_model(spec)
+    quats = W.generate.orientation_grid(spec)[::5]           # 13 orientations
+    ctfs = np.array([[0.0, 1.0, 0.0]])
+    D, N, px = 3, spec.n_pix, spec.pixel_A
+    o_true, dx, dy = 7, 2, -3
+    I1 = oracle.calc_image(model, quats[o_true], ctfs[0], N, px)
+    img = (1.7 * np.roll(I1, shift=(-dy, -dx), axis=(0, 1)) + 0.3).astype(np.float32)[None]
+    st = oracle.run_model(model, N, px, D, quats, ctfs, img)
+    o, c, bx, by = oracle.unflatten(st.best_flat, 1, D)
+    assert (o[0], c[0], bx[0], by[0]) == (o_true, 0, dx, dy)
+    assert st.best[0] - st.second[0] > 100.0
+
+
+def test_log_sum_exp_equals_brute_force_and_chunking_is_exact():
+    wl = W.build_workload("tiny_mini")
+    s = wl["spec"]
+    m = wl["models"][0]
+    st = oracle.run_model(m, s.n_pix, s.pixel_A, s.max_shift, wl["quats"], wl["ctfs"], wl["images"])
+    # brute force: all terms from per-pair maps, summed in long double
+    logw = oracle.uniform_logw(len(wl["quats"]), len(wl["ctfs"]), s.max_shift)
+    terms = [[] for _ in range(s.n_images)]
+    for o, q in enumerate(wl["quats"]):
+        for c, ctf in enumerate(wl["ctfs"]):
+            I1 = oracle.calc_image(m, q, ctf, s.n_pix, s.pixel_A)
+            for w in range(s.n_images):
+                terms[w].append(oracle.shift_map(wl["images"][w], I1, s.max_shift, logw).ravel())
+    for w in range(s.n_images):
+        t = np.concatenate(terms[w]).astype(np.longdouble)
+        want = float(t.max() + np.log(np.exp(t - t.max()).sum()))
+        assert abs(st.log_posterior()[w] - want) < 1e-10
+        assert st.best_flat[w] == int(np.argmax(t)) and st.best[w] == float(t.max())
+    # chunked over orientations == one shot, bit for bit
+    st2 = oracle.run_model(m, s.n_pix, s.pixel_A, s.max_shift, wl["quats"], wl["ctfs"], wl["images"], o_end=2)
+    st2 = oracle.run_model(m, s.n_pix, s.pixel_A, s.max_shift, wl["quats"], wl["ctfs"], wl["images"], o_begin=2, state=st2)
+    assert np.array_equal(st2.log_posterior(), st.log_posterior()) and np.array_equal(st2.best_flat, st.best_flat)
+    # tier B agrees with the definition
+    st3 = oracle.run_model(m, s.n_pix, s.pixel_A, s.max_shift, wl["quats"], wl["ctfs"], wl["images"], tier=1)
+    assert np.abs(st3.log_posterior() - st.log_posterior()).max() < 1e-8
+    assert np.array_equal(st3.best_flat, st.best_flat)
+
+
+def test_equal_terms_sum_to_the_term():
+    # R7: with uniform weights, identical terms -> LSE equals the term (weights sum to one)
+    st = oracle.RunState(1)
+    N = 8
+    model = dict(kind="atoms", xyz=np.zeros((1, 3)), radius=np.array([3.0]), weight=np.array([1.0]), Kq=4)
+    img = RNG.normal(size=(1, N, N)).astype(np.float32)
+    # a sphere at the origin looks the same from every orientation about z; D = 0 -> one shift
+    quats = np.array([[math.cos(t / 2), 0, 0, math.sin(t / 2)] for t in (0.0, math.pi / 2, math.pi, 3 * math.pi / 2)])
+    st = oracle.run_model(model, N, 1.0, 0, quats, np.array([[0.0, 1.0, 0.0]]), img)
+    one = oracle.run_model(model, N, 1.0, 0, quats[:1], np.array([[0.0, 1.0, 0.0]]), img)
+    assert abs(st.log_posterior()[0] - one.log_posterior()[0]) < 1e-10
+    assert st.best_flat[0] == 0            # exact ties keep the lowest flat index (R15)

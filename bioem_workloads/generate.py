@@ -166,6 +166,12 @@ def build_workload(name_or_spec, with_images: bool = True, **overrides):
         models = [make_density_model(spec)]
     quats = orientation_grid(spec)
     ctfs = ctf_grid(spec)
+    # The C ABI takes float32 models / grids: round here, once, so that every consumer sees identical numbers.
+    r32 = lambda a: np.ascontiguousarray(a, dtype=np.float32).astype(np.float64)
+    for m in models:
+        if m["kind"] == "atoms":
+            m["xyz"], m["radius"], m["weight"] = r32(m["xyz"]), r32(m["radius"]), r32(m["weight"])
+    quats, ctfs = r32(quats), r32(ctfs)
     wl = dict(spec=spec, models=models, quats=quats, ctfs=ctfs)
     if with_images:
         rng = _rng(spec, "images")

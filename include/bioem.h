@@ -1,0 +1,114 @@
+/*
+ * bioem.h -- C ABI of the B200-native BioEM hot path (arXiv:1609.06634).
+ *
+ * The library scores every experimental particle image against every calculated image
+ * (model x orientation x CTF parameter set) over all in-plane centre displacements and
+ * accumulates the marginal log-posterior per (image, model), with the maximising grid
+ * parameters (paper sections 2-3; citations "P:<line>" are lines of PAPER.md, "R<k>" the
+ * readings of DESIGN.md section 3).
+ *
+ * Conventions
+ *   - every call returns an int: 0 = ok, negative = one of the BIOEM_E* codes; nothing throws or
+ *     aborts across the ABI; bioem_last_error(ctx) returns a ctx-owned, NUL-terminated message.
+ *   - INPUTS ARE COPIED: the caller keeps ownership of every pointer passed in and may free it
+ *     after the call returns.  OUTPUTS ARE CALLER-ALLOCATED host arrays.
+ *   - pointers are HOST pointers unless the argument list has an `is_device` flag set to 1, in
+ *     which case they are CUDA device pointers on the context's device (e.g. torch data_ptr()).
+ *   - all device work is enqueued on the cudaStream_t given at creation (NULL = default stream,
+ *     e.g. torch.cuda.current_stream().cuda_stream); bioem_run returns after enqueueing and
+ *     bioem_get_* synchronise that stream.
+ *   - images are row-major [k][j] = [y][x], x fastest (R11); pixel (N/2, N/2) is the model
+ *     origin.
+ *   - there is NO CPU fallback: without a CUDA device bioem_create fails with BIOEM_ECUDA.
+ */
+#ifndef BIOEM_H
+#define BIOEM_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define BIOEM_OK            0
+#define BIOEM_EBADARG      (-1)   /* NULL / out-of-range argument                         */
+#define BIOEM_EBADSTATE    (-2)   /* call order: something required has not been set yet   */
+#define BIOEM_EOOM         (-3)   /* device allocation failed                              */
+#define BIOEM_ECUDA        (-4)   /* CUDA runtime error (message in bioem_last_error)      */
+#define BIOEM_EUNSUPPORTED (-5)   /* image size / grid size the kernels are not built for  */
+
+#define BIOEM_TOPK 8              /* candidates per (image, model) re-scored in FP64 (a7)  */
+
+typedef struct bioem_ctx bioem_ctx;
+
+/* Create a context on CUDA device `device`; `cuda_stream` is a cudaStream_t (may be NULL). */
+int bioem_create(bioem_ctx **out, int device, void *cuda_stream);
+int bioem_destroy(bioem_ctx *ctx);
+const char *bioem_last_error(const bioem_ctx *ctx);
+
+/* Square images of n_pix x n_pix pixels of pixel_size_A Angstrom.  Supported n_pix:
+ * 64, 128, 224, 256 (BIOEM_EUNSUPPORTED otherwise).  Clears images, models stay. */
+int bioem_set_image_geometry(bioem_ctx *ctx, int n_pix, float pixel_size_A);
+
+/* Models.  Atoms: uniform-density spheres, centre xyz_A [n][3], radius_A [n], total
+ * weight [n] (R10); projected by Eq. 1 with 4x4 mid-point sub-sampling per pixel.
+ * Density: cube of n_vox^3 voxels rho[z][y][x] of voxel_A Angstrom, origin at voxel n_vox/2,
+ * projected as a trilinear central section of its 3-D DFT (R21); requires n_vox == n_pix and
+ * voxel_A == pixel_size_A.  *model_id receives 0, 1, ... in order of addition. */
+int bioem_clear_models(bioem_ctx *ctx);
+int bioem_add_model_atoms(bioem_ctx *ctx, int n_atoms, const float *xyz_A, const float *radius_A,
+                          const float *weight, int *model_id);
+int bioem_add_model_density(bioem_ctx *ctx, int n_vox, float voxel_A, const float *rho, int *model_id);
+
+/* Orientation grid: n unit quaternions (w,x,y,z), ACTIVE rotation r' = R(q) r,
+ * projection along z' (R12).  log_prior [n] or NULL = uniform (-log n) (R7). */
+int bioem_set_orientations_quat(bioem_ctx *ctx, int n, const float *q_wxyz, const float *log_prior);
+
+/* CTF / envelope grid: CTF(s|a,A) Env(s|b), s = 2 pi x spatial frequency, a and b in A^2,
+ * 0 <= A <= 1.  log_prior [n] or NULL = uniform. */
+int bioem_set_ctf_grid(bioem_ctx *ctx, int n, const float *a_A2, const float *A, const float *b_A2,
+                       const float *log_prior);
+
+/* Helper (R8, R9): defocus [um], B-factor [A^2], voltage [kV] -> a = lambda_e dz / (2 pi), b = B / (8 pi^2). */
+int bioem_ctf_from_defocus(float defocus_um, float bfactor_A2, float kV, float *a_A2, float *b_A2);
+
+/* Centre displacements (Eq. 7): all integer (dx,dy) with |dx|,|dy| <= max_shift_px, circular
+ * (R5, R6); 2*max_shift_px + 1 <= n_pix. */
+int bioem_set_shift_range(bioem_ctx *ctx, int max_shift_px);
+
+/* Replace the image stack: n_img images [n][N][N] float32 (host, or device if is_device). Runs the
+ * observed-image preprocessing (a0: mean removal, spectra, C_o / C_oo sums). */
+int bioem_push_images(bioem_ctx *ctx, int n_img, const float *pixels, int is_device);
+
+/* The hot path: all models x orientations x CTFs x shifts against all images (Eq. 9 on the grid,
+ * P:126; Eqs. 11-12; closed-form marginal over N, mu, lambda).  Requires geometry,
+ * >= 1 model, orientations, CTFs, a shift range and images (else BIOEM_EBADSTATE). */
+int bioem_run(bioem_ctx *ctx);
+
+/* Results of the last bioem_run, each [n_img][n_model] (image-major):
+ *   log_posterior = log sum_theta w(theta) P_m,omega(theta), w uniform unless priors were given (R7);
+ *   best = grid parameters of the largest term (R15: exact ties -> lowest flat index) and its value. */
+int bioem_get_log_posterior(bioem_ctx *ctx, double *out);
+int bioem_get_best(bioem_ctx *ctx, int32_t *orient_idx, int32_t *ctf_idx, int32_t *dx, int32_t *dy,
+                   double *best_log_p);
+
+/* ---- test / debug entry points (not on the measured path) ---- */
+/* real-space calculated image I1 of (model, orient, ctf) [N][N] ("synthetic map"). */
+int bioem_debug_calc_image(bioem_ctx *ctx, int model, int orient, int ctf, float *out_real);
+/* per-shift terms log P + log w of one (image, calc image) pair, [dy+D][dx+D]:
+ * _map: as the FP32 fused kernel computes them (a4+a5); _map_f64: as the FP64 re-scoring kernel (a7) does. */
+int bioem_debug_shift_map(bioem_ctx *ctx, int img, int model, int orient, int ctf, double *out);
+int bioem_debug_shift_map_f64(bioem_ctx *ctx, int img, int model, int orient, int ctf, double *out);
+/* FP32-only result of the last run (before FP64 re-scoring), [n_img][n_model]. */
+int bioem_debug_log_posterior_f32(bioem_ctx *ctx, double *out);
+/* CUDA-event times of the last bioem_run [ms]: whole run, fused kernel only; number of kernel launches. */
+int bioem_get_timing(bioem_ctx *ctx, double *ms_total, double *ms_fused_kernel);
+int bioem_get_launch_count(bioem_ctx *ctx, int64_t *n_launches, int64_t *n_fused_launches);
+/* FP32 FMA rate of this device measured with a register-resident FFMA loop [TFLOP/s] and the SM clock [MHz]
+ * seen while it ran (bench.py's "alu" roofline denominator). */
+int bioem_measure_fp32_peak(bioem_ctx *ctx, double *tflops, double *sm_mhz);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* BIOEM_H */

@@ -1,0 +1,620 @@
+// bioem_api.cu -- the C ABI declared in include/bioem.h: context, argument checking, device buffers, and the
+// orchestration of one bioem_run (precompute a1-a3 -> fused a4-a6 -> merge -> FP64 re-score a7 -> results).
+#include "../../include/bioem.h"
+#include "common.cuh"
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+using namespace bioem;
+
+namespace {
+
+struct DBuf {
+    void *p = nullptr;
+    size_t cap = 0;
+    cudaError_t ensure(size_t bytes)
+    {
+        if (bytes <= cap) return cudaSuccess;
+        if (p) { cudaFree(p); p = nullptr; cap = 0; }
+        cudaError_t e = cudaMalloc(&p, bytes ? bytes : 1);
+        if (e == cudaSuccess) cap = bytes;
+        return e;
+    }
+    void release() { if (p) cudaFree(p); p = nullptr; cap = 0; }
+    template <typename T> T *as() const { return reinterpret_cast<T *>(p); }
+};
+
+struct Model {
+    int kind = 0;                 // 0 atoms, 1 density
+    int n_atoms = 0;
+    DBuf xyz, rad, wt;            // double
+    double sum_abs_w = 0.0;
+    int n_vox = 0;
+    double voxel = 0.0;
+    DBuf rho;                     // float [n_vox^3]
+};
+
+}  // namespace
+
+struct bioem_ctx {
+    int device = 0;
+    cudaStream_t stream = nullptr;
+    std::string err;
+    int N = 0;
+    double px = 0.0;
+    int D = -1;
+    std::vector<Model> models;
+    int n_orient = 0;
+    DBuf rot, lp_orient;          // double [O][9], double [O]
+    bool has_lp_orient = false;
+    int n_ctf = 0;
+    DBuf ctf_a, ctf_A, ctf_b, lp_ctf;
+    bool has_lp_ctf = false;
+    int n_img = 0;
+    DBuf Ohat64, Ohat32, Dw, beta;
+    // run state
+    bool ran = false;
+    int run_models = 0, run_orient = 0, run_ctf = 0, run_D = 0, run_img = 0;
+    DBuf F064, F032, K64, K32, Tc64, h64, alpha32, h32;
+    DBuf part_m, part_s, part_top, m32, s32, top, g64;
+    DBuf logp, logp32, best, best_logp;
+    DBuf scratch_a, scratch_b, scratch_c, dump;
+    cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
+    int64_t launches = 0, fused_launches = 0;
+};
+
+#define CK(call)                                                                                     \
+    do {                                                                                             \
+        cudaError_t e__ = (call);                                                                    \
+        if (e__ != cudaSuccess) {                                                                    \
+            ctx->err = std::string(#call) + ": " + cudaGetErrorString(e__);                          \
+            cudaGetLastError();                                                                      \
+            return e__ == cudaErrorMemoryAllocation ? BIOEM_EOOM : BIOEM_ECUDA;                      \
+        }                                                                                            \
+    } while (0)
+
+#define FAIL(code, msg)          \
+    do {                         \
+        ctx->err = (msg);        \
+        return (code);           \
+    } while (0)
+
+static bool supported_n(int n) { return n == 64 || n == 128 || n == 224 || n == 256; }
+
+extern "C" {
+
+int bioem_create(bioem_ctx **out, int device, void *cuda_stream)
+{
+    if (!out) return BIOEM_EBADARG;
+    *out = nullptr;
+    int count = 0;
+    if (cudaGetDeviceCount(&count) != cudaSuccess || device < 0 || device >= count) { cudaGetLastError(); return BIOEM_ECUDA; }
+    if (cudaSetDevice(device) != cudaSuccess) { cudaGetLastError(); return BIOEM_ECUDA; }
+    bioem_ctx *ctx = new bioem_ctx();
+    ctx->device = device;
+    ctx->stream = reinterpret_cast<cudaStream_t>(cuda_stream);
+    for (int i = 0; i < 4; ++i)
+        if (cudaEventCreate(&ctx->ev[i]) != cudaSuccess) { delete ctx; return BIOEM_ECUDA; }
+    *out = ctx;
+    return BIOEM_OK;
+}
+
+int bioem_destroy(bioem_ctx *ctx)
+{
+    if (!ctx) return BIOEM_EBADARG;
+    cudaSetDevice(ctx->device);
+    cudaStreamSynchronize(ctx->stream);
+    for (auto &m : ctx->models) { m.xyz.release(); m.rad.release(); m.wt.release(); m.rho.release(); }
+    DBuf *all[] = {&ctx->rot, &ctx->lp_orient, &ctx->ctf_a, &ctx->ctf_A, &ctx->ctf_b, &ctx->lp_ctf, &ctx->Ohat64, &ctx->Ohat32, &ctx->Dw,
+                   &ctx->beta, &ctx->F064, &ctx->F032, &ctx->K64, &ctx->K32, &ctx->Tc64, &ctx->h64, &ctx->alpha32, &ctx->h32,
+                   &ctx->part_m, &ctx->part_s, &ctx->part_top, &ctx->m32, &ctx->s32, &ctx->top, &ctx->g64, &ctx->logp, &ctx->logp32,
+                   &ctx->best, &ctx->best_logp, &ctx->scratch_a, &ctx->scratch_b, &ctx->scratch_c, &ctx->dump};
+    for (DBuf *b : all) b->release();
+    for (int i = 0; i < 4; ++i) if (ctx->ev[i]) cudaEventDestroy(ctx->ev[i]);
+    delete ctx;
+    return BIOEM_OK;
+}
+
+const char *bioem_last_error(const bioem_ctx *ctx) { return ctx ? ctx->err.c_str() : "null context"; }
+
+int bioem_set_image_geometry(bioem_ctx *ctx, int n_pix, float pixel_size_A)
+{
+    if (!ctx) return BIOEM_EBADARG;
+    if (!(pixel_size_A > 0.f)) FAIL(BIOEM_EBADARG, "pixel_size_A must be > 0");
+    if (!supported_n(n_pix)) FAIL(BIOEM_EUNSUPPORTED, "n_pix must be one of 64, 128, 224, 256");
+    ctx->N = n_pix;
+    ctx->px = (double)pixel_size_A;
+    ctx->n_img = 0;
+    ctx->ran = false;
+    return BIOEM_OK;
+}
+
+int bioem_clear_models(bioem_ctx *ctx)
+{
+    if (!ctx) return BIOEM_EBADARG;
+    cudaSetDevice(ctx->device);
+    cudaStreamSynchronize(ctx->stream);
+    for (auto &m : ctx->models) { m.xyz.release(); m.rad.release(); m.wt.release(); m.rho.release(); }
+    ctx->models.clear();
+    ctx->ran = false;
+    return BIOEM_OK;
+}
+
+static int upload_doubles(bioem_ctx *ctx, DBuf &buf, const std::vector<double> &v)
+{
+    CK(buf.ensure(v.size() * sizeof(double)));
+    CK(cudaMemcpyAsync(buf.p, v.data(), v.size() * sizeof(double), cudaMemcpyHostToDevice, ctx->stream));
+    CK(cudaStreamSynchronize(ctx->stream));       // v is a temporary
+    return BIOEM_OK;
+}
+
+int bioem_add_model_atoms(bioem_ctx *ctx, int n_atoms, const float *xyz_A, const float *radius_A, const float *weight, int *model_id)
+{
+    if (!ctx) return BIOEM_EBADARG;
+    if (n_atoms <= 0 || !xyz_A || !radius_A || !weight) FAIL(BIOEM_EBADARG, "add_model_atoms: empty model or NULL array");
+    CK(cudaSetDevice(ctx->device));
+    std::vector<double> x(3 * (size_t)n_atoms), r(n_atoms), w(n_atoms);
+    double sw = 0.0;
+    for (int i = 0; i < n_atoms; ++i) {
+        if (!(radius_A[i] > 0.f)) FAIL(BIOEM_EBADARG, "add_model_atoms: radius must be > 0");
+        x[3 * i] = xyz_A[3 * i]; x[3 * i + 1] = xyz_A[3 * i + 1]; x[3 * i + 2] = xyz_A[3 * i + 2];
+        r[i] = radius_A[i]; w[i] = weight[i];
+        sw += std::fabs((double)weight[i]);
+    }
+    ctx->models.emplace_back();
+    Model &m = ctx->models.back();
+    m.kind = 0; m.n_atoms = n_atoms; m.sum_abs_w = sw;
+    int rc;
+    if ((rc = upload_doubles(ctx, m.xyz, x)) || (rc = upload_doubles(ctx, m.rad, r)) || (rc = upload_doubles(ctx, m.wt, w))) {
+        ctx->models.pop_back();
+        return rc;
+    }
+    if (model_id) *model_id = (int)ctx->models.size() - 1;
+    ctx->ran = false;
+    return BIOEM_OK;
+}
+
+int bioem_add_model_density(bioem_ctx *ctx, int n_vox, float voxel_A, const float *rho, int *model_id)
+{
+    if (!ctx) return BIOEM_EBADARG;
+    if (!rho || !(voxel_A > 0.f)) FAIL(BIOEM_EBADARG, "add_model_density: NULL map or voxel size <= 0");
+    if (!supported_n(n_vox)) FAIL(BIOEM_EUNSUPPORTED, "add_model_density: n_vox must be one of 64, 128, 224, 256");
+    CK(cudaSetDevice(ctx->device));
+    ctx->models.emplace_back();
+    Model &m = ctx->models.back();
+    m.kind = 1; m.n_vox = n_vox; m.voxel = (double)voxel_A;
+    size_t bytes = (size_t)n_vox * n_vox * n_vox * sizeof(float);
+    cudaError_t e = m.rho.ensure(bytes);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(m.rho.p, rho, bytes, cudaMemcpyHostToDevice, ctx->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+    if (e != cudaSuccess) { m.rho.release(); ctx->models.pop_back(); CK(e); }
+    if (model_id) *model_id = (int)ctx->models.size() - 1;
+    ctx->ran = false;
+    return BIOEM_OK;
+}
+
+int bioem_set_orientations_quat(bioem_ctx *ctx, int n, const float *q, const float *log_prior)
+{
+    if (!ctx) return BIOEM_EBADARG;
+    if (n <= 0 || !q) FAIL(BIOEM_EBADARG, "set_orientations_quat: n <= 0 or NULL");
+    CK(cudaSetDevice(ctx->device));
+    std::vector<double> R(9 * (size_t)n), lp;
+    for (int i = 0; i < n; ++i) {
+        double w = q[4 * i], x = q[4 * i + 1], y = q[4 * i + 2], z = q[4 * i + 3];
+        double nr = std::sqrt(w * w + x * x + y * y + z * z);
+        if (!(nr > 0.0)) FAIL(BIOEM_EBADARG, "set_orientations_quat: zero quaternion");
+        w /= nr; x /= nr; y /= nr; z /= nr;
+        double *r = &R[9 * (size_t)i];                       // active rotation r' = R r (R12)
+        r[0] = 1 - 2 * (y * y + z * z); r[1] = 2 * (x * y - w * z);     r[2] = 2 * (x * z + w * y);
+        r[3] = 2 * (x * y + w * z);     r[4] = 1 - 2 * (x * x + z * z); r[5] = 2 * (y * z - w * x);
+        r[6] = 2 * (x * z - w * y);     r[7] = 2 * (y * z + w * x);     r[8] = 1 - 2 * (x * x + y * y);
+    }
+    int rc = upload_doubles(ctx, ctx->rot, R);
+    if (rc) return rc;
+    ctx->has_lp_orient = log_prior != nullptr;
+    if (log_prior) {
+        lp.assign(log_prior, log_prior + n);
+        if ((rc = upload_doubles(ctx, ctx->lp_orient, lp))) return rc;
+    }
+    ctx->n_orient = n;
+    ctx->ran = false;
+    return BIOEM_OK;
+}
+
+int bioem_set_ctf_grid(bioem_ctx *ctx, int n, const float *a, const float *A, const float *b, const float *log_prior)
+{
+    if (!ctx) return BIOEM_EBADARG;
+    if (n <= 0 || !a || !A || !b) FAIL(BIOEM_EBADARG, "set_ctf_grid: n <= 0 or NULL");
+    CK(cudaSetDevice(ctx->device));
+    std::vector<double> va(n), vA(n), vb(n), lp;
+    for (int i = 0; i < n; ++i) {
+        if (!(A[i] >= 0.f && A[i] <= 1.f)) FAIL(BIOEM_EBADARG, "set_ctf_grid: amplitude contrast A must be in [0,1]");
+        va[i] = a[i]; vA[i] = A[i]; vb[i] = b[i];
+    }
+    int rc;
+    if ((rc = upload_doubles(ctx, ctx->ctf_a, va)) || (rc = upload_doubles(ctx, ctx->ctf_A, vA)) || (rc = upload_doubles(ctx, ctx->ctf_b, vb)))
+        return rc;
+    ctx->has_lp_ctf = log_prior != nullptr;
+    if (log_prior) {
+        lp.assign(log_prior, log_prior + n);
+        if ((rc = upload_doubles(ctx, ctx->lp_ctf, lp))) return rc;
+    }
+    ctx->n_ctf = n;
+    ctx->ran = false;
+    return BIOEM_OK;
+}
+
+int bioem_ctf_from_defocus(float defocus_um, float bfactor_A2, float kV, float *a_A2, float *b_A2)
+{
+    if (!a_A2 || !b_A2 || !(kV > 0.f)) return BIOEM_EBADARG;
+    const double V = (double)kV * 1e3;
+    const double lambda = 12.2643 / std::sqrt(V + 0.97845e-6 * V * V);          // electron wavelength [A]
+    *a_A2 = (float)(lambda * (double)defocus_um * 1e4 / (2.0 * M_PI));            // R8
+    *b_A2 = (float)((double)bfactor_A2 / (8.0 * M_PI * M_PI));                    // R9
+    return BIOEM_OK;
+}
+
+int bioem_set_shift_range(bioem_ctx *ctx, int max_shift_px)
+{
+    if (!ctx) return BIOEM_EBADARG;
+    if (max_shift_px < 0) FAIL(BIOEM_EBADARG, "set_shift_range: negative");
+    if (ctx->N && 2 * max_shift_px + 1 > ctx->N) FAIL(BIOEM_EBADARG, "set_shift_range: 2D+1 exceeds n_pix");
+    ctx->D = max_shift_px;
+    ctx->ran = false;
+    return BIOEM_OK;
+}
+
+int bioem_push_images(bioem_ctx *ctx, int n_img, const float *pixels, int is_device)
+{
+    if (!ctx) return BIOEM_EBADARG;
+    if (!ctx->N) FAIL(BIOEM_EBADSTATE, "push_images: set_image_geometry first");
+    if (n_img <= 0 || !pixels) FAIL(BIOEM_EBADARG, "push_images: n_img <= 0 or NULL");
+    CK(cudaSetDevice(ctx->device));
+    const int N = ctx->N;
+    const size_t n = (size_t)N * N, H = (size_t)(N / 2 + 1) * N;
+    cudaStream_t st = ctx->stream;
+    // process in slabs so that scratch stays bounded
+    const int slab = 256;
+    CK(ctx->Ohat64.ensure((size_t)n_img * H * sizeof(cd)));
+    CK(ctx->Ohat32.ensure((size_t)n_img * H * sizeof(cf)));
+    CK(ctx->Dw.ensure((size_t)n_img * sizeof(double)));
+    CK(ctx->beta.ensure((size_t)n_img * sizeof(float)));
+    CK(ctx->scratch_a.ensure((size_t)slab * n * sizeof(double)));       // centred images
+    CK(ctx->scratch_b.ensure((size_t)slab * H * sizeof(cd)));           // transform intermediate
+    DBuf staging;
+    const float *dsrc = pixels;
+    if (!is_device) {
+        cudaError_t e = staging.ensure((size_t)n_img * n * sizeof(float));
+        if (e == cudaSuccess) e = cudaMemcpyAsync(staging.p, pixels, (size_t)n_img * n * sizeof(float), cudaMemcpyHostToDevice, st);
+        if (e != cudaSuccess) { staging.release(); CK(e); }
+        dsrc = staging.as<float>();
+    }
+    cudaError_t e = cudaSuccess;
+    for (int i0 = 0; i0 < n_img && e == cudaSuccess; i0 += slab) {
+        const int nb = std::min(slab, n_img - i0);
+        e = launch_image_stats(dsrc + (size_t)i0 * n, nb, N, ctx->scratch_a.as<double>(), ctx->Dw.as<double>() + i0, st);
+        if (e == cudaSuccess) e = launch_fft2_r2c_f64(ctx->scratch_a.as<double>(), nb, N, ctx->scratch_b.as<cd>(), ctx->Ohat64.as<cd>() + (size_t)i0 * H, st);
+        if (e == cudaSuccess) e = launch_zero_dc(ctx->Ohat64.as<cd>() + (size_t)i0 * H, nb, H, st);
+    }
+    if (e == cudaSuccess) e = launch_cast_spectrum(ctx->Ohat64.as<cd>(), ctx->Ohat32.as<cf>(), (size_t)n_img * H, st);
+    if (e == cudaSuccess) e = launch_beta(ctx->Dw.as<double>(), n_img, ctx->beta.as<float>(), st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);      // inputs are copied: safe to free after return
+    staging.release();
+    CK(e);
+    ctx->n_img = n_img;
+    ctx->ran = false;
+    return BIOEM_OK;
+}
+
+static int choose_oc(long long n_img, long long n_model, long long n_orient)
+{
+    long long oc = n_img * n_model * n_orient / 4736;      // aim at >= 32 work items per SM
+    if (oc < 1) oc = 1;
+    if (oc > 32) oc = 32;
+    if (oc > n_orient) oc = n_orient;
+    return (int)oc;
+}
+
+int bioem_run(bioem_ctx *ctx)
+{
+    if (!ctx) return BIOEM_EBADARG;
+    if (!ctx->N) FAIL(BIOEM_EBADSTATE, "run: image geometry not set");
+    if (ctx->models.empty()) FAIL(BIOEM_EBADSTATE, "run: no model");
+    if (!ctx->n_orient) FAIL(BIOEM_EBADSTATE, "run: no orientations");
+    if (!ctx->n_ctf) FAIL(BIOEM_EBADSTATE, "run: no CTF grid");
+    if (ctx->D < 0) FAIL(BIOEM_EBADSTATE, "run: shift range not set");
+    if (!ctx->n_img) FAIL(BIOEM_EBADSTATE, "run: no images");
+    const int N = ctx->N, D = ctx->D, O = ctx->n_orient, C = ctx->n_ctf, I = ctx->n_img, M = (int)ctx->models.size();
+    if (2 * D + 1 > N) FAIL(BIOEM_EBADARG, "run: 2D+1 exceeds n_pix");
+    if ((long long)O * C > 0x7fffffffLL) FAIL(BIOEM_EUNSUPPORTED, "run: orientations x CTFs exceeds 2^31");
+    if (fused_smem_bytes(N, D) == 0) FAIL(BIOEM_EUNSUPPORTED, "run: shift range too large for the shared-memory plan at this n_pix");
+    for (auto &m : ctx->models)
+        if (m.kind == 1 && (m.n_vox != N || std::fabs(m.voxel - ctx->px) > 1e-9 * ctx->px))
+            FAIL(BIOEM_EUNSUPPORTED, "run: density model needs n_vox == n_pix and voxel_A == pixel_size_A (R21)");
+    CK(cudaSetDevice(ctx->device));
+    cudaStream_t st = ctx->stream;
+    const size_t n = (size_t)N * N, H = (size_t)(N / 2 + 1) * N;
+    const size_t MO = (size_t)M * O, MOC = MO * C;
+    ctx->ran = false;
+    ctx->launches = 0; ctx->fused_launches = 0;
+
+    CK(ctx->F064.ensure(MO * H * sizeof(cd)));
+    CK(ctx->F032.ensure(MO * H * sizeof(cf)));
+    CK(ctx->K64.ensure((size_t)C * H * sizeof(double)));
+    CK(ctx->K32.ensure((size_t)C * H * sizeof(float)));
+    CK(ctx->Tc64.ensure(MOC * sizeof(double)));
+    CK(ctx->h64.ensure(MOC * sizeof(double)));
+    CK(ctx->alpha32.ensure(MOC * sizeof(float)));
+    CK(ctx->h32.ensure(MOC * sizeof(float)));
+    const int oc = choose_oc(I, M, O), cpm = (O + oc - 1) / oc;
+    const size_t items = (size_t)I * M * cpm, IM = (size_t)I * M;
+    CK(ctx->part_m.ensure(items * sizeof(float)));
+    CK(ctx->part_s.ensure(items * sizeof(float)));
+    CK(ctx->part_top.ensure(items * BIOEM_TOPK * sizeof(TopEntry)));
+    CK(ctx->m32.ensure(IM * sizeof(double)));
+    CK(ctx->s32.ensure(IM * sizeof(double)));
+    CK(ctx->top.ensure(IM * BIOEM_TOPK * sizeof(TopEntry)));
+    CK(ctx->g64.ensure(IM * BIOEM_TOPK * sizeof(double)));
+    CK(ctx->logp.ensure(IM * sizeof(double)));
+    CK(ctx->logp32.ensure(IM * sizeof(double)));
+    CK(ctx->best.ensure(IM * 4 * sizeof(int32_t)));
+    CK(ctx->best_logp.ensure(IM * sizeof(double)));
+
+    CK(cudaEventRecord(ctx->ev[0], st));
+
+    // ---- a3: CTF tables
+    CK(launch_ctf_tables(ctx->ctf_a.as<double>(), ctx->ctf_A.as<double>(), ctx->ctf_b.as<double>(), C, N, ctx->px, ctx->K64.as<double>(),
+                         ctx->K32.as<float>(), st));
+    ctx->launches += 1;
+
+    // ---- a1/a1' + a2: spectra of all projections, model by model, orientation batch by batch
+    const int OB = 256;
+    for (int mi = 0; mi < M; ++mi) {
+        Model &m = ctx->models[mi];
+        cd *F64m = ctx->F064.as<cd>() + (size_t)mi * O * H;
+        if (m.kind == 0) {
+            CK(ctx->scratch_a.ensure((size_t)OB * n * sizeof(double)));      // I0 (double)
+            CK(ctx->scratch_b.ensure((size_t)OB * H * sizeof(cd)));          // transform intermediate
+            CK(ctx->scratch_c.ensure((size_t)OB * n * sizeof(long long)));   // fixed-point accumulator
+            // fixed-point scale: a pixel can never hold more than the total |weight| of the model
+            int ex = 0;
+            std::frexp(m.sum_abs_w > 0 ? m.sum_abs_w : 1.0, &ex);
+            const double fx_scale = std::ldexp(1.0, 60 - ex);
+            for (int o0 = 0; o0 < O; o0 += OB) {
+                const int nb = std::min(OB, O - o0);
+                CK(launch_project_atoms(m.xyz.as<double>(), m.rad.as<double>(), m.wt.as<double>(), m.n_atoms, ctx->rot.as<double>() + (size_t)o0 * 9,
+                                        nb, N, ctx->px, fx_scale, ctx->scratch_c.as<long long>(), ctx->scratch_a.as<double>(), st));
+                CK(launch_fft2_r2c_f64(ctx->scratch_a.as<double>(), nb, N, ctx->scratch_b.as<cd>(), F64m + (size_t)o0 * H, st));
+                ctx->launches += 4;
+            }
+        } else {
+            const size_t n3 = (size_t)N * N * N;
+            CK(ctx->scratch_a.ensure(n3 * sizeof(cd)));
+            CK(ctx->scratch_b.ensure(n3 * sizeof(cd)));
+            CK(launch_dft3_f64(m.rho.as<float>(), N, ctx->scratch_a.as<cd>(), ctx->scratch_b.as<cd>(), st));
+            CK(launch_slice_f64(ctx->scratch_a.as<cd>(), N, m.voxel, ctx->rot.as<double>(), O, F64m, st));
+            ctx->launches += 6;
+        }
+    }
+    CK(launch_cast_spectrum(ctx->F064.as<cd>(), ctx->F032.as<cf>(), MO * H, st));
+    CK(launch_calc_stats(ctx->F064.as<cd>(), ctx->K64.as<double>(), (int)MO, O, C, N, ctx->has_lp_orient ? ctx->lp_orient.as<double>() : nullptr,
+                         ctx->has_lp_ctf ? ctx->lp_ctf.as<double>() : nullptr, std::log((double)(2 * D + 1) * (2 * D + 1)),
+                         ctx->Tc64.as<double>(), ctx->h64.as<double>(), ctx->alpha32.as<float>(), ctx->h32.as<float>(), st));
+    ctx->launches += 2;
+
+    // ---- a4-a6: the fused kernel
+    FusedParams p{};
+    p.Ohat = ctx->Ohat32.as<cf>(); p.F0 = ctx->F032.as<cf>(); p.K = ctx->K32.as<float>();
+    p.alpha = ctx->alpha32.as<float>(); p.hterm = ctx->h32.as<float>(); p.beta = ctx->beta.as<float>();
+    p.n_img = I; p.n_model = M; p.n_orient = O; p.n_ctf = C; p.D = D; p.oc = oc; p.chunks_per_model = cpm;
+    p.cA = (float)(-0.5 * ((double)n - 3.0));
+    p.part_m = ctx->part_m.as<float>(); p.part_s = ctx->part_s.as<float>(); p.part_top = ctx->part_top.as<TopEntry>();
+    CK(cudaEventRecord(ctx->ev[1], st));
+    int nl = 0;
+    CK(launch_fused(N, p, false, st, &nl));
+    CK(cudaEventRecord(ctx->ev[2], st));
+    ctx->launches += nl; ctx->fused_launches += nl;
+
+    // ---- a6 combine, a7 re-score, results
+    CK(launch_merge(p.part_m, p.part_s, p.part_top, I, M, cpm, ctx->m32.as<double>(), ctx->s32.as<double>(), ctx->top.as<TopEntry>(), st));
+    CK(launch_rescore(ctx->Ohat64.as<cd>(), ctx->F064.as<cd>(), ctx->K64.as<double>(), ctx->Tc64.as<double>(), ctx->h64.as<double>(),
+                      ctx->Dw.as<double>(), ctx->top.as<TopEntry>(), BIOEM_TOPK, I, M, O, C, N, D, -1, ctx->g64.as<double>(), st));
+    const double nn = (double)n;
+    const double const_n = -0.5 * (nn - 2.0) * std::log(2.0 * M_PI) + 0.5 * (nn - 5.0) * std::log(2.0) + std::lgamma(0.5 * (nn - 3.0));
+    CK(launch_final(ctx->m32.as<double>(), ctx->s32.as<double>(), ctx->top.as<TopEntry>(), ctx->g64.as<double>(), ctx->Dw.as<double>(), I, M,
+                    C, N, D, const_n, ctx->logp.as<double>(), ctx->logp32.as<double>(), ctx->best.as<int32_t>(), ctx->best_logp.as<double>(), st));
+    ctx->launches += 3;
+    CK(cudaEventRecord(ctx->ev[3], st));
+    ctx->ran = true;
+    ctx->run_models = M; ctx->run_orient = O; ctx->run_ctf = C; ctx->run_D = D; ctx->run_img = I;
+    return BIOEM_OK;
+}
+
+static int fetch(bioem_ctx *ctx, void *dst, const void *src, size_t bytes)
+{
+    CK(cudaSetDevice(ctx->device));
+    CK(cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToHost, ctx->stream));
+    CK(cudaStreamSynchronize(ctx->stream));
+    return BIOEM_OK;
+}
+
+int bioem_get_log_posterior(bioem_ctx *ctx, double *out)
+{
+    if (!ctx || !out) return BIOEM_EBADARG;
+    if (!ctx->ran) FAIL(BIOEM_EBADSTATE, "get_log_posterior: no completed run");
+    return fetch(ctx, out, ctx->logp.p, (size_t)ctx->run_img * ctx->run_models * sizeof(double));
+}
+
+int bioem_debug_log_posterior_f32(bioem_ctx *ctx, double *out)
+{
+    if (!ctx || !out) return BIOEM_EBADARG;
+    if (!ctx->ran) FAIL(BIOEM_EBADSTATE, "debug_log_posterior_f32: no completed run");
+    return fetch(ctx, out, ctx->logp32.p, (size_t)ctx->run_img * ctx->run_models * sizeof(double));
+}
+
+int bioem_get_best(bioem_ctx *ctx, int32_t *orient_idx, int32_t *ctf_idx, int32_t *dx, int32_t *dy, double *best_log_p)
+{
+    if (!ctx) return BIOEM_EBADARG;
+    if (!ctx->ran) FAIL(BIOEM_EBADSTATE, "get_best: no completed run");
+    const size_t IM = (size_t)ctx->run_img * ctx->run_models;
+    std::vector<int32_t> b(4 * IM);
+    int rc = fetch(ctx, b.data(), ctx->best.p, 4 * IM * sizeof(int32_t));
+    if (rc) return rc;
+    for (size_t i = 0; i < IM; ++i) {
+        if (orient_idx) orient_idx[i] = b[4 * i];
+        if (ctf_idx) ctf_idx[i] = b[4 * i + 1];
+        if (dx) dx[i] = b[4 * i + 2];
+        if (dy) dy[i] = b[4 * i + 3];
+    }
+    if (best_log_p) return fetch(ctx, best_log_p, ctx->best_logp.p, IM * sizeof(double));
+    return BIOEM_OK;
+}
+
+static int check_tuple(bioem_ctx *ctx, int img, int model, int orient, int ctf)
+{
+    if (!ctx->ran) FAIL(BIOEM_EBADSTATE, "debug: call bioem_run first (the precomputed spectra are reused)");
+    if (img < 0 || img >= ctx->run_img || model < 0 || model >= ctx->run_models || orient < 0 || orient >= ctx->run_orient || ctf < 0 ||
+        ctf >= ctx->run_ctf)
+        FAIL(BIOEM_EBADARG, "debug: index out of range");
+    return BIOEM_OK;
+}
+
+int bioem_debug_calc_image(bioem_ctx *ctx, int model, int orient, int ctf, float *out_real)
+{
+    if (!ctx || !out_real) return BIOEM_EBADARG;
+    int rc = check_tuple(ctx, 0, model, orient, ctf);
+    if (rc) return rc;
+    CK(cudaSetDevice(ctx->device));
+    const int N = ctx->N;
+    const size_t n = (size_t)N * N, H = (size_t)(N / 2 + 1) * N;
+    CK(ctx->dump.ensure(n * sizeof(double)));
+    CK(launch_calc_image(ctx->F064.as<cd>() + ((size_t)model * ctx->run_orient + orient) * H, ctx->K64.as<double>() + (size_t)ctf * H, N,
+                         ctx->dump.as<double>(), ctx->stream));
+    std::vector<double> tmp(n);
+    rc = fetch(ctx, tmp.data(), ctx->dump.p, n * sizeof(double));
+    if (rc) return rc;
+    for (size_t i = 0; i < n; ++i) out_real[i] = (float)tmp[i];
+    return BIOEM_OK;
+}
+
+int bioem_debug_shift_map(bioem_ctx *ctx, int img, int model, int orient, int ctf, double *out)
+{
+    if (!ctx || !out) return BIOEM_EBADARG;
+    int rc = check_tuple(ctx, img, model, orient, ctf);
+    if (rc) return rc;
+    CK(cudaSetDevice(ctx->device));
+    const int N = ctx->N, D = ctx->run_D, KK = 2 * D + 1;
+    const size_t n = (size_t)N * N;
+    CK(ctx->dump.ensure((size_t)KK * KK * sizeof(float)));
+    FusedParams p{};
+    p.Ohat = ctx->Ohat32.as<cf>(); p.F0 = ctx->F032.as<cf>(); p.K = ctx->K32.as<float>();
+    p.alpha = ctx->alpha32.as<float>(); p.hterm = ctx->h32.as<float>(); p.beta = ctx->beta.as<float>();
+    p.n_img = ctx->run_img; p.n_model = ctx->run_models; p.n_orient = ctx->run_orient; p.n_ctf = ctx->run_ctf; p.D = D; p.oc = 1;
+    p.chunks_per_model = 1;
+    p.cA = (float)(-0.5 * ((double)n - 3.0));
+    p.dump = ctx->dump.as<float>(); p.dump_img = img; p.dump_model = model; p.dump_orient = orient; p.dump_ctf = ctf;
+    CK(launch_fused(N, p, true, ctx->stream, nullptr));
+    std::vector<float> tmp((size_t)KK * KK);
+    rc = fetch(ctx, tmp.data(), ctx->dump.p, tmp.size() * sizeof(float));
+    if (rc) return rc;
+    std::vector<double> dw(1);
+    rc = fetch(ctx, dw.data(), ctx->Dw.as<double>() + img, sizeof(double));
+    if (rc) return rc;
+    const double nn = (double)n;
+    const double base = -0.5 * (nn - 2.0) * std::log(2.0 * M_PI) + 0.5 * (nn - 5.0) * std::log(2.0) + std::lgamma(0.5 * (nn - 3.0)) -
+                        0.5 * (nn - 3.0) * std::log(dw[0]);
+    for (size_t i = 0; i < tmp.size(); ++i) out[i] = base + (double)tmp[i];
+    return BIOEM_OK;
+}
+
+int bioem_debug_shift_map_f64(bioem_ctx *ctx, int img, int model, int orient, int ctf, double *out)
+{
+    if (!ctx || !out) return BIOEM_EBADARG;
+    int rc = check_tuple(ctx, img, model, orient, ctf);
+    if (rc) return rc;
+    CK(cudaSetDevice(ctx->device));
+    const int N = ctx->N, D = ctx->run_D, KK = 2 * D + 1, S = KK * KK;
+    const size_t n = (size_t)N * N;
+    std::vector<TopEntry> cand(S);
+    for (int s = 0; s < S; ++s) cand[s] = {0.f, (uint32_t)(orient * ctx->run_ctf + ctf), (uint32_t)s};
+    DBuf dc, dg;
+    cudaError_t e = dc.ensure(S * sizeof(TopEntry));
+    if (e == cudaSuccess) e = dg.ensure(S * sizeof(double));
+    if (e == cudaSuccess) e = cudaMemcpyAsync(dc.p, cand.data(), S * sizeof(TopEntry), cudaMemcpyHostToDevice, ctx->stream);
+    // one "image" slot = img: pass pointers offset so that candidate block 0 maps to (img, model)
+    if (e == cudaSuccess)
+        e = launch_rescore(ctx->Ohat64.as<cd>() + (size_t)img * (size_t)(N / 2 + 1) * N, ctx->F064.as<cd>(), ctx->K64.as<double>(),
+                           ctx->Tc64.as<double>(), ctx->h64.as<double>(), ctx->Dw.as<double>() + img, dc.as<TopEntry>(), S, 1, ctx->run_models,
+                           ctx->run_orient, ctx->run_ctf, N, D, model, dg.as<double>(), ctx->stream);
+    std::vector<double> g(S), dw(1);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(g.data(), dg.p, S * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(dw.data(), ctx->Dw.as<double>() + img, sizeof(double), cudaMemcpyDeviceToHost, ctx->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+    dc.release(); dg.release();
+    CK(e);
+    const double nn = (double)n;
+    const double base = -0.5 * (nn - 2.0) * std::log(2.0 * M_PI) + 0.5 * (nn - 5.0) * std::log(2.0) + std::lgamma(0.5 * (nn - 3.0)) -
+                        0.5 * (nn - 3.0) * std::log(dw[0]);
+    for (int s = 0; s < S; ++s) out[s] = base + g[s];
+    return BIOEM_OK;
+}
+
+int bioem_get_timing(bioem_ctx *ctx, double *ms_total, double *ms_fused_kernel)
+{
+    if (!ctx) return BIOEM_EBADARG;
+    if (!ctx->ran) FAIL(BIOEM_EBADSTATE, "get_timing: no completed run");
+    CK(cudaSetDevice(ctx->device));
+    CK(cudaEventSynchronize(ctx->ev[3]));
+    float a = 0.f, b = 0.f;
+    CK(cudaEventElapsedTime(&a, ctx->ev[0], ctx->ev[3]));
+    CK(cudaEventElapsedTime(&b, ctx->ev[1], ctx->ev[2]));
+    if (ms_total) *ms_total = a;
+    if (ms_fused_kernel) *ms_fused_kernel = b;
+    return BIOEM_OK;
+}
+
+int bioem_get_launch_count(bioem_ctx *ctx, int64_t *n_launches, int64_t *n_fused_launches)
+{
+    if (!ctx) return BIOEM_EBADARG;
+    if (n_launches) *n_launches = ctx->launches;
+    if (n_fused_launches) *n_fused_launches = ctx->fused_launches;
+    return BIOEM_OK;
+}
+
+int bioem_measure_fp32_peak(bioem_ctx *ctx, double *tflops, double *sm_mhz)
+{
+    if (!ctx) return BIOEM_EBADARG;
+    CK(cudaSetDevice(ctx->device));
+    DBuf sink;
+    CK(sink.ensure(64));
+    const int iters = 4096;
+    cudaEvent_t a, b;
+    CK(cudaEventCreate(&a));
+    CK(cudaEventCreate(&b));
+    cudaError_t e = launch_fp32_peak(sink.as<float>(), 256, ctx->stream);        // warm-up
+    float best = 1e30f;
+    for (int r = 0; r < 5 && e == cudaSuccess; ++r) {
+        cudaEventRecord(a, ctx->stream);
+        e = launch_fp32_peak(sink.as<float>(), iters, ctx->stream);
+        cudaEventRecord(b, ctx->stream);
+        if (e == cudaSuccess) e = cudaEventSynchronize(b);
+        float ms = 0.f;
+        if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, a, b);
+        if (ms < best) best = ms;
+    }
+    cudaEventDestroy(a); cudaEventDestroy(b);
+    sink.release();
+    CK(e);
+    const double flops = 148.0 * 8 * 256 * (double)iters * 128.0 * 2.0;
+    if (tflops) *tflops = flops / (best * 1e-3) / 1e12;
+    int khz = 0;
+    cudaDeviceGetAttribute(&khz, cudaDevAttrClockRate, ctx->device);
+    if (sm_mhz) *sm_mhz = khz / 1000.0;
+    return BIOEM_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,81 @@
+// common.cuh -- shared declarations of the bioem_b200 library (device-side layouts and host launchers).
+//
+// Device layouts:
+//   half-spectrum  [l][m]   l = 0..N/2 (x frequency, Hermitian half), m = 0..N-1 (y frequency), m fastest:
+//                  a column of fixed l is contiguous -> pass 1 of the pruned inverse transform streams it coalesced.
+//   Ohat32/64      [image][l][m]        spectrum of the mean-free observed image (a0), DC bin exactly 0
+//   F0_32/64       [model*O + o][l][m]  spectrum of the projection I0 (a1/a1'+a2)
+//   K32/64         [c][l][m]            CTF(s)Env(s) of CTF set c (a3; the paper's "precalculated radially symmetric images")
+//   alpha/hterm    [(model*O + o)*C + c]
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include "fft_core.cuh"
+
+#ifndef BIOEM_TOPK
+#define BIOEM_TOPK 8
+#endif
+
+namespace bioem {
+
+typedef cx<float> cf;
+typedef cx<double> cd;
+
+struct TopEntry { float g; uint32_t pair; uint32_t shift; };   // pair = o*C + c within the model, shift = (dy+D)*S1 + (dx+D)
+
+// choice of the two-step factorisation N = N1 * N2 per supported image size
+__host__ __device__ constexpr int n1_of(int N) { return N == 64 ? 16 : N == 128 ? 16 : N == 224 ? 32 : N == 256 ? 32 : 0; }
+
+struct FusedParams {
+    // inputs
+    const cf *Ohat;        // [I][H]
+    const cf *F0;          // [M*O][H]
+    const float *K;        // [C][H]
+    const float *alpha;    // [M*O*C]   1/sqrt(n T_c)
+    const float *hterm;    // [M*O*C]   -1/2 log T_c + log w
+    const float *beta;     // [I]       1/sqrt(D_omega)
+    int n_img, n_model, n_orient, n_ctf, D;
+    int oc;                // orientations per work item (chunk)
+    int chunks_per_model;
+    float cA;              // -(n-3)/2
+    // outputs: one partial per work item = (model, chunk, image)
+    float *part_m, *part_s;      // [items]
+    TopEntry *part_top;          // [items][TOPK]
+    // debug dump of one pair (DUMP instantiation only)
+    float *dump;                 // [S1*S1]
+    int dump_img, dump_model, dump_orient, dump_ctf;
+};
+
+// host launchers (each enqueues on `st`); return cudaError_t
+cudaError_t launch_fused(int N, const FusedParams &p, bool dump, cudaStream_t st, int *n_launches);
+size_t fused_smem_bytes(int N, int D);
+
+// precompute
+cudaError_t launch_image_stats(const float *img, int n_img, int N, double *centered, double *Dw, cudaStream_t st);
+cudaError_t launch_fft2_r2c_f64(const double *in, int batch, int N, cd *tmp, cd *out, cudaStream_t st);   // out [b][l][m]
+cudaError_t launch_cast_spectrum(const cd *in, cf *out, size_t count, cudaStream_t st);
+cudaError_t launch_zero_dc(cd *spec, int batch, size_t H, cudaStream_t st);
+cudaError_t launch_project_atoms(const double *xyz, const double *rad, const double *wt, int n_atoms, const double *rot,
+                                 int n_orient, int N, double px, double fx_scale, long long *acc, double *out, cudaStream_t st);
+cudaError_t launch_dft3_f64(const float *rho, int N, cd *work_a, cd *work_b, cudaStream_t st);           // result in work_a, centred sign applied
+cudaError_t launch_slice_f64(const cd *Vc, int N, double voxel, const double *rot, int n_orient, cd *out, cudaStream_t st);
+cudaError_t launch_ctf_tables(const double *a, const double *A, const double *b, int n_ctf, int N, double px,
+                              double *K64, float *K32, cudaStream_t st);
+cudaError_t launch_calc_stats(const cd *F0, const double *K64, int n_mo, int n_orient, int n_ctf, int N,
+                              const double *lp_orient, const double *lp_ctf, double log_shifts,
+                              double *Tc64, double *h64, float *alpha32, float *h32, cudaStream_t st);
+cudaError_t launch_beta(const double *Dw, int n_img, float *beta, cudaStream_t st);
+
+// finalise
+cudaError_t launch_merge(const float *part_m, const float *part_s, const TopEntry *part_top, int n_img, int n_model,
+                         int chunks_per_model, double *m32, double *s32, TopEntry *top, cudaStream_t st);
+cudaError_t launch_rescore(const cd *Ohat64, const cd *F064, const double *K64, const double *Tc64, const double *h64,
+                           const double *Dw, const TopEntry *cand, int n_cand_per, int n_img, int n_model, int n_orient,
+                           int n_ctf, int N, int D, int cand_model_fixed, double *g64, cudaStream_t st);
+cudaError_t launch_final(const double *m32, const double *s32, const TopEntry *top, const double *g64, const double *Dw,
+                         int n_img, int n_model, int n_ctf, int N, int D, double const_n, double *logp, double *logp32,
+                         int32_t *best, double *best_logp, cudaStream_t st);
+cudaError_t launch_calc_image(const cd *F0, const double *K64, int N, double *out, cudaStream_t st);
+cudaError_t launch_fp32_peak(float *sink, int iters, cudaStream_t st);
+
+}  // namespace bioem

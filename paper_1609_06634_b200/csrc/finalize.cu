@@ -1,0 +1,168 @@
+// finalize.cu -- SURVEY section 8 rows a6 (fixed-order combine of the per-chunk partials) and a7 (FP64 re-scoring of
+// the K best terms per (image, model), corrected log-sum-exp, argmax, constants).  Not in the paper: the paper runs
+// single precision and states it gives "the same numerical result"; the 1e-3 absolute parity bar on
+// log-posteriors of magnitude 1e4-1e5 needs the dominant terms in FP64 (hard part 1; DESIGN 6).
+#include "common.cuh"
+#include <math_constants.h>
+
+namespace bioem {
+
+__device__ __forceinline__ bool before(const TopEntry &a, const TopEntry &b)
+{
+    return a.g > b.g || (a.g == b.g && (a.pair < b.pair || (a.pair == b.pair && a.shift < b.shift)));
+}
+
+// One thread per (image, model): combine chunk partials in chunk order (bit-reproducible).
+__global__ void k_merge(const float *part_m, const float *part_s, const TopEntry *part_top, int n_img, int n_model, int cpm, double *m32,
+                        double *s32, TopEntry *top)
+{
+    const int im = blockIdx.x * blockDim.x + threadIdx.x;
+    if (im >= n_img * n_model) return;
+    const int img = im / n_model, model = im % n_model;
+    double M = -CUDART_INF, S = 0.0;
+    TopEntry best[BIOEM_TOPK];
+#pragma unroll
+    for (int k = 0; k < BIOEM_TOPK; ++k) best[k] = {-CUDART_INF_F, 0xffffffffu, 0xffffffffu};
+    for (int ch = 0; ch < cpm; ++ch) {
+        const size_t item = ((size_t)model * cpm + ch) * n_img + img;
+        const double m = part_m[item], s = part_s[item];
+        if (m != -CUDART_INF) {
+            if (M == -CUDART_INF) { M = m; S = s; }
+            else if (m > M) { S = S * exp(M - m) + s; M = m; }
+            else S += s * exp(m - M);
+        }
+        for (int k = 0; k < BIOEM_TOPK; ++k) {
+            TopEntry e = part_top[item * BIOEM_TOPK + k];
+            if (e.pair == 0xffffffffu) break;
+            if (!before(e, best[BIOEM_TOPK - 1])) continue;
+            int pos = BIOEM_TOPK - 1;
+            while (pos > 0 && before(e, best[pos - 1])) { best[pos] = best[pos - 1]; --pos; }
+            best[pos] = e;
+        }
+    }
+    m32[im] = M; s32[im] = S;
+    for (int k = 0; k < BIOEM_TOPK; ++k) top[(size_t)im * BIOEM_TOPK + k] = best[k];
+}
+
+cudaError_t launch_merge(const float *part_m, const float *part_s, const TopEntry *part_top, int n_img, int n_model, int cpm, double *m32,
+                         double *s32, TopEntry *top, cudaStream_t st)
+{
+    int n = n_img * n_model;
+    k_merge<<<(n + 63) / 64, 64, 0, st>>>(part_m, part_s, part_top, n_img, n_model, cpm, m32, s32, top);
+    return cudaGetLastError();
+}
+
+// a7: one CTA per candidate.  B(d) = 1/n sum_s conj(Ohat(s)) F0(s) K_c(s) exp(+2 pi i (l dx + m dy)/N)  (Eq. 12, R3/R4),
+// summed over the Hermitian half with weights (1 | 2) in FP64 in a fixed order.
+// g = -(n-3)/2 log1p(-rho^2) + h,  rho^2 = B_fft^2 / (n T_c D_w)  (form C2).
+__global__ void __launch_bounds__(256) k_rescore(const cd *Ohat, const cd *F0, const double *K64, const double *Tc64, const double *h64,
+                                                 const double *Dw, const TopEntry *cand, int ncp, int n_img, int n_model, int n_orient,
+                                                 int n_ctf, int N, int D, int model_fixed, double *g64)
+{
+    __shared__ double sh[256];
+    __shared__ cd tw[256];
+    const int NC = N / 2 + 1, H = NC * N, KK = 2 * D + 1;
+    const size_t ci = blockIdx.x;                       // candidate index = (img*n_model + model)*ncp + k
+    const TopEntry e = cand[ci];
+    if (e.pair == 0xffffffffu) { if (threadIdx.x == 0) g64[ci] = -CUDART_INF; return; }
+    const int im = (int)(ci / ncp);
+    const int img = model_fixed >= 0 ? im : im / n_model, model = model_fixed >= 0 ? model_fixed : im % n_model;
+    const int o = e.pair / n_ctf, c = e.pair % n_ctf;
+    const int dy = (int)(e.shift / KK) - D, dx = (int)(e.shift % KK) - D;
+    for (int i = threadIdx.x; i < N; i += 256) {
+        double sn, cs;
+        sincospi(2.0 * i / N, &sn, &cs);
+        tw[i] = {cs, sn};
+    }
+    __syncthreads();
+    const cd *Oi = Ohat + (size_t)img * H;
+    const cd *F = F0 + ((size_t)model * n_orient + o) * H;
+    const double *K = K64 + (size_t)c * H;
+    double s = 0.0;
+    for (int i = threadIdx.x; i < H; i += 256) {
+        const int l = i / N, m = i % N;
+        const double w = (l == 0 || l == N / 2) ? 1.0 : 2.0;
+        const cd a = Oi[i], b = F[i];
+        const double pr = a.x * b.x + a.y * b.y, pi = a.x * b.y - a.y * b.x;      // conj(a) b
+        const cd ph = tw[(((l * dx + m * dy) % N) + N) % N];
+        s += w * K[i] * (pr * ph.x - pi * ph.y);
+    }
+    __syncthreads();
+    sh[threadIdx.x] = s;
+    __syncthreads();
+    for (int st = 128; st >= 1; st >>= 1) {
+        if ((int)threadIdx.x < st) sh[threadIdx.x] += sh[threadIdx.x + st];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) {
+        const size_t moc = ((size_t)model * n_orient + o) * n_ctf + c;
+        const double n = (double)N * N;
+        const double B = sh[0];
+        double rho2 = B * B / (n * Tc64[moc] * Dw[img]);
+        if (rho2 > 1.0 - 1e-300) rho2 = 1.0 - 1e-300;                               // R14
+        g64[ci] = -0.5 * (n - 3.0) * log1p(-rho2) + h64[moc];
+    }
+}
+
+cudaError_t launch_rescore(const cd *Ohat64, const cd *F064, const double *K64, const double *Tc64, const double *h64, const double *Dw,
+                           const TopEntry *cand, int n_cand_per, int n_img, int n_model, int n_orient, int n_ctf, int N, int D,
+                           int cand_model_fixed, double *g64, cudaStream_t st)
+{
+    size_t total = (size_t)n_img * (cand_model_fixed >= 0 ? 1 : n_model) * n_cand_per;
+    k_rescore<<<(unsigned)total, 256, 0, st>>>(Ohat64, F064, K64, Tc64, h64, Dw, cand, n_cand_per, n_img, n_model, n_orient, n_ctf, N, D,
+                                               cand_model_fixed, g64);
+    return cudaGetLastError();
+}
+
+// One thread per (image, model): replace the K best FP32 terms by their FP64 values, argmax among them, constants.
+__global__ void k_final(const double *m32, const double *s32, const TopEntry *top, const double *g64, const double *Dw, int n_img,
+                        int n_model, int n_ctf, int N, int D, double const_n, double *logp, double *logp32, int32_t *best,
+                        double *best_logp)
+{
+    const int im = blockIdx.x * blockDim.x + threadIdx.x;
+    if (im >= n_img * n_model) return;
+    const int img = im / n_model, KK = 2 * D + 1;
+    const double n = (double)N * N;
+    const double base = const_n - 0.5 * (n - 3.0) * log(Dw[img]);
+    const TopEntry *t = top + (size_t)im * BIOEM_TOPK;
+    const double *g = g64 + (size_t)im * BIOEM_TOPK;
+    double M = m32[im];
+    int kb = -1;
+    for (int k = 0; k < BIOEM_TOPK; ++k) {
+        if (t[k].pair == 0xffffffffu) break;
+        if (g[k] > M) M = g[k];
+        if (kb < 0 || g[k] > g[kb] || (g[k] == g[kb] && (t[k].pair < t[kb].pair || (t[k].pair == t[kb].pair && t[k].shift < t[kb].shift))))
+            kb = k;
+    }
+    double tot32 = s32[im] * exp(m32[im] - M), top32 = 0.0, top64 = 0.0;
+    for (int k = 0; k < BIOEM_TOPK; ++k) {
+        if (t[k].pair == 0xffffffffu) break;
+        top32 += exp((double)t[k].g - M);
+        top64 += exp(g[k] - M);
+    }
+    double rest = tot32 - top32;
+    if (rest < 0.0) rest = 0.0;
+    logp[im] = base + M + log(top64 + rest);
+    logp32[im] = base + m32[im] + log(s32[im]);
+    if (kb >= 0) {
+        best[4 * im + 0] = (int32_t)(t[kb].pair / n_ctf);
+        best[4 * im + 1] = (int32_t)(t[kb].pair % n_ctf);
+        best[4 * im + 2] = (int32_t)(t[kb].shift % KK) - D;
+        best[4 * im + 3] = (int32_t)(t[kb].shift / KK) - D;
+        best_logp[im] = base + g[kb];
+    } else {
+        best[4 * im + 0] = best[4 * im + 1] = -1; best[4 * im + 2] = best[4 * im + 3] = 0;
+        best_logp[im] = -CUDART_INF;
+    }
+}
+
+cudaError_t launch_final(const double *m32, const double *s32, const TopEntry *top, const double *g64, const double *Dw, int n_img,
+                         int n_model, int n_ctf, int N, int D, double const_n, double *logp, double *logp32, int32_t *best,
+                         double *best_logp, cudaStream_t st)
+{
+    int n = n_img * n_model;
+    k_final<<<(n + 63) / 64, 64, 0, st>>>(m32, s32, top, g64, Dw, n_img, n_model, n_ctf, N, D, const_n, logp, logp32, best, best_logp);
+    return cudaGetLastError();
+}
+
+}  // namespace bioem

@@ -1,0 +1,400 @@
+// precompute.cu -- SURVEY section 8 rows a0 (observed images), a1 (atom projection, Eq. 1), a1' (Fourier slice, R21),
+// a2 (forward transform, Eq. 2) and a3 (CTF tables, Eq. 5, and the per-calc-image statistics).  Everything here runs
+// once per image / per (model, orientation) / per (model, orientation, CTF): <= 1/N_img of the hot loop's work.  It is
+// done in FP64 so that (i) the FP32 operands of the hot loop are correctly rounded and (ii) the FP64 re-scoring pass
+// (a7) can reuse the same spectra.
+#include "common.cuh"
+#include <math_constants.h>
+
+namespace bioem {
+
+// deterministic block sum (fixed tree), result valid in thread 0
+template <int NT>
+__device__ __forceinline__ double block_sum(double v, double *sh)
+{
+    sh[threadIdx.x] = v;
+    __syncthreads();
+#pragma unroll
+    for (int s = NT / 2; s >= 1; s >>= 1) {
+        if ((int)threadIdx.x < s) sh[threadIdx.x] += sh[threadIdx.x + s];
+        __syncthreads();
+    }
+    double r = sh[0];
+    __syncthreads();
+    return r;
+}
+
+// ------------------------------------------------------------------------------------------------ a0: C_o, C_oo
+// centered = I_obs - mean (so the correlation with it IS B(d), SURVEY 7 hard part 2);  Dw = sum centered^2 = C_oo - C_o^2/n.
+__global__ void __launch_bounds__(256) k_image_stats(const float *img, int n, double *centered, double *Dw)
+{
+    __shared__ double sh[256];
+    const float *src = img + (size_t)blockIdx.x * n;
+    double *dst = centered + (size_t)blockIdx.x * n;
+    double s = 0;
+    for (int i = threadIdx.x; i < n; i += 256) s += (double)src[i];
+    double mean = block_sum<256>(s, sh) / n;
+    double q = 0;
+    for (int i = threadIdx.x; i < n; i += 256) { double v = (double)src[i] - mean; dst[i] = v; q += v * v; }
+    q = block_sum<256>(q, sh);
+    if (threadIdx.x == 0) Dw[blockIdx.x] = q;
+}
+
+cudaError_t launch_image_stats(const float *img, int n_img, int N, double *centered, double *Dw, cudaStream_t st)
+{
+    k_image_stats<<<n_img, 256, 0, st>>>(img, N * N, centered, Dw);
+    return cudaGetLastError();
+}
+
+__global__ void k_beta(const double *Dw, int n, float *beta)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) beta[i] = (float)(1.0 / sqrt(Dw[i]));
+}
+cudaError_t launch_beta(const double *Dw, int n_img, float *beta, cudaStream_t st)
+{
+    k_beta<<<(n_img + 255) / 256, 256, 0, st>>>(Dw, n_img, beta);
+    return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------------ generic FP64 1-D transform (two-step)
+// y[k] = sum_e x[e] exp(SIGN 2 pi i e k / N), k < kout.  Sequence g: batch b = g / spb, s = g % spb;
+// x[e] at in + b*ibs + s*iss + e*ies (real or complex), y[k] at out + b*obs + s*oss + k*oes.
+template <int N, int SIGN, bool REAL_IN, int SPB>
+__global__ void __launch_bounds__(SPB *(N / n1_of(N))) k_fft1d_f64(const void *in_, long ibs, long iss, long ies, cd *out, long obs,
+                                                                    long oss, long oes, int nseq, int spb, int kout)
+{
+    constexpr int N1 = n1_of(N), N2 = N / N1, ZP = N1 + 1, LB = ilog2(N1), NT = SPB * N2;
+    __shared__ cd Z[SPB * N2 * ZP];
+    __shared__ cd tw[N];
+    const int tid = threadIdx.x;
+    for (int i = tid; i < N; i += NT) {
+        double sn, cs;
+        sincospi(2.0 * i / N, &sn, &cs);
+        tw[i] = {cs, SIGN > 0 ? sn : -sn};
+    }
+    const int sl = tid / N2, t = tid % N2;
+    const int g = blockIdx.x * SPB + sl;
+    if (g < nseq) {
+        const long off = (long)(g / spb) * ibs + (long)(g % spb) * iss;
+        cd a[N1];
+#pragma unroll
+        for (int j = 0; j < N1; ++j) {
+            long e = off + (long)(N2 * j + t) * ies;
+            if (REAL_IN) a[j] = {reinterpret_cast<const double *>(in_)[e], 0.0};
+            else a[j] = reinterpret_cast<const cd *>(in_)[e];
+        }
+        fft_dif<double, N1, SIGN>(a);
+#pragma unroll
+        for (int r = 0; r < N1; ++r) Z[(sl * N2 + t) * ZP + bitrev(r, LB)] = a[r];
+    }
+    __syncthreads();
+    for (int idx = tid; idx < SPB * kout; idx += NT) {
+        const int s2 = idx / kout, k = idx % kout;
+        const int g2 = blockIdx.x * SPB + s2;
+        if (g2 >= nseq) break;
+        const int k1 = k % N1;
+        cd acc = {0.0, 0.0};
+#pragma unroll
+        for (int tt = 0; tt < N2; ++tt) {
+            cd w = tw[(tt * k) % N], z = Z[(s2 * N2 + tt) * ZP + k1];
+            acc.x += w.x * z.x - w.y * z.y;
+            acc.y += w.x * z.y + w.y * z.x;
+        }
+        out[(long)(g2 / spb) * obs + (long)(g2 % spb) * oss + (long)k * oes] = acc;
+    }
+}
+
+template <int SIGN, bool REAL_IN>
+static cudaError_t fft1d(int N, const void *in, long ibs, long iss, long ies, cd *out, long obs, long oss, long oes, int nseq,
+                         int spb, int kout, cudaStream_t st)
+{
+    constexpr int SPB = 4;
+    int grid = (nseq + SPB - 1) / SPB;
+    switch (N) {
+    case 64: k_fft1d_f64<64, SIGN, REAL_IN, SPB><<<grid, SPB * 4, 0, st>>>(in, ibs, iss, ies, out, obs, oss, oes, nseq, spb, kout); break;
+    case 128: k_fft1d_f64<128, SIGN, REAL_IN, SPB><<<grid, SPB * 8, 0, st>>>(in, ibs, iss, ies, out, obs, oss, oes, nseq, spb, kout); break;
+    case 224: k_fft1d_f64<224, SIGN, REAL_IN, SPB><<<grid, SPB * 7, 0, st>>>(in, ibs, iss, ies, out, obs, oss, oes, nseq, spb, kout); break;
+    case 256: k_fft1d_f64<256, SIGN, REAL_IN, SPB><<<grid, SPB * 8, 0, st>>>(in, ibs, iss, ies, out, obs, oss, oes, nseq, spb, kout); break;
+    default: return cudaErrorInvalidValue;
+    }
+    return cudaGetLastError();
+}
+
+// a0 / a2: real [b][k][j] -> half spectrum [b][l][m], forward sign (Eq. 2 under R3).  tmp: [b][l][k].
+cudaError_t launch_fft2_r2c_f64(const double *in, int batch, int N, cd *tmp, cd *out, cudaStream_t st)
+{
+    const int NC = N / 2 + 1;
+    const long H = (long)NC * N;
+    // along x: sequence = row k of image b
+    cudaError_t e = fft1d<-1, true>(N, in, (long)N * N, N, 1, tmp, H, 1, N, batch * N, N, NC, st);
+    if (e != cudaSuccess) return e;
+    // along y: sequence = column l of image b
+    return fft1d<-1, false>(N, tmp, H, N, 1, out, H, N, 1, batch * NC, NC, N, st);
+}
+
+__global__ void k_cast_spec(const cd *in, cf *out, size_t n)
+{
+    size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) { cd v = in[i]; out[i] = {(float)v.x, (float)v.y}; }
+}
+cudaError_t launch_cast_spectrum(const cd *in, cf *out, size_t count, cudaStream_t st)
+{
+    k_cast_spec<<<(unsigned)((count + 255) / 256), 256, 0, st>>>(in, out, count);
+    return cudaGetLastError();
+}
+
+__global__ void k_zero_dc(cd *spec, int batch, size_t H)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < batch) spec[(size_t)i * H] = {0.0, 0.0};
+}
+cudaError_t launch_zero_dc(cd *spec, int batch, size_t H, cudaStream_t st)
+{
+    k_zero_dc<<<(batch + 255) / 256, 256, 0, st>>>(spec, batch, H);
+    return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------------ a1: Eq. 1, R10-R12
+// One CTA per orientation; each thread takes atoms.  The pixel integral is the 4x4 mid-point sum of the chord length
+// 2 sqrt(R^2 - r^2)_+ (R10), accumulated as 64-bit FIXED-POINT integers with atomics: integer addition is associative,
+// so the image is bit-identical from run to run whatever the order of the atoms (no float atomics).
+__global__ void __launch_bounds__(256) k_project(const double *xyz, const double *rad, const double *wt, int n_atoms, const double *rot,
+                                                 int N, double px, double fx_scale, long long *acc)
+{
+    const double *R = rot + (size_t)blockIdx.x * 9;
+    unsigned long long *img = reinterpret_cast<unsigned long long *>(acc) + (size_t)blockIdx.x * N * N;
+    constexpr int KQ = 4;
+    const double h = px / KQ;
+    for (int a = threadIdx.x; a < n_atoms; a += 256) {
+        const double x0 = xyz[3 * a], y0 = xyz[3 * a + 1], z0 = xyz[3 * a + 2];
+        const double xr = R[0] * x0 + R[1] * y0 + R[2] * z0;
+        const double yr = R[3] * x0 + R[4] * y0 + R[5] * z0;
+        const double Ra = rad[a], R2 = Ra * Ra;
+        const double dens = wt[a] / (4.0 / 3.0 * CUDART_PI * Ra * Ra * Ra) * h * h;
+        const int j0 = (int)floor((xr - Ra) / px + N / 2 - 0.5) - 1, j1 = (int)ceil((xr + Ra) / px + N / 2 + 0.5) + 1;
+        const int k0 = (int)floor((yr - Ra) / px + N / 2 - 0.5) - 1, k1 = (int)ceil((yr + Ra) / px + N / 2 + 0.5) + 1;
+        for (int k = k0; k <= k1; ++k) {
+            if (k < 0 || k >= N) continue;
+            const double yc = (k - N / 2) * px - 0.5 * px - yr;
+            for (int j = j0; j <= j1; ++j) {
+                if (j < 0 || j >= N) continue;
+                const double xc = (j - N / 2) * px - 0.5 * px - xr;
+                double s = 0.0;
+#pragma unroll
+                for (int sy = 0; sy < KQ; ++sy) {
+                    const double dy = yc + (sy + 0.5) * h;
+#pragma unroll
+                    for (int sx = 0; sx < KQ; ++sx) {
+                        const double dx = xc + (sx + 0.5) * h;
+                        const double d2 = R2 - dx * dx - dy * dy;
+                        if (d2 > 0.0) s += 2.0 * sqrt(d2);
+                    }
+                }
+                if (s > 0.0) {
+                    long long q = __double2ll_rn(dens * s * fx_scale);
+                    atomicAdd(img + (size_t)k * N + j, (unsigned long long)q);
+                }
+            }
+        }
+    }
+}
+
+__global__ void k_fixed_to_double(const long long *acc, double *out, size_t n, double inv_scale)
+{
+    size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) out[i] = (double)acc[i] * inv_scale;
+}
+
+cudaError_t launch_project_atoms(const double *xyz, const double *rad, const double *wt, int n_atoms, const double *rot, int n_orient,
+                                 int N, double px, double fx_scale, long long *acc, double *out, cudaStream_t st)
+{
+    size_t n = (size_t)n_orient * N * N;
+    cudaError_t e = cudaMemsetAsync(acc, 0, n * sizeof(long long), st);
+    if (e != cudaSuccess) return e;
+    k_project<<<n_orient, 256, 0, st>>>(xyz, rad, wt, n_atoms, rot, N, px, fx_scale, acc);
+    k_fixed_to_double<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(acc, out, n, 1.0 / fx_scale);
+    return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------------ a1': density model (R21)
+__global__ void k_rho_to_cd(const float *rho, cd *out, size_t n)
+{
+    size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) out[i] = {(double)rho[i], 0.0};
+}
+__global__ void k_centre_sign(cd *V, int N)
+{
+    size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    size_t n3 = (size_t)N * N * N;
+    if (i < n3) {
+        int kx = (int)(i % N), ky = (int)((i / N) % N), kz = (int)(i / ((size_t)N * N));
+        if ((kx + ky + kz) & 1) { cd v = V[i]; V[i] = {-v.x, -v.y}; }       // (-1)^(kx+ky+kz): parity of the index == parity of the signed frequency (N even)
+    }
+}
+
+// 3-D forward DFT of rho[z][y][x]; result (with the origin moved to voxel N/2) in work_a.
+cudaError_t launch_dft3_f64(const float *rho, int N, cd *work_a, cd *work_b, cudaStream_t st)
+{
+    const size_t n3 = (size_t)N * N * N;
+    const long N2 = (long)N * N;
+    k_rho_to_cd<<<(unsigned)((n3 + 255) / 256), 256, 0, st>>>(rho, work_a, n3);
+    // x: sequences (z,y) contiguous
+    cudaError_t e = fft1d<-1, false>(N, work_a, 0, N, 1, work_b, 0, N, 1, N * N, N * N, N, st);
+    if (e != cudaSuccess) return e;
+    // y: batch z, sequence kx, element stride N
+    e = fft1d<-1, false>(N, work_b, N2, 1, N, work_a, N2, 1, N, N * N, N, N, st);
+    if (e != cudaSuccess) return e;
+    // z: sequence (ky,kx) flat, element stride N^2
+    e = fft1d<-1, false>(N, work_a, 0, 1, N2, work_b, 0, 1, N2, N * N, N * N, N, st);
+    if (e != cudaSuccess) return e;
+    e = cudaMemcpyAsync(work_a, work_b, n3 * sizeof(cd), cudaMemcpyDeviceToDevice, st);
+    if (e != cudaSuccess) return e;
+    k_centre_sign<<<(unsigned)((n3 + 255) / 256), 256, 0, st>>>(work_a, N);
+    return cudaGetLastError();
+}
+
+// Central section: F0(l,m) = (-1)^(l'+m') voxel * trilinear[Vc](R^T (l',m',0)); zero outside |k_i| <= N/2-1 and on the
+// 2-D Nyquist bins; column l = 0 is completed from m' >= 0 so that the spectrum is exactly Hermitian.
+__global__ void __launch_bounds__(256) k_slice(const cd *Vc, int N, double voxel, const double *rot, cd *out)
+{
+    const double *R = rot + (size_t)blockIdx.y * 9;
+    const int NC = N / 2 + 1, h = N / 2;
+    const int idx = blockIdx.x * 256 + threadIdx.x;
+    if (idx >= NC * N) return;
+    const int l = idx / N, m = idx % N;
+    int ls = l, ms = (m <= h) ? m : m - N;
+    cd r = {0.0, 0.0};
+    bool conj = false;
+    if (ls == 0 && ms < 0) { ms = -ms; conj = true; }
+    if (ls < h && ms > -h && ms < h) {
+        const double k[3] = {R[0] * ls + R[3] * ms, R[1] * ls + R[4] * ms, R[2] * ls + R[5] * ms};
+        if (fabs(k[0]) <= h - 1 && fabs(k[1]) <= h - 1 && fabs(k[2]) <= h - 1) {
+            int f[3];
+            double t[3];
+#pragma unroll
+            for (int c = 0; c < 3; ++c) { double fl = floor(k[c]); f[c] = (int)fl; t[c] = k[c] - fl; }
+#pragma unroll
+            for (int cz = 0; cz < 2; ++cz)
+#pragma unroll
+                for (int cy = 0; cy < 2; ++cy)
+#pragma unroll
+                    for (int cx_ = 0; cx_ < 2; ++cx_) {
+                        const int ix = ((f[0] + cx_) % N + N) % N, iy = ((f[1] + cy) % N + N) % N, iz = ((f[2] + cz) % N + N) % N;
+                        const double w = (cx_ ? t[0] : 1 - t[0]) * (cy ? t[1] : 1 - t[1]) * (cz ? t[2] : 1 - t[2]);
+                        const cd v = Vc[((size_t)iz * N + iy) * N + ix];
+                        r.x += w * v.x; r.y += w * v.y;
+                    }
+            const double sg = ((ls + ms) & 1) ? -voxel : voxel;
+            r.x *= sg; r.y *= sg;
+            if (conj) r.y = -r.y;
+            if (ls == 0 && ms == 0) r.y = 0.0;
+        }
+    }
+    out[(size_t)blockIdx.y * NC * N + idx] = r;
+}
+
+cudaError_t launch_slice_f64(const cd *Vc, int N, double voxel, const double *rot, int n_orient, cd *out, cudaStream_t st)
+{
+    const int NC = N / 2 + 1;
+    dim3 grid((NC * N + 255) / 256, n_orient);
+    k_slice<<<grid, 256, 0, st>>>(Vc, N, voxel, rot, out);
+    return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------------ a3: Eqs. 4-5
+__global__ void k_ctf_tables(const double *a, const double *A, const double *b, int N, double px, double *K64, float *K32)
+{
+    const int NC = N / 2 + 1;
+    const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= NC * N) return;
+    const int c = blockIdx.y;
+    const int l = idx / N, m = idx % N;
+    const int ms = (m <= N / 2) ? m : m - N;
+    const double f = 2.0 * CUDART_PI / (N * px);
+    const double s2 = f * f * ((double)l * l + (double)ms * ms);
+    const double ph = 0.5 * a[c] * s2;
+    double sn, cs;
+    sincos(ph, &sn, &cs);
+    const double v = (-A[c] * cs - sqrt(1.0 - A[c] * A[c]) * sn) * exp(-0.5 * b[c] * s2);
+    K64[(size_t)c * NC * N + idx] = v;
+    K32[(size_t)c * NC * N + idx] = (float)v;
+}
+
+cudaError_t launch_ctf_tables(const double *a, const double *A, const double *b, int n_ctf, int N, double px, double *K64, float *K32,
+                              cudaStream_t st)
+{
+    const int NC = N / 2 + 1;
+    dim3 grid((NC * N + 255) / 256, n_ctf);
+    k_ctf_tables<<<grid, 256, 0, st>>>(a, A, b, N, px, K64, K32);
+    return cudaGetLastError();
+}
+
+// T_c = n C_cc - C_c^2 = sum_{s != 0} |F0(s) K_c(s)|^2 (Plancherel; "Eqs. S4, S6"), Hermitian weights:
+// columns l = 0 and l = N/2 count once, the others twice.  One CTA per (model, orientation), loop over CTFs.
+__global__ void __launch_bounds__(256) k_calc_stats(const cd *F0, const double *K64, int n_orient, int n_ctf, int N, const double *lp_orient,
+                                                    const double *lp_ctf, double log_shifts, double *Tc64, double *h64, float *alpha32,
+                                                    float *h32)
+{
+    __shared__ double sh[256];
+    const int NC = N / 2 + 1, H = NC * N;
+    const int mo = blockIdx.x, o = mo % n_orient;
+    const cd *F = F0 + (size_t)mo * H;
+    for (int c = 0; c < n_ctf; ++c) {
+        const double *K = K64 + (size_t)c * H;
+        double s = 0.0;
+        for (int i = threadIdx.x + 1; i < H; i += 256) {          // i = 0 is the DC bin
+            const int l = i / N;
+            const double w = (l == 0 || l == N / 2) ? 1.0 : 2.0;
+            const cd v = F[i];
+            const double k = K[i];
+            s += w * (v.x * v.x + v.y * v.y) * k * k;
+        }
+        s = block_sum<256>(s, sh);
+        if (threadIdx.x == 0) {
+            const size_t moc = (size_t)mo * n_ctf + c;
+            const double n = (double)N * N;
+            const double lpo = lp_orient ? lp_orient[o] : -log((double)n_orient);
+            const double lpc = lp_ctf ? lp_ctf[c] : -log((double)n_ctf);
+            const double h = -0.5 * log(s) + lpo + lpc - log_shifts;
+            Tc64[moc] = s; h64[moc] = h;
+            alpha32[moc] = (float)(1.0 / sqrt(n * s)); h32[moc] = (float)h;
+        }
+    }
+}
+
+cudaError_t launch_calc_stats(const cd *F0, const double *K64, int n_mo, int n_orient, int n_ctf, int N, const double *lp_orient,
+                              const double *lp_ctf, double log_shifts, double *Tc64, double *h64, float *alpha32, float *h32,
+                              cudaStream_t st)
+{
+    k_calc_stats<<<n_mo, 256, 0, st>>>(F0, K64, n_orient, n_ctf, N, lp_orient, lp_ctf, log_shifts, Tc64, h64, alpha32, h32);
+    return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------------ debug: I1 = F^-1(F0 K)   (Eq. 3)
+__global__ void __launch_bounds__(256) k_calc_image(const cd *F0, const double *K64, int N, double *out)
+{
+    const int NC = N / 2 + 1;
+    const int pix = blockIdx.x * 256 + threadIdx.x;
+    if (pix >= N * N) return;
+    const int k = pix / N, j = pix % N;
+    double acc = 0.0;
+    for (int l = 0; l < NC; ++l) {
+        const double w = (l == 0 || l == N / 2) ? 1.0 : 2.0;
+        for (int m = 0; m < N; ++m) {
+            const cd v = F0[(size_t)l * N + m];
+            const double kk = K64[(size_t)l * N + m];
+            double sn, cs;
+            sincospi(2.0 * (double)((l * j + m * k) % N) / N, &sn, &cs);
+            acc += w * kk * (v.x * cs - v.y * sn);
+        }
+    }
+    out[pix] = acc / ((double)N * N);
+}
+cudaError_t launch_calc_image(const cd *F0, const double *K64, int N, double *out, cudaStream_t st)
+{
+    k_calc_image<<<(N * N + 255) / 256, 256, 0, st>>>(F0, K64, N, out);
+    return cudaGetLastError();
+}
+
+}  // namespace bioem

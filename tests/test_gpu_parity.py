@@ -1,0 +1,127 @@
+"""Parity of the CUDA path (through the C ABI) against the FP64 oracle on the same seeded inputs.
+Bar (BASELINE.json north_star): |delta log-posterior| <= 1e-3 absolute per (image, model), identical argmax
+(orientation, CTF, dx, dy).  Run on the B200 box: pytest -m gpu."""
+import math
+
+import numpy as np
+import pytest
+
+import bioem_workloads as W
+
+pytestmark = pytest.mark.gpu
+
+TOL_LOGP = 1e-3
+
+
+def _oracle_full(wl):
+    import oracle
+    s = wl["spec"]
+    states = [oracle.run_model(m, s.n_pix, s.pixel_A, s.max_shift, wl["quats"], wl["ctfs"], wl["images"]) for m in wl["models"]]
+    logp = np.stack([st.log_posterior() for st in states], axis=1)
+    best = np.stack([st.best for st in states], axis=1)
+    gap = np.stack([st.best - st.second for st in states], axis=1)
+    o, c, dx, dy = (np.stack(x, axis=1) for x in zip(*[oracle.unflatten(st.best_flat, s.n_ctf, s.max_shift) for st in states]))
+    return dict(logp=logp, best=best, gap=gap, orient=o, ctf=c, dx=dx, dy=dy)
+
+
+def _gpu_full(wl):
+    from paper_1609_06634_b200 import BioEM
+    with BioEM() as b:
+        b.load_workload(wl)
+        b.run()
+        return dict(logp=b.get_log_posterior(), logp32=b.debug_log_posterior_f32(), **b.get_best())
+
+
+def _check(wl):
+    ref, got = _oracle_full(wl), _gpu_full(wl)
+    err = np.abs(got["logp"] - ref["logp"])
+    assert err.max() <= TOL_LOGP, f"max |dlogP| = {err.max():.3e}"
+    for k in ("orient", "ctf", "dx", "dy"):
+        bad = got[k] != ref[k]
+        # R15: a mismatch is only tolerated as an exact tie of the oracle (gap < 1e-6), otherwise it is a failure
+        assert not np.any(bad & (ref["gap"] >= 1e-6)), f"argmax {k} differs: gpu {got[k][bad]} oracle {ref[k][bad]}"
+    assert np.abs(got["log_p"] - ref["best"]).max() <= TOL_LOGP
+    return ref, got
+
+
+def test_tiny_config_all_images():
+    wl = W.build_workload("tiny")
+    ref, got = _check(wl)
+    # planted parameters are recovered (sanity of the whole chain)
+    t = wl["truth"]
+    assert np.array_equal(got["orient"][:, 0], t["orient"]) and np.array_equal(got["dx"][:, 0], t["dx"])
+
+
+@pytest.mark.parametrize("name", ["tiny_mini", "small_mini", "paper_mini", "density_mini", "ensemble_mini"])
+def test_mini_configs_element_by_element(name):
+    _check(W.build_workload(name))
+
+
+@pytest.mark.parametrize("name", ["tiny_mini", "small_mini", "paper_mini", "density_mini"])
+def test_shift_maps_and_calc_images(name):
+    import oracle
+    from paper_1609_06634_b200 import BioEM
+    wl = W.build_workload(name)
+    s = wl["spec"]
+    n = s.n_pix ** 2
+    model = oracle.prepare_model(wl["models"][0])
+    logw = oracle.uniform_logw(len(wl["quats"]), len(wl["ctfs"]), s.max_shift)
+    with BioEM() as b:
+        b.load_workload(wl)
+        b.run()
+        rng = np.random.default_rng(1)
+        for _ in range(3):
+            img, o, c = int(rng.integers(s.n_images)), int(rng.integers(len(wl["quats"]))), int(rng.integers(len(wl["ctfs"])))
+            I1 = oracle.calc_image(model, wl["quats"][o], wl["ctfs"][c], s.n_pix, s.pixel_A)
+            got_img = b.debug_calc_image(0, o, c)
+            assert np.abs(got_img - I1).max() <= 2e-6 * np.abs(I1).max()
+            ref = oracle.shift_map(wl["images"][img], I1, s.max_shift, logw)
+            m64 = b.debug_shift_map(img, 0, o, c, f64=True)
+            assert np.abs(m64 - ref).max() <= 1e-6
+            m32 = b.debug_shift_map(img, 0, o, c)
+            # FP32 hot loop: |d g| <~ (n/2) * (relative error of rho^2 ~ 1e-6) * rho^2/(1-rho^2) + ulp(g); DESIGN.md section 6
+            tol32 = 5e-7 * n + 1e-3
+            assert np.abs(m32 - ref).max() <= tol32, np.abs(m32 - ref).max()
+
+
+def test_bitwise_determinism():
+    wl = W.build_workload("small_mini")
+    a, b = _gpu_full(wl), _gpu_full(wl)
+    assert np.array_equal(a["logp"], b["logp"]) and np.array_equal(a["logp32"], b["logp32"])
+    for k in ("orient", "ctf", "dx", "dy", "log_p"):
+        assert np.array_equal(a[k], b[k])
+
+
+def test_edge_cases_and_errors():
+    import oracle
+    from paper_1609_06634_b200 import BioEM, BioEMError
+    wl = W.build_workload("tiny_mini")
+    s = wl["spec"]
+    with BioEM() as b:
+        with pytest.raises(BioEMError) as ei:
+            b.run()
+        assert ei.value.code == -2                                  # BAD_STATE
+        with pytest.raises(BioEMError) as ei:
+            b.set_image_geometry(100, 1.0)
+        assert ei.value.code == -5                                  # UNSUPPORTED
+        b.load_workload(wl)
+        # degenerate grid: one orientation, one CTF, D = 0, one image -> a single term, log P == that term
+        b.set_orientations_quat(wl["quats"][:1])
+        b.set_ctf_grid(wl["ctfs"][:1, 0], wl["ctfs"][:1, 1], wl["ctfs"][:1, 2])
+        b.set_shift_range(0)
+        b.push_images(wl["images"][:1])
+        b.run()
+        st = oracle.run_model(wl["models"][0], s.n_pix, s.pixel_A, 0, wl["quats"][:1], wl["ctfs"][:1], wl["images"][:1])
+        assert abs(b.get_log_posterior()[0, 0] - st.log_posterior()[0]) <= 1e-6
+        bb = b.get_best()
+        assert (bb["orient"][0, 0], bb["ctf"][0, 0], bb["dx"][0, 0], bb["dy"][0, 0]) == (0, 0, 0, 0)
+        with pytest.raises(BioEMError):
+            b.set_shift_range(40)                                   # 2D+1 > n_pix
+    # device-resident input (torch tensor) gives the same result as host input
+    import torch
+    with BioEM() as b:
+        b.load_workload(wl, images=False)
+        b.push_images(torch.from_numpy(wl["images"]).cuda())
+        b.run()
+        dev = b.get_log_posterior()
+    assert np.array_equal(dev, _gpu_full(wl)["logp"])

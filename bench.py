@@ -1,0 +1,278 @@
+#!/usr/bin/env python
+"""bench.py -- posterior evaluations/s of the BioEM hot path on B200 (BASELINE.json metric).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config small] [--impl ours|reference]
+
+A "step" is one pass of the whole hot path over one batch of synthetic images: bioem_push_images (a0) +
+bioem_run (a1-a7) for the named config (default: BASELINE.json configs[1] "small": 128^2 px, 256 images,
+4608 orientations x 32 CTFs x 33^2 shifts = 4.11e10 evaluations per step).  `value` is timed with the images
+already resident in HBM; `e2e` is the same step through the C ABI with HOST buffers (H2D of the image stack and
+D2H of the results inside the timed region).  One process per GPU (torchrun for N > 1): the path shards over
+images with no data-path collective (paper: P:199), every rank scores its own batch -> "scaling": "weak".
+`--impl reference` times the FP64 CPU oracle (the only reference there is) on a bounded sample of the same workload.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import math
+import os
+import subprocess
+import sys
+import tempfile
+import time
+from pathlib import Path
+
+import numpy as np
+
+ROOT = Path(__file__).resolve().parent
+sys.path.insert(0, str(ROOT))
+
+import bioem_workloads as W  # noqa: E402
+
+METRIC = "posterior evaluations/s (image x orientation x CTF x shift)"
+UNIT = "evaluations/s"
+SM_COUNT, FP32_LANES = 148, 128
+# dram__bytes_read.sum + dram__bytes_write.sum of the fused kernel, per launch, from the committed `ncu --set full`
+# capture (profiles/); None until a capture of the current kernel exists for that config.
+NCU_TRAFFIC_BYTES = {"small": None}
+
+
+def algorithmic_flops_per_pair(N: int, D: int) -> float:
+    """SURVEY 8(d) / DESIGN 7: conj-multiply 6H + pruned inverse transform ((N/2+1) column FFTs of 5 N log2 N,
+    (2D+1) c2r row FFTs of 2.5 N log2 N) + 30 flops per shift for the closed form."""
+    H = N * (N // 2 + 1)
+    S = (2 * D + 1) ** 2
+    lg = math.log2(N)
+    return 6 * H + (N // 2 + 1) * 5 * N * lg + (2 * D + 1) * 2.5 * N * lg + 30 * S
+
+
+def measured_peaks():
+    p = ROOT / "MEASURED_PEAKS.json"
+    if p.exists():
+        return json.loads(p.read_text()), "measured (MEASURED_PEAKS.json)"
+    return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0}, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        self.p = None
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "100",
+                                       "-i", str(index)], stdout=self.f, stderr=subprocess.DEVNULL)
+        except OSError:
+            pass
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.p is None:
+            return out
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.p.kill()
+        self.f.flush()
+        rows = [r.split(",") for r in Path(self.f.name).read_text().splitlines() if r.count(",") >= 6]
+        os.unlink(self.f.name)
+        clk, reasons, mx = [], set(), None
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in rows:
+            try:
+                clk.append(float(r[0])); mx = float(r[1])
+            except ValueError:
+                continue
+            for nm, v in zip(names, r[3:7]):
+                if v.strip().lower() == "active":
+                    reasons.add(nm)
+        if clk:
+            out.update(sm_mhz=float(np.median(clk)), sm_max_mhz=mx, reasons=sorted(reasons), samples=len(clk))
+        return out
+
+
+def build_inputs(config, rank, orient_stride=1):
+    spec = W.get_spec(config)
+    if orient_stride > 1:
+        from dataclasses import replace
+        spec = replace(spec, name=f"{spec.name}/orient_stride{orient_stride}", orient_stride=spec.orient_stride * orient_stride)
+    if rank:
+        from dataclasses import replace
+        spec = replace(spec, index=spec.index + 100 * rank)      # other ranks: same config, different image seeds
+    return W.build_workload(spec)
+
+
+def oracle_sample_rate(wl, n_img, n_orient, n_ctf):
+    """The oracle as it stands on a bounded sample (first images / orientations / CTFs of the workload)."""
+    import oracle
+    s = wl["spec"]
+    oracle.build()
+    oracle.lib()
+    t0 = time.perf_counter()
+    for m in wl["models"][:1]:
+        oracle.run_model(m, s.n_pix, s.pixel_A, s.max_shift, wl["quats"][:n_orient], wl["ctfs"][:n_ctf], wl["images"][:n_img])
+    dt = time.perf_counter() - t0
+    pairs = n_img * n_orient * n_ctf
+    return pairs * s.n_shifts / dt, dt, oracle.num_threads(), f"{n_img} images x {n_orient} orientations x {n_ctf} CTFs x {s.n_shifts} shifts of '{s.name}' (direct summation, model 0)"
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    wl = build_inputs(args.config, 0)
+    s = wl["spec"]
+    ni, no, nc = min(s.n_images, 8), min(s.n_orient, 2), min(s.n_ctf, 4)
+    for _ in range(args.warmup):
+        oracle_sample_rate(wl, 1, 1, 1)
+    t_tot, ev = 0.0, 0.0
+    for _ in range(args.steps):
+        rate, dt, cores, sample = oracle_sample_rate(wl, ni, no, nc)
+        t_tot += dt
+        ev += rate * dt
+    value = ev / t_tot
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * t_tot / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": s.name, "n_pix": s.n_pix, "note": "FP64 CPU oracle, bounded sample per step"},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_1609_06634_b200 import BioEM
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    wl = build_inputs(args.config, rank, args.orient_stride)
+    s = wl["spec"]
+    img_host = torch.from_numpy(wl["images"]).pin_memory()
+    img_dev = img_host.cuda()
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")          # > 126 MB L2
+    b = BioEM(device=local)
+    b.load_workload(wl, images=False)
+
+    def step_device():
+        flush.zero_()                                                          # L2 flush between iterations
+        b.push_images(img_dev)
+        b.run()
+
+    def step_e2e():
+        flush.zero_()
+        b.push_images(img_host)                                                # H2D inside the step
+        b.run()
+        lp = b.get_log_posterior()                                             # D2H inside the step
+        best = b.get_best()
+        return lp, best
+
+    for _ in range(max(args.warmup, 1)):
+        step_device()
+    barrier()
+    sampler = ClockSampler(local) if rank == 0 else None
+    fused_ms, launches = [], 0
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(args.steps):
+        step_device()
+        launches += b.get_launch_count()[0]                                    # kernels of push_images + run
+    e1.record()
+    barrier()
+    clocks = sampler.stop() if sampler else None
+    fused_ms = b.get_timing()[1]                                               # CUDA events around the fused kernel (last step)
+    total_ms_last = b.get_timing()[0]
+    t_dev = e0.elapsed_time(e1) * 1e-3
+
+    # ---- end to end through the C ABI with host buffers
+    lp, best = step_e2e()
+    barrier()
+    t0 = time.perf_counter()
+    e0.record()
+    for _ in range(args.steps):
+        lp, best = step_e2e()
+    e1.record()
+    barrier()
+    t_e2e = max(e0.elapsed_time(e1) * 1e-3, time.perf_counter() - t0)
+    h2d = int(img_host.numel() * 4)
+    d2h = int(lp.nbytes + sum(v.nbytes for v in best.values()))
+
+    if world > 1:
+        t = torch.tensor([t_dev, t_e2e], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        t_dev, t_e2e = float(t[0]), float(t[1])
+    evals_job = float(s.n_evaluations) * world * args.steps
+    if rank == 0:
+        peaks, peak_src = measured_peaks()
+        fp32_peak = SM_COUNT * FP32_LANES * 2 * peaks.get("sm_max_mhz", 1965.0) * 1e6 / 1e12          # TFLOP/s, DESIGN 7
+        fma_meas, _ = b.measure_fp32_peak()
+        fl = algorithmic_flops_per_pair(s.n_pix, s.max_shift) * s.n_pairs
+        achieved = fl / (fused_ms * 1e-3) / 1e12
+        hbm_bytes = s.n_pairs * 8.0 * s.n_pix * (s.n_pix // 2 + 1)               # streaming Ohat once per pair
+        roof = {
+            "bound": "alu", "kernel": "k_fused (a4+a5+a6)", "achieved": achieved, "peak": fp32_peak, "unit": "TFLOP/s",
+            "frac": achieved / fp32_peak, "traffic": NCU_TRAFFIC_BYTES.get(s.name),
+            "peak_source": f"148 SM x 128 lanes x 2 x {peaks.get('sm_max_mhz', 1965.0):.0f} MHz (formula, {peak_src})",
+            "measured_ffma_tflops": fma_meas, "frac_of_measured_ffma": achieved / fma_meas,
+            "kernel_ms": fused_ms, "step_ms_on_device": total_ms_last, "flops_per_pair": algorithmic_flops_per_pair(s.n_pix, s.max_shift),
+            "hbm_alt": {"bytes_per_launch_if_streamed": hbm_bytes, "gbs_equivalent": hbm_bytes / (fused_ms * 1e-3) / 1e9,
+                        "peak_gbs": peaks.get("hbm_gbs")},
+        }
+        ni, no, nc = min(s.n_images, 8), min(s.n_orient, 2), min(s.n_ctf, 4)
+        rate, dt, cores, sample = oracle_sample_rate(wl, ni, no, nc)
+        line = {
+            "metric": METRIC, "value": evals_job / t_dev, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": 1e3 * t_dev / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f32", "data": "synthetic",
+            "config": {"workload": s.name, "n_pix": s.n_pix, "n_images_per_gpu": s.n_images, "n_models": s.n_models,
+                       "n_orient": s.n_orient, "n_ctf": s.n_ctf, "max_shift": s.max_shift, "evaluations_per_step_per_gpu": s.n_evaluations,
+                       "cache": "L2 flushed between iterations (256 MiB write); projection spectra (>= 306 MB) are regenerated every step",
+                       "precision": "hot loop FP32, precompute and top-8 re-scoring FP64", "parallelism": f"images sharded, dp{world}"},
+            "e2e": {"value": evals_job / t_e2e, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
+            "gpu_launches": launches, "clocks": clocks, "roofline": roof,
+            "cpu_baseline": {"value": rate, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample, "seconds": dt},
+        }
+        print(json.dumps(line), flush=True)
+    b.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", default="small", choices=sorted(W.CONFIGS))
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--orient-stride", type=int, default=1,
+                    help="profiling aid: keep every k-th orientation of the grid (the workload name in the JSON line says so)")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

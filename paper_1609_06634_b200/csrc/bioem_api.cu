@@ -59,12 +59,12 @@ struct bioem_ctx {
     // run state
     bool ran = false;
     int run_models = 0, run_orient = 0, run_ctf = 0, run_D = 0, run_img = 0;
-    DBuf F064, F032, K64, K32, Tc64, h64, alpha32, h32;
+    DBuf F064, F032, K64, K32, Kt, Tc64, h64, alpha32, h32;
     DBuf part_m, part_s, part_top, m32, s32, top, g64;
     DBuf logp, logp32, best, best_logp;
     DBuf scratch_a, scratch_b, scratch_c, dump;
     cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
-    int64_t launches = 0, fused_launches = 0;
+    int64_t launches = 0, fused_launches = 0, push_launches = 0;
 };
 
 #define CK(call)                                                                                     \
@@ -110,7 +110,7 @@ int bioem_destroy(bioem_ctx *ctx)
     cudaStreamSynchronize(ctx->stream);
     for (auto &m : ctx->models) { m.xyz.release(); m.rad.release(); m.wt.release(); m.rho.release(); }
     DBuf *all[] = {&ctx->rot, &ctx->lp_orient, &ctx->ctf_a, &ctx->ctf_A, &ctx->ctf_b, &ctx->lp_ctf, &ctx->Ohat64, &ctx->Ohat32, &ctx->Dw,
-                   &ctx->beta, &ctx->F064, &ctx->F032, &ctx->K64, &ctx->K32, &ctx->Tc64, &ctx->h64, &ctx->alpha32, &ctx->h32,
+                   &ctx->beta, &ctx->F064, &ctx->F032, &ctx->K64, &ctx->K32, &ctx->Kt, &ctx->Tc64, &ctx->h64, &ctx->alpha32, &ctx->h32,
                    &ctx->part_m, &ctx->part_s, &ctx->part_top, &ctx->m32, &ctx->s32, &ctx->top, &ctx->g64, &ctx->logp, &ctx->logp32,
                    &ctx->best, &ctx->best_logp, &ctx->scratch_a, &ctx->scratch_b, &ctx->scratch_c, &ctx->dump};
     for (DBuf *b : all) b->release();
@@ -305,6 +305,7 @@ int bioem_push_images(bioem_ctx *ctx, int n_img, const float *pixels, int is_dev
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);      // inputs are copied: safe to free after return
     staging.release();
     CK(e);
+    ctx->push_launches = 4 * (int64_t)((n_img + slab - 1) / slab) + 2;
     ctx->n_img = n_img;
     ctx->ran = false;
     return BIOEM_OK;
@@ -370,6 +371,12 @@ int bioem_run(bioem_ctx *ctx)
     CK(launch_ctf_tables(ctx->ctf_a.as<double>(), ctx->ctf_A.as<double>(), ctx->ctf_b.as<double>(), C, N, ctx->px, ctx->K64.as<double>(),
                          ctx->K32.as<float>(), st));
     ctx->launches += 1;
+    const bool use_rq = rq_supported(N);
+    if (use_rq) {
+        CK(ctx->Kt.ensure(rq_kt_bytes(N, C)));
+        CK(launch_relayout_K(N, ctx->K32.as<float>(), ctx->Kt.as<float>(), C, st));
+        ctx->launches += 1;
+    }
 
     // ---- a1/a1' + a2: spectra of all projections, model by model, orientation batch by batch
     const int OB = 256;
@@ -411,11 +418,12 @@ int bioem_run(bioem_ctx *ctx)
     p.Ohat = ctx->Ohat32.as<cf>(); p.F0 = ctx->F032.as<cf>(); p.K = ctx->K32.as<float>();
     p.alpha = ctx->alpha32.as<float>(); p.hterm = ctx->h32.as<float>(); p.beta = ctx->beta.as<float>();
     p.n_img = I; p.n_model = M; p.n_orient = O; p.n_ctf = C; p.D = D; p.oc = oc; p.chunks_per_model = cpm;
-    p.cA = (float)(-0.5 * ((double)n - 3.0));
+    p.cA = (float)(-0.5 * ((double)n - 3.0) * 1.4426950408889634);
     p.part_m = ctx->part_m.as<float>(); p.part_s = ctx->part_s.as<float>(); p.part_top = ctx->part_top.as<TopEntry>();
     CK(cudaEventRecord(ctx->ev[1], st));
-    int nl = 0;
-    CK(launch_fused(N, p, false, st, &nl));
+    int nl = 1;
+    if (use_rq) CK(launch_fused_rq(N, p, ctx->Kt.as<float>(), false, st));
+    else CK(launch_fused(N, p, false, st, &nl));
     CK(cudaEventRecord(ctx->ev[2], st));
     ctx->launches += nl; ctx->fused_launches += nl;
 
@@ -515,9 +523,10 @@ int bioem_debug_shift_map(bioem_ctx *ctx, int img, int model, int orient, int ct
     p.alpha = ctx->alpha32.as<float>(); p.hterm = ctx->h32.as<float>(); p.beta = ctx->beta.as<float>();
     p.n_img = ctx->run_img; p.n_model = ctx->run_models; p.n_orient = ctx->run_orient; p.n_ctf = ctx->run_ctf; p.D = D; p.oc = 1;
     p.chunks_per_model = 1;
-    p.cA = (float)(-0.5 * ((double)n - 3.0));
+    p.cA = (float)(-0.5 * ((double)n - 3.0) * 1.4426950408889634);
     p.dump = ctx->dump.as<float>(); p.dump_img = img; p.dump_model = model; p.dump_orient = orient; p.dump_ctf = ctf;
-    CK(launch_fused(N, p, true, ctx->stream, nullptr));
+    if (rq_supported(N)) CK(launch_fused_rq(N, p, ctx->Kt.as<float>(), true, ctx->stream));
+    else CK(launch_fused(N, p, true, ctx->stream, nullptr));
     std::vector<float> tmp((size_t)KK * KK);
     rc = fetch(ctx, tmp.data(), ctx->dump.p, tmp.size() * sizeof(float));
     if (rc) return rc;
@@ -527,7 +536,7 @@ int bioem_debug_shift_map(bioem_ctx *ctx, int img, int model, int orient, int ct
     const double nn = (double)n;
     const double base = -0.5 * (nn - 2.0) * std::log(2.0 * M_PI) + 0.5 * (nn - 5.0) * std::log(2.0) + std::lgamma(0.5 * (nn - 3.0)) -
                         0.5 * (nn - 3.0) * std::log(dw[0]);
-    for (size_t i = 0; i < tmp.size(); ++i) out[i] = base + (double)tmp[i];
+    for (size_t i = 0; i < tmp.size(); ++i) out[i] = base + (double)tmp[i] * 0.6931471805599453;   // kernel units are base 2
     return BIOEM_OK;
 }
 
@@ -580,7 +589,7 @@ int bioem_get_timing(bioem_ctx *ctx, double *ms_total, double *ms_fused_kernel)
 int bioem_get_launch_count(bioem_ctx *ctx, int64_t *n_launches, int64_t *n_fused_launches)
 {
     if (!ctx) return BIOEM_EBADARG;
-    if (n_launches) *n_launches = ctx->launches;
+    if (n_launches) *n_launches = ctx->launches + ctx->push_launches;       /* last push_images + last run */
     if (n_fused_launches) *n_fused_launches = ctx->fused_launches;
     return BIOEM_OK;
 }

@@ -21,7 +21,7 @@ namespace bioem {
 typedef cx<float> cf;
 typedef cx<double> cd;
 
-struct TopEntry { float g; uint32_t pair; uint32_t shift; };   // pair = o*C + c within the model, shift = (dy+D)*S1 + (dx+D)
+struct TopEntry { float g; uint32_t pair; uint32_t shift; };   // g in BASE-2 units (log2 of the term); pair = o*C + c within the model, shift = (dy+D)*S1 + (dx+D)
 
 // choice of the two-step factorisation N = N1 * N2 per supported image size
 __host__ __device__ constexpr int n1_of(int N) { return N == 64 ? 16 : N == 128 ? 16 : N == 224 ? 32 : N == 256 ? 32 : 0; }
@@ -32,14 +32,14 @@ struct FusedParams {
     const cf *F0;          // [M*O][H]
     const float *K;        // [C][H]
     const float *alpha;    // [M*O*C]   1/sqrt(n T_c)
-    const float *hterm;    // [M*O*C]   -1/2 log T_c + log w
+    const float *hterm;    // [M*O*C]   (-1/2 log T_c + log w) * log2(e)   -- the fused kernels work in base-2 units
     const float *beta;     // [I]       1/sqrt(D_omega)
     int n_img, n_model, n_orient, n_ctf, D;
     int oc;                // orientations per work item (chunk)
     int chunks_per_model;
-    float cA;              // -(n-3)/2
+    float cA;              // -(n-3)/2 * log2(e)
     // outputs: one partial per work item = (model, chunk, image)
-    float *part_m, *part_s;      // [items]
+    float *part_m, *part_s;      // [items]   partial sum = part_s * 2^part_m
     TopEntry *part_top;          // [items][TOPK]
     // debug dump of one pair (DUMP instantiation only)
     float *dump;                 // [S1*S1]
@@ -49,6 +49,11 @@ struct FusedParams {
 // host launchers (each enqueues on `st`); return cudaError_t
 cudaError_t launch_fused(int N, const FusedParams &p, bool dump, cudaStream_t st, int *n_launches);
 size_t fused_smem_bytes(int N, int D);
+// register-resident-Q variant (N = 64, 128)
+bool rq_supported(int N);
+size_t rq_kt_bytes(int N, int n_ctf);
+cudaError_t launch_relayout_K(int N, const float *K32, float *Kt, int n_ctf, cudaStream_t st);
+cudaError_t launch_fused_rq(int N, const FusedParams &p, const float *Kt, bool dump, cudaStream_t st);
 
 // precompute
 cudaError_t launch_image_stats(const float *img, int n_img, int N, double *centered, double *Dw, cudaStream_t st);

@@ -28,8 +28,8 @@ __global__ void k_merge(const float *part_m, const float *part_s, const TopEntry
         const double m = part_m[item], s = part_s[item];
         if (m != -CUDART_INF) {
             if (M == -CUDART_INF) { M = m; S = s; }
-            else if (m > M) { S = S * exp(M - m) + s; M = m; }
-            else S += s * exp(m - M);
+            else if (m > M) { S = S * exp2(M - m) + s; M = m; }          // base-2 units
+            else S += s * exp2(m - M);
         }
         for (int k = 0; k < BIOEM_TOPK; ++k) {
             TopEntry e = part_top[item * BIOEM_TOPK + k];
@@ -126,7 +126,9 @@ __global__ void k_final(const double *m32, const double *s32, const TopEntry *to
     const double base = const_n - 0.5 * (n - 3.0) * log(Dw[img]);
     const TopEntry *t = top + (size_t)im * BIOEM_TOPK;
     const double *g = g64 + (size_t)im * BIOEM_TOPK;
-    double M = m32[im];
+    const double LN2 = 0.6931471805599453;
+    const double m32n = m32[im] * LN2;                     // FP32 partials are in base-2 units; convert in double
+    double M = m32n;
     int kb = -1;
     for (int k = 0; k < BIOEM_TOPK; ++k) {
         if (t[k].pair == 0xffffffffu) break;
@@ -134,16 +136,16 @@ __global__ void k_final(const double *m32, const double *s32, const TopEntry *to
         if (kb < 0 || g[k] > g[kb] || (g[k] == g[kb] && (t[k].pair < t[kb].pair || (t[k].pair == t[kb].pair && t[k].shift < t[kb].shift))))
             kb = k;
     }
-    double tot32 = s32[im] * exp(m32[im] - M), top32 = 0.0, top64 = 0.0;
+    double tot32 = s32[im] * exp(m32n - M), top32 = 0.0, top64 = 0.0;
     for (int k = 0; k < BIOEM_TOPK; ++k) {
         if (t[k].pair == 0xffffffffu) break;
-        top32 += exp((double)t[k].g - M);
+        top32 += exp((double)t[k].g * LN2 - M);
         top64 += exp(g[k] - M);
     }
     double rest = tot32 - top32;
     if (rest < 0.0) rest = 0.0;
     logp[im] = base + M + log(top64 + rest);
-    logp32[im] = base + m32[im] + log(s32[im]);
+    logp32[im] = base + m32n + log(s32[im]);
     if (kb >= 0) {
         best[4 * im + 0] = (int32_t)(t[kb].pair / n_ctf);
         best[4 * im + 1] = (int32_t)(t[kb].pair % n_ctf);

@@ -44,8 +44,8 @@ __device__ __forceinline__ void warp_topk_insert(float g, uint32_t pair, uint32_
 
 __device__ __forceinline__ void lse_add(float &m, float &s, float g)
 {
-    if (g > m) { s = s * __expf(m - g) + 1.f; m = g; }
-    else s += __expf(g - m);
+    if (g > m) { s = s * exp2f(m - g) + 1.f; m = g; }          // base-2 units: sum = s * 2^m
+    else s += exp2f(g - m);
 }
 
 __device__ __forceinline__ void lse_merge(float &m, float &s, float m2, float s2)
@@ -53,7 +53,7 @@ __device__ __forceinline__ void lse_merge(float &m, float &s, float m2, float s2
     if (m2 == -CUDART_INF_F) return;
     if (m == -CUDART_INF_F) { m = m2; s = s2; return; }
     float M = fmaxf(m, m2);
-    s = s * __expf(m - M) + s2 * __expf(m2 - M);
+    s = s * exp2f(m - M) + s2 * exp2f(m2 - M);
     m = M;
 }
 
@@ -185,7 +185,7 @@ __global__ void __launch_bounds__(NT) k_fused(FusedParams p, int CB, int GP)
                         acc.y = fmaf(w.x, z.y, fmaf(w.y, z.x, acc.y));
                     }
                     const int ra = 2 * (pb0 + cl), rb = ra + 1;
-                    // rho = B / sqrt(A D) (form C2);  g = -(n-3)/2 log1p(-rho^2) + h
+                    // rho = B / sqrt(A D) (form C2);  g = -(n-3)/2 log1p(-rho^2) + h, in base-2 units (cA and hterm carry log2 e)
                     float r0 = acc.x * ab, r1 = acc.y * ab;
                     float q0 = fminf(r0 * r0, 0.99999994f), q1 = fminf(r1 * r1, 0.99999994f);      // R14 clamp
                     float g0 = fmaf(p.cA, log1pf(-q0), hterm), g1 = fmaf(p.cA, log1pf(-q1), hterm);
@@ -211,8 +211,8 @@ __global__ void __launch_bounds__(NT) k_fused(FusedParams p, int CB, int GP)
         float m2 = __shfl_xor_sync(FULL, lse_m, off), s2 = __shfl_xor_sync(FULL, lse_s, off);
         // make the pairwise merge symmetric so both partners hold the same value
         float M = fmaxf(lse_m, m2);
-        float sa = (lse_m == -CUDART_INF_F) ? 0.f : lse_s * __expf(lse_m - M);
-        float sb = (m2 == -CUDART_INF_F) ? 0.f : s2 * __expf(m2 - M);
+        float sa = (lse_m == -CUDART_INF_F) ? 0.f : lse_s * exp2f(lse_m - M);
+        float sb = (m2 == -CUDART_INF_F) ? 0.f : s2 * exp2f(m2 - M);
         bool lo = (lane & off) == 0;
         lse_s = lo ? sa + sb : sb + sa;
         lse_m = M;

@@ -358,7 +358,7 @@ __global__ void __launch_bounds__(256) k_calc_stats(const cd *F0, const double *
             const double lpc = lp_ctf ? lp_ctf[c] : -log((double)n_ctf);
             const double h = -0.5 * log(s) + lpo + lpc - log_shifts;
             Tc64[moc] = s; h64[moc] = h;
-            alpha32[moc] = (float)(1.0 / sqrt(n * s)); h32[moc] = (float)h;
+            alpha32[moc] = (float)(1.0 / sqrt(n * s)); h32[moc] = (float)(h * 1.4426950408889634);   // FP32 path: base-2 units
         }
     }
 }

@@ -371,7 +371,7 @@ int bioem_run(bioem_ctx *ctx)
     CK(launch_ctf_tables(ctx->ctf_a.as<double>(), ctx->ctf_A.as<double>(), ctx->ctf_b.as<double>(), C, N, ctx->px, ctx->K64.as<double>(),
                          ctx->K32.as<float>(), st));
     ctx->launches += 1;
-    const bool use_rq = rq_supported(N);
+    const bool use_rq = rq_supported(N, D);
     if (use_rq) {
         CK(ctx->Kt.ensure(rq_kt_bytes(N, C)));
         CK(launch_relayout_K(N, ctx->K32.as<float>(), ctx->Kt.as<float>(), C, st));
@@ -525,7 +525,7 @@ int bioem_debug_shift_map(bioem_ctx *ctx, int img, int model, int orient, int ct
     p.chunks_per_model = 1;
     p.cA = (float)(-0.5 * ((double)n - 3.0) * 1.4426950408889634);
     p.dump = ctx->dump.as<float>(); p.dump_img = img; p.dump_model = model; p.dump_orient = orient; p.dump_ctf = ctf;
-    if (rq_supported(N)) CK(launch_fused_rq(N, p, ctx->Kt.as<float>(), true, ctx->stream));
+    if (rq_supported(N, D)) CK(launch_fused_rq(N, p, ctx->Kt.as<float>(), true, ctx->stream));
     else CK(launch_fused(N, p, true, ctx->stream, nullptr));
     std::vector<float> tmp((size_t)KK * KK);
     rc = fetch(ctx, tmp.data(), ctx->dump.p, tmp.size() * sizeof(float));

@@ -50,7 +50,7 @@ struct FusedParams {
 cudaError_t launch_fused(int N, const FusedParams &p, bool dump, cudaStream_t st, int *n_launches);
 size_t fused_smem_bytes(int N, int D);
 // register-resident-Q variant (N = 64, 128)
-bool rq_supported(int N);
+bool rq_supported(int N, int D);
 size_t rq_kt_bytes(int N, int n_ctf);
 cudaError_t launch_relayout_K(int N, const float *K32, float *Kt, int n_ctf, cudaStream_t st);
 cudaError_t launch_fused_rq(int N, const FusedParams &p, const float *Kt, bool dump, cudaStream_t st);

@@ -15,6 +15,9 @@
 //       A2  16-point FFT, B2 Horner sum -> B(dx,dy) for two dy at once
 //       a5  rho^2 = B^2 alpha_c^2 beta_w^2, g = cA log1p(-rho^2) + h_c (form C2; base-2 units inside the kernel)
 //       a6  running log-sum-exp in registers, K best terms in per-warp sorted lists
+// B-phase mapping (v3): a lane owns one residue k1 = lane % 16 of one column (or row pair) per round and forms BOTH pruned
+// outputs k = k1 - 16 and k = k1 from the same N2 shared-memory loads (two Horner chains, twiddles in registers); the single
+// k = +16 output of D = 16 is an extra round.  No index arithmetic is left in the CTF loop.  Requires D <= 16.
 // No float atomics, fixed reduction orders: bit-reproducible.
 #include "common.cuh"
 #include <math_constants.h>
@@ -25,7 +28,7 @@ static constexpr unsigned FULLM = 0xffffffffu;
 
 template <int N> struct RQ {
     static constexpr int N1 = 16, N2 = N / 16, NC = N / 2 + 1, NTASK = NC * N2, NW = (NTASK + 31) / 32, NT = NW * 32;
-    static constexpr int ZP = 17, ZW = 32 * ZP, CPW = 32 / N2;      // Z pitch, Z words per warp, columns per warp
+    static constexpr int ZP = 18, ZW = 32 * ZP, CPW = 32 / N2;      // Z pitch (even: 16-byte aligned pairs), Z words per warp, columns per warp
 };
 
 __device__ __forceinline__ float ex2f(float x)
@@ -63,22 +66,34 @@ __device__ __forceinline__ void warp_topk_insert_rq(float g, uint32_t pair, uint
     }
 }
 
-// log1p(-x) for 0 <= x < 1: 5-term series below 2^-6 (truncation < 2e-10 relative), libdevice log1pf above.
-__device__ __forceinline__ float log1p_neg(float x)
+// log1p(-x), 0 <= x < 2^-6: 5-term series (truncation < 2e-10 relative)
+__device__ __forceinline__ float log1p_neg_small(float x)
 {
-    if (x < 0.015625f) {
-        float p = fmaf(x, 0.2f, 0.25f);
-        p = fmaf(x, p, 0.33333334f);
-        p = fmaf(x, p, 0.5f);
-        p = fmaf(x, p, 1.0f);
-        return -x * p;
-    }
-    return log1pf(-x);
+    float p = fmaf(x, 0.2f, 0.25f);
+    p = fmaf(x, p, 0.33333334f);
+    p = fmaf(x, p, 0.5f);
+    p = fmaf(x, p, 1.0f);
+    return -x * p;
 }
 
-// Horner sum over the N2 residues: sum_t r^t z[t*ZP]
+// Two Horner sums over the N2 residues sharing their loads: ylo = sum_t rlo^t z[t], yhi = sum_t rhi^t z[t]
 template <int N2, int ZP>
-__device__ __forceinline__ cf horner(const cf *zc, cf r)
+__device__ __forceinline__ void horner2(const cf *zc, cf rlo, cf rhi, cf &ylo, cf &yhi)
+{
+    cf z = zc[(N2 - 1) * ZP];
+    ylo = z; yhi = z;
+#pragma unroll
+    for (int t = N2 - 2; t >= 0; --t) {
+        z = zc[t * ZP];
+        float ax = fmaf(rlo.x, ylo.x, fmaf(-rlo.y, ylo.y, z.x));
+        float ay = fmaf(rlo.x, ylo.y, fmaf(rlo.y, ylo.x, z.y));
+        float bx = fmaf(rhi.x, yhi.x, fmaf(-rhi.y, yhi.y, z.x));
+        float by = fmaf(rhi.x, yhi.y, fmaf(rhi.y, yhi.x, z.y));
+        ylo.x = ax; ylo.y = ay; yhi.x = bx; yhi.y = by;
+    }
+}
+template <int N2, int ZP>
+__device__ __forceinline__ cf horner1(const cf *zc, cf r)
 {
     cf acc = zc[(N2 - 1) * ZP];
 #pragma unroll
@@ -91,20 +106,70 @@ __device__ __forceinline__ cf horner(const cf *zc, cf r)
     return acc;
 }
 
+// spill the bit-reversed FFT output as 8 16-byte stores: a[r] = y[bitrev4(r)], so (a[r], a[r+8]) = (y[2b], y[2b+1]), b = bitrev3(r)
+__device__ __forceinline__ void spill16(cf *zst, const cf (&a)[16])
+{
+#pragma unroll
+    for (int r = 0; r < 8; ++r) {
+        const int b = bitrev(r, 3);
+        *reinterpret_cast<float4 *>(zst + 2 * b) = make_float4(a[r].x, a[r].y, a[r + 8].x, a[r + 8].y);
+    }
+}
+
+// per-shift closed form for the (up to) four values a lane produces per round, running log-sum-exp and candidates
+struct LseState { float m, s, thr; };
+
+template <bool DUMP>
+__device__ __forceinline__ void score4(const FusedParams &p, LseState &st, TopEntry *mylist, const float (&b)[4], const bool (&v)[4],
+                                       const uint32_t (&sh)[4], float ab, float hterm, uint32_t pair)
+{
+    float g[4];
+    float xmax = 0.f;
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        const float r = b[i] * ab;
+        const float x = fminf(r * r, 0.99999994f);                         // rho^2, R14 clamp
+        xmax = fmaxf(xmax, x);
+        g[i] = fmaf(p.cA, log1p_neg_small(x), hterm);                       // form C2, base-2 units
+    }
+    if (__any_sync(FULLM, xmax >= 0.015625f)) {                             // rare (near the posterior peak): accurate log1p
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            const float r = b[i] * ab;
+            const float x = fminf(r * r, 0.99999994f);
+            if (x >= 0.015625f) g[i] = fmaf(p.cA, log1pf(-x), hterm);
+        }
+    }
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        if (!v[i]) g[i] = -CUDART_INF_F;
+        if (DUMP && v[i]) p.dump[sh[i]] = g[i];
+    }
+    const float gmax = fmaxf(fmaxf(g[0], g[1]), fmaxf(g[2], g[3]));
+    if (gmax > -CUDART_INF_F) {
+        const float mn = fmaxf(st.m, gmax);
+        st.s = st.s * ex2f(st.m - mn) + ((ex2f(g[0] - mn) + ex2f(g[1] - mn)) + (ex2f(g[2] - mn) + ex2f(g[3] - mn)));
+        st.m = mn;
+    }
+    if (__any_sync(FULLM, gmax >= st.thr)) {
+#pragma unroll
+        for (int i = 0; i < 4; ++i) warp_topk_insert_rq(g[i], pair, sh[i], v[i], st.thr, mylist);
+    }
+}
+
 template <int N, bool DUMP>
-__global__ void __launch_bounds__(RQ<N>::NT, 1) k_fused_rq(FusedParams p, const float4 *__restrict__ Kt, int CG, int GP, unsigned magicKK)
+__global__ void __launch_bounds__(RQ<N>::NT, 1) k_fused_rq(FusedParams p, const float4 *__restrict__ Kt, int CG, int GP)
 {
     typedef RQ<N> C_;
     constexpr int N1 = C_::N1, N2 = C_::N2, NC = C_::NC, NTASK = C_::NTASK, NW = C_::NW, NT = C_::NT, ZP = C_::ZP, ZW = C_::ZW, CPW = C_::CPW;
     constexpr size_t H = (size_t)NC * N;
-    const int D = p.D, KK = 2 * D + 1, NP = (KK + 1) / 2;
+    const int D = p.D, KK = 2 * D + 1, NP = (KK + 1) / 2;                 // host guarantees D <= 16
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
 
     extern __shared__ __align__(16) unsigned char smem_raw[];
     cf *Z = reinterpret_cast<cf *>(smem_raw);                        // [NW][32][ZP]  warp-private tiles
     cf *G = Z + (size_t)NW * ZW;                                     // [CG][KK][GP]
-    cf *twH = G + (size_t)CG * KK * GP;                              // [KK]  w_N^{k}, k = kk - D
-    float2 *sc = reinterpret_cast<float2 *>(twH + KK);               // [CG]  (alpha*beta, h) of the group's CTFs
+    float2 *sc = reinterpret_cast<float2 *>(G + (size_t)CG * KK * GP);   // [CG]  (alpha*beta, h) of the group's CTFs
     TopEntry *tops = reinterpret_cast<TopEntry *>(sc + CG);          // [NW][TOPK]
     float *red = reinterpret_cast<float *>(tops + NW * BIOEM_TOPK);  // [2 NW]
 
@@ -119,31 +184,40 @@ __global__ void __launch_bounds__(RQ<N>::NT, 1) k_fused_rq(FusedParams p, const 
         o_end = min(o_begin + p.oc, p.n_orient);
     }
     const float beta = p.beta[img];
-    for (int i = tid; i < KK; i += NT) {
-        float sn, cs;
-        sincospif(2.0f * (float)(((i - D) % N + N) % N) / (float)N, &sn, &cs);
-        twH[i] = {cs, sn};
-    }
     if (tid < NW * BIOEM_TOPK) { TopEntry e0 = {-CUDART_INF_F, 0xffffffffu, 0xffffffffu}; tops[tid] = e0; }
     __syncthreads();
 
-    // ---- per-thread constants
+    // ---- A-phase constants: thread = (column, residue t)
     const bool act1 = tid < NTASK;
     const int col = act1 ? tid / N2 : 0, t = tid % N2;
     const size_t qbase = (size_t)col * N + t;
     cf *Zw = Z + (size_t)warp * ZW;
     cf *zst = Zw + lane * ZP;
     const int ncols_w = max(0, min(CPW, NC - warp * CPW));           // whole columns owned by this warp
-    const int nout1 = ncols_w * KK;
+    // ---- B-phase constants: lane = (half, k1); outputs k = k1 - 16 ("lo") and k = k1 ("hi")
+    const int half = lane >> 4, k1 = lane & 15;
+    const bool vlo = k1 >= 16 - D, vhi = k1 <= D;
+    const int kk_lo = k1 - 16 + D, kk_hi = k1 + D;                    // row / dx index of the two outputs
+    cf rlo, rhi, rx;
+    {
+        float sn, cs;
+        sincospif(2.0f * (float)(k1 - 16 + N) / (float)N, &sn, &cs); rlo = {cs, sn};
+        sincospif(2.0f * (float)k1 / (float)N, &sn, &cs);            rhi = {cs, sn};
+        sincospif(2.0f * 16.0f / (float)N, &sn, &cs);                rx = {cs, sn};      // k = +16 (only when D == 16)
+    }
+    const bool has_x = D == 16;
+    const cf *zrd = Zw + half * N2 * ZP + k1;                         // + cp * 2 * N2 * ZP per round
+
     const cf *Oimg = p.Ohat + (size_t)img * H;
-    float lse_m = -CUDART_INF_F, lse_s = 0.f, thr = -CUDART_INF_F;
+    LseState st = {-CUDART_INF_F, 0.f, -CUDART_INF_F};
     TopEntry *mylist = tops + warp * BIOEM_TOPK;
     const int c_lo = DUMP ? p.dump_ctf : 0, c_hi = DUMP ? p.dump_ctf + 1 : p.n_ctf;
+    const float4 *Kt_t = Kt + tid;
+    constexpr size_t KSTR = (size_t)(N1 / 4) * NT;                   // float4 per CTF
 
-    // K of the first CTF
     float4 kq[N1 / 4];
 #pragma unroll
-    for (int g4 = 0; g4 < N1 / 4; ++g4) kq[g4] = Kt[((size_t)c_lo * (N1 / 4) + g4) * NT + tid];
+    for (int g4 = 0; g4 < N1 / 4; ++g4) kq[g4] = Kt_t[(size_t)c_lo * KSTR + (size_t)g4 * NT];
 
     for (int o = o_begin; o < o_end; ++o) {
         // ---- Q = conj(Ohat) F0 for this thread's 16 bins (Eq. 12)
@@ -171,21 +245,28 @@ __global__ void __launch_bounds__(RQ<N>::NT, 1) k_fused_rq(FusedParams p, const 
                 {   // prefetch K of the next CTF (wraps to the first CTF for the next orientation)
                     int cn = c0 + ci + 1;
                     if (cn >= c_hi) cn = c_lo;
+                    const float4 *kp = Kt_t + (size_t)cn * KSTR;
 #pragma unroll
-                    for (int g4 = 0; g4 < N1 / 4; ++g4) kq[g4] = Kt[((size_t)cn * (N1 / 4) + g4) * NT + tid];
+                    for (int g4 = 0; g4 < N1 / 4; ++g4) kq[g4] = kp[(size_t)g4 * NT];
                 }
                 fft_dif<float, N1, +1>(a);
-#pragma unroll
-                for (int r = 0; r < N1; ++r) zst[bitrev(r, 4)] = a[r];
+                spill16(zst, a);
                 __syncwarp();
-                cf *Gc = G + (size_t)ci * KK * GP + warp * CPW;
-                for (int idx0 = 0; idx0 < nout1; idx0 += 32) {
-                    const int idx = idx0 + lane;
-                    const int cl = magicKK ? (int)__umulhi((unsigned)idx, magicKK) : idx, kk = idx - cl * KK;   // idx / KK (magic = 0: KK == 1)
-                    const bool valid = idx < nout1;
-                    const int k1 = (kk - D) & (N1 - 1);
-                    const cf y = horner<N2, ZP>(Zw + (valid ? cl * N2 * ZP + k1 : 0), twH[valid ? kk : 0]);
-                    if (valid) Gc[kk * GP + cl] = y;
+                cf *Gc = G + (size_t)ci * KK * GP + warp * CPW + half;
+#pragma unroll
+                for (int cp = 0; cp < CPW / 2; ++cp) {
+                    if (2 * cp < ncols_w) {                                       // warp-uniform
+                        cf ylo, yhi;
+                        horner2<N2, ZP>(zrd + cp * 2 * N2 * ZP, rlo, rhi, ylo, yhi);
+                        const bool cv = 2 * cp + half < ncols_w;
+                        if (cv && vlo) Gc[kk_lo * GP + 2 * cp] = ylo;
+                        if (cv && vhi) Gc[kk_hi * GP + 2 * cp] = yhi;
+                    }
+                }
+                if (has_x) {                                                      // k = +16: one output per column, k1 = 0
+                    const int cl = lane < ncols_w ? lane : 0;
+                    const cf y = horner1<N2, ZP>(Zw + cl * N2 * ZP, rx);
+                    if (lane < ncols_w) G[(size_t)ci * KK * GP + (KK - 1) * GP + warp * CPW + lane] = y;
                 }
                 __syncwarp();
             }
@@ -216,39 +297,41 @@ __global__ void __launch_bounds__(RQ<N>::NT, 1) k_fused_rq(FusedParams p, const 
                         a[j] = {va.x - bsel * sg * vb.y, sg * va.y + bsel * vb.x};
                     }
                     fft_dif<float, N1, +1>(a);
-#pragma unroll
-                    for (int r = 0; r < N1; ++r) zst[bitrev(r, 4)] = a[r];
+                    spill16(zst, a);
                 }
                 __syncwarp();
                 const int cb0 = warp * CPW;
-                const int nout2 = max(0, min(CPW, ncombo - cb0)) * KK;
-                for (int idx0 = 0; idx0 < nout2; idx0 += 32) {
-                    const int idx = idx0 + lane;
-                    const bool valid = idx < nout2;
-                    const int cw = magicKK ? (int)__umulhi((unsigned)idx, magicKK) : idx, kk = idx - cw * KK;     // combo within warp, dx index
-                    const int k1 = (kk - D) & (N1 - 1);
-                    const cf y = horner<N2, ZP>(Zw + (valid ? cw * N2 * ZP + k1 : 0), twH[valid ? kk : 0]);
-                    const int combo2 = cb0 + (valid ? cw : 0);
+                const int ncw = max(0, min(CPW, ncombo - cb0));     // combos of this warp
+#pragma unroll
+                for (int cp = 0; cp < CPW / 2; ++cp) {
+                    if (2 * cp < ncw) {                              // warp-uniform
+                        cf ylo, yhi;
+                        horner2<N2, ZP>(zrd + cp * 2 * N2 * ZP, rlo, rhi, ylo, yhi);
+                        const int cw = 2 * cp + half;
+                        const bool cv = cw < ncw;
+                        const int combo2 = cb0 + (cv ? cw : 0);
+                        const int cl = combo2 / NP, pr = combo2 - cl * NP;
+                        const int ra = 2 * pr, rb = ra + 1;
+                        const float2 s2 = sc[cl];
+                        const float b[4] = {ylo.x, ylo.y, yhi.x, yhi.y};
+                        const bool v[4] = {cv && vlo, cv && vlo && rb < KK, cv && vhi, cv && vhi && rb < KK};
+                        const uint32_t sh[4] = {(uint32_t)(ra * KK + kk_lo), (uint32_t)(rb * KK + kk_lo), (uint32_t)(ra * KK + kk_hi),
+                                                (uint32_t)(rb * KK + kk_hi)};
+                        score4<DUMP>(p, st, mylist, b, v, sh, s2.x, s2.y, (uint32_t)(o * p.n_ctf + c0 + cl));
+                    }
+                }
+                if (has_x && ncw > 0) {                              // dx = +16
+                    const bool cv = lane < ncw;
+                    const int cw = cv ? lane : 0;
+                    const cf y = horner1<N2, ZP>(Zw + cw * N2 * ZP, rx);
+                    const int combo2 = cb0 + cw;
                     const int cl = combo2 / NP, pr = combo2 - cl * NP;
                     const int ra = 2 * pr, rb = ra + 1;
                     const float2 s2 = sc[cl];
-                    const float r0 = y.x * s2.x, r1 = y.y * s2.x;
-                    const float x0 = fminf(r0 * r0, 0.99999994f), x1 = fminf(r1 * r1, 0.99999994f);          // R14 clamp
-                    const float g0 = fmaf(p.cA, log1p_neg(x0), s2.y), g1 = fmaf(p.cA, log1p_neg(x1), s2.y);  // base-2 units
-                    const bool v0 = valid, v1 = valid && rb < KK;
-                    if (DUMP) {
-                        if (v0) p.dump[ra * KK + kk] = g0;
-                        if (v1) p.dump[rb * KK + kk] = g1;
-                    }
-                    if (v0) {
-                        const float gb1 = v1 ? g1 : -CUDART_INF_F;
-                        const float mn = fmaxf(lse_m, fmaxf(g0, gb1));
-                        lse_s = lse_s * ex2f(lse_m - mn) + ex2f(g0 - mn) + ex2f(gb1 - mn);
-                        lse_m = mn;
-                    }
-                    const uint32_t pair = (uint32_t)(o * p.n_ctf + c0 + cl);
-                    warp_topk_insert_rq(g0, pair, (uint32_t)(ra * KK + kk), v0, thr, mylist);
-                    warp_topk_insert_rq(g1, pair, (uint32_t)(rb * KK + kk), v1, thr, mylist);
+                    const float b[4] = {y.x, y.y, 0.f, 0.f};
+                    const bool v[4] = {cv, cv && rb < KK, false, false};
+                    const uint32_t sh[4] = {(uint32_t)(ra * KK + KK - 1), (uint32_t)(rb * KK + KK - 1), 0u, 0u};
+                    score4<DUMP>(p, st, mylist, b, v, sh, s2.x, s2.y, (uint32_t)(o * p.n_ctf + c0 + cl));
                 }
             }
             __syncthreads();
@@ -257,6 +340,7 @@ __global__ void __launch_bounds__(RQ<N>::NT, 1) k_fused_rq(FusedParams p, const 
     if (DUMP) return;
 
     // ---- block reduction, fixed order
+    float lse_m = st.m, lse_s = st.s;
 #pragma unroll
     for (int off = 16; off >= 1; off >>= 1) {
         const float m2 = __shfl_xor_sync(FULLM, lse_m, off), s2 = __shfl_xor_sync(FULLM, lse_s, off);
@@ -307,7 +391,7 @@ __global__ void k_relayout_K(const float *K32, float4 *Kt, int n_ctf)
     Kt[(size_t)c * (C_::N1 / 4) * C_::NT + i] = make_float4(v[0], v[1], v[2], v[3]);
 }
 
-bool rq_supported(int N) { return N == 64 || N == 128; }
+bool rq_supported(int N, int D) { return (N == 64 || N == 128) && D <= 16; }
 size_t rq_kt_bytes(int N, int n_ctf) { return N == 64 ? (size_t)n_ctf * 4 * RQ<64>::NT * 16 : (size_t)n_ctf * 4 * RQ<128>::NT * 16; }
 
 cudaError_t launch_relayout_K(int N, const float *K32, float *Kt, int n_ctf, cudaStream_t st)
@@ -333,7 +417,7 @@ static void rq_plan(int D, int n_ctf, int &CG, int &GP, size_t &bytes)
     if (CG > n_ctf) CG = n_ctf;
     const size_t budget = 220 * 1024;
     for (;;) {
-        bytes = (size_t)C_::NW * C_::ZW * 8 + (size_t)CG * KK * GP * 8 + (size_t)KK * 8 + (size_t)CG * 8 +
+        bytes = (size_t)C_::NW * C_::ZW * 8 + (size_t)CG * KK * GP * 8 + (size_t)CG * 8 +
                 (size_t)C_::NW * BIOEM_TOPK * sizeof(TopEntry) + 2 * C_::NW * 4 + 64;
         if (bytes <= budget || CG == 1) break;
         --CG;
@@ -347,18 +431,16 @@ static cudaError_t launch_rq_t(const FusedParams &p, const float *Kt, bool dump,
     size_t bytes;
     rq_plan<N>(p.D, p.n_ctf, CG, GP, bytes);
     if (bytes > 227 * 1024) return cudaErrorInvalidConfiguration;
-    const int KK = 2 * p.D + 1;
-    const unsigned magic = KK == 1 ? 0u : (unsigned)((0x100000000ull + KK - 1) / KK);     // exact idx / KK for idx < 2^16
     cudaError_t e;
     if (dump) {
         e = cudaFuncSetAttribute(k_fused_rq<N, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
         if (e != cudaSuccess) return e;
-        k_fused_rq<N, true><<<1, RQ<N>::NT, bytes, st>>>(p, reinterpret_cast<const float4 *>(Kt), CG, GP, magic);
+        k_fused_rq<N, true><<<1, RQ<N>::NT, bytes, st>>>(p, reinterpret_cast<const float4 *>(Kt), CG, GP);
     } else {
         e = cudaFuncSetAttribute(k_fused_rq<N, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
         if (e != cudaSuccess) return e;
         const int items = p.n_img * p.n_model * p.chunks_per_model;
-        k_fused_rq<N, false><<<items, RQ<N>::NT, bytes, st>>>(p, reinterpret_cast<const float4 *>(Kt), CG, GP, magic);
+        k_fused_rq<N, false><<<items, RQ<N>::NT, bytes, st>>>(p, reinterpret_cast<const float4 *>(Kt), CG, GP);
     }
     return cudaGetLastError();
 }

@@ -28,7 +28,9 @@ static constexpr unsigned FULLM = 0xffffffffu;
 
 template <int N> struct RQ {
     static constexpr int N1 = 16, N2 = N / 16, NC = N / 2 + 1, NTASK = NC * N2, NW = (NTASK + 31) / 32, NT = NW * 32;
-    static constexpr int ZP = 18, ZW = 32 * ZP, CPW = 32 / N2;      // Z pitch (even: 16-byte aligned pairs), Z words per warp, columns per warp
+    static constexpr int ZP = 18, CPW = 32 / N2;      // Z pitch (even: 16-byte aligned pairs), columns per warp
+    static constexpr int CS = N2 * ZP + 2;            // column-tile pitch: +2 keeps the k = +16 round (one lane per column) conflict-free
+    static constexpr int ZW = CPW * CS;               // Z words (complex) per warp
 };
 
 __device__ __forceinline__ float ex2f(float x)
@@ -158,19 +160,20 @@ __device__ __forceinline__ void score4(const FusedParams &p, LseState &st, TopEn
 }
 
 template <int N, bool DUMP>
-__global__ void __launch_bounds__(RQ<N>::NT, 1) k_fused_rq(FusedParams p, const float4 *__restrict__ Kt, int CG, int GP)
+__global__ void __launch_bounds__(RQ<N>::NT, 1) k_fused_rq(FusedParams p, const float4 *__restrict__ Kt, int CG, int GP, unsigned magicNP, int NBUF)
 {
     typedef RQ<N> C_;
-    constexpr int N1 = C_::N1, N2 = C_::N2, NC = C_::NC, NTASK = C_::NTASK, NW = C_::NW, NT = C_::NT, ZP = C_::ZP, ZW = C_::ZW, CPW = C_::CPW;
+    constexpr int N1 = C_::N1, N2 = C_::N2, NC = C_::NC, NTASK = C_::NTASK, NW = C_::NW, NT = C_::NT, ZP = C_::ZP, ZW = C_::ZW, CPW = C_::CPW, CS = C_::CS;
     constexpr size_t H = (size_t)NC * N;
     const int D = p.D, KK = 2 * D + 1, NP = (KK + 1) / 2;                 // host guarantees D <= 16
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
 
     extern __shared__ __align__(16) unsigned char smem_raw[];
     cf *Z = reinterpret_cast<cf *>(smem_raw);                        // [NW][32][ZP]  warp-private tiles
-    cf *G = Z + (size_t)NW * ZW;                                     // [CG][KK][GP]
-    float2 *sc = reinterpret_cast<float2 *>(G + (size_t)CG * KK * GP);   // [CG]  (alpha*beta, h) of the group's CTFs
-    TopEntry *tops = reinterpret_cast<TopEntry *>(sc + CG);          // [NW][TOPK]
+    cf *G = Z + (size_t)NW * ZW;                                     // [2][CG][KK][GP]  double-buffered over CTF groups
+    const int GSZ = CG * KK * GP;
+    float2 *sc = reinterpret_cast<float2 *>(G + (size_t)NBUF * GSZ); // [2][CG]  (alpha*beta, h) of the group's CTFs
+    TopEntry *tops = reinterpret_cast<TopEntry *>(sc + 2 * CG);      // [NW][TOPK]
     float *red = reinterpret_cast<float *>(tops + NW * BIOEM_TOPK);  // [2 NW]
 
     int img, model, o_begin, o_end, item;
@@ -192,21 +195,22 @@ __global__ void __launch_bounds__(RQ<N>::NT, 1) k_fused_rq(FusedParams p, const 
     const int col = act1 ? tid / N2 : 0, t = tid % N2;
     const size_t qbase = (size_t)col * N + t;
     cf *Zw = Z + (size_t)warp * ZW;
-    cf *zst = Zw + lane * ZP;
+    cf *zst = Zw + (lane / N2) * CS + (lane % N2) * ZP;
     const int ncols_w = max(0, min(CPW, NC - warp * CPW));           // whole columns owned by this warp
     // ---- B-phase constants: lane = (half, k1); outputs k = k1 - 16 ("lo") and k = k1 ("hi")
     const int half = lane >> 4, k1 = lane & 15;
     const bool vlo = k1 >= 16 - D, vhi = k1 <= D;
     const int kk_lo = k1 - 16 + D, kk_hi = k1 + D;                    // row / dx index of the two outputs
-    cf rlo, rhi, rx;
+    cf rlo, rhi;
     {
         float sn, cs;
         sincospif(2.0f * (float)(k1 - 16 + N) / (float)N, &sn, &cs); rlo = {cs, sn};
         sincospif(2.0f * (float)k1 / (float)N, &sn, &cs);            rhi = {cs, sn};
-        sincospif(2.0f * 16.0f / (float)N, &sn, &cs);                rx = {cs, sn};      // k = +16 (only when D == 16)
     }
+    const cf rx = {(float)cos32(512 / N), (float)cos32(8 - 512 / N)};        // w_N^{16} = exp(2 pi i 16/N), k = +16 (only when D == 16)
     const bool has_x = D == 16;
-    const cf *zrd = Zw + half * N2 * ZP + k1;                         // + cp * 2 * N2 * ZP per round
+    const cf *zrd = Zw + half * CS + k1;                              // + cp * 2 * CS per round
+    const int a2combo = tid / N2;                                     // this thread's A2 task: (CTF in group) x (row pair)
 
     const cf *Oimg = p.Ohat + (size_t)img * H;
     LseState st = {-CUDART_INF_F, 0.f, -CUDART_INF_F};
@@ -218,6 +222,7 @@ __global__ void __launch_bounds__(RQ<N>::NT, 1) k_fused_rq(FusedParams p, const 
     float4 kq[N1 / 4];
 #pragma unroll
     for (int g4 = 0; g4 < N1 / 4; ++g4) kq[g4] = Kt_t[(size_t)c_lo * KSTR + (size_t)g4 * NT];
+    int gbuf = 0;
 
     for (int o = o_begin; o < o_end; ++o) {
         // ---- Q = conj(Ohat) F0 for this thread's 16 bins (Eq. 12)
@@ -232,6 +237,14 @@ __global__ void __launch_bounds__(RQ<N>::NT, 1) k_fused_rq(FusedParams p, const 
         }
         for (int c0 = c_lo; c0 < c_hi; c0 += CG) {
             const int nc = min(CG, c_hi - c0);
+            cf *Gb = G + (size_t)gbuf * GSZ;
+            float2 *scb = sc + gbuf * CG;
+            gbuf ^= (NBUF - 1);
+            float2 schold = make_float2(0.f, 0.f);                 // (alpha*beta, h) of CTF c0 + tid: fetched now, published before the barrier
+            if (tid < nc) {
+                const size_t moc = ((size_t)model * p.n_orient + o) * p.n_ctf + c0 + tid;
+                schold = make_float2(p.alpha[moc] * beta, p.hterm[moc]);
+            }
             // ================= pass 1, one CTF at a time, warp-local
             for (int ci = 0; ci < nc; ++ci) {
                 cf a[N1];
@@ -242,6 +255,8 @@ __global__ void __launch_bounds__(RQ<N>::NT, 1) k_fused_rq(FusedParams p, const 
                     a[4 * g4 + 2] = {q[4 * g4 + 2].x * kq[g4].z, q[4 * g4 + 2].y * kq[g4].z};
                     a[4 * g4 + 3] = {q[4 * g4 + 3].x * kq[g4].w, q[4 * g4 + 3].y * kq[g4].w};
                 }
+                fft_dif<float, N1, +1>(a);
+                spill16(zst, a);
                 {   // prefetch K of the next CTF (wraps to the first CTF for the next orientation)
                     int cn = c0 + ci + 1;
                     if (cn >= c_hi) cn = c_lo;
@@ -249,15 +264,13 @@ __global__ void __launch_bounds__(RQ<N>::NT, 1) k_fused_rq(FusedParams p, const 
 #pragma unroll
                     for (int g4 = 0; g4 < N1 / 4; ++g4) kq[g4] = kp[(size_t)g4 * NT];
                 }
-                fft_dif<float, N1, +1>(a);
-                spill16(zst, a);
                 __syncwarp();
-                cf *Gc = G + (size_t)ci * KK * GP + warp * CPW + half;
+                cf *Gc = Gb + (size_t)ci * KK * GP + warp * CPW + half;
 #pragma unroll
                 for (int cp = 0; cp < CPW / 2; ++cp) {
                     if (2 * cp < ncols_w) {                                       // warp-uniform
                         cf ylo, yhi;
-                        horner2<N2, ZP>(zrd + cp * 2 * N2 * ZP, rlo, rhi, ylo, yhi);
+                        horner2<N2, ZP>(zrd + cp * 2 * CS, rlo, rhi, ylo, yhi);
                         const bool cv = 2 * cp + half < ncols_w;
                         if (cv && vlo) Gc[kk_lo * GP + 2 * cp] = ylo;
                         if (cv && vhi) Gc[kk_hi * GP + 2 * cp] = yhi;
@@ -265,26 +278,21 @@ __global__ void __launch_bounds__(RQ<N>::NT, 1) k_fused_rq(FusedParams p, const 
                 }
                 if (has_x) {                                                      // k = +16: one output per column, k1 = 0
                     const int cl = lane < ncols_w ? lane : 0;
-                    const cf y = horner1<N2, ZP>(Zw + cl * N2 * ZP, rx);
-                    if (lane < ncols_w) G[(size_t)ci * KK * GP + (KK - 1) * GP + warp * CPW + lane] = y;
+                    const cf y = horner1<N2, ZP>(Zw + cl * CS, rx);
+                    if (lane < ncols_w) Gb[(size_t)ci * KK * GP + (KK - 1) * GP + warp * CPW + lane] = y;
                 }
                 __syncwarp();
             }
-            if (tid < nc) {
-                const size_t moc = ((size_t)model * p.n_orient + o) * p.n_ctf + c0 + tid;
-                sc[tid] = make_float2(p.alpha[moc] * beta, p.hterm[moc]);
-            }
+            if (tid < nc) scb[tid] = schold;
             __syncthreads();
             // ================= pass 2: (CTF, row pair) combos, CPW per warp, warp-local
             {
                 const int ncombo = nc * NP;
-                const int combo = tid / N2;                        // this thread's A2 task
-                if (combo < ncombo) {                                // whole (combo, t) groups: N2 lanes each
-                    const int cl = combo / NP, pr = combo - cl * NP;
-                    const int ra = 2 * pr, rb = 2 * pr + 1;
-                    const cf *ga = G + ((size_t)cl * KK + ra) * GP;
-                    const cf *gb = G + ((size_t)cl * KK + (rb < KK ? rb : ra)) * GP;
-                    const float bsel = rb < KK ? 1.f : 0.f;
+                if (a2combo < ncombo) {                              // whole (combo, t) groups: N2 lanes each
+                    const int a2cl = magicNP ? (int)__umulhi((unsigned)a2combo, magicNP) : a2combo, a2pr = a2combo - a2cl * NP;     // a2combo / NP
+                    const bool a2two = 2 * a2pr + 1 < KK;
+                    const cf *ga = Gb + (a2cl * KK + 2 * a2pr) * GP, *gb = ga + (a2two ? GP : 0);
+                    const float a2bsel = a2two ? 1.f : 0.f;
                     cf a[N1];
 #pragma unroll
                     for (int j = 0; j < N1; ++j) {
@@ -294,7 +302,7 @@ __global__ void __launch_bounds__(RQ<N>::NT, 1) k_fused_rq(FusedParams p, const 
                         const int ll = direct ? l : N - l;
                         cf va = ga[ll], vb = gb[ll];
                         const float sg = direct ? 1.f : -1.f;
-                        a[j] = {va.x - bsel * sg * vb.y, sg * va.y + bsel * vb.x};
+                        a[j] = {va.x - a2bsel * sg * vb.y, sg * va.y + a2bsel * vb.x};
                     }
                     fft_dif<float, N1, +1>(a);
                     spill16(zst, a);
@@ -306,35 +314,32 @@ __global__ void __launch_bounds__(RQ<N>::NT, 1) k_fused_rq(FusedParams p, const 
                 for (int cp = 0; cp < CPW / 2; ++cp) {
                     if (2 * cp < ncw) {                              // warp-uniform
                         cf ylo, yhi;
-                        horner2<N2, ZP>(zrd + cp * 2 * N2 * ZP, rlo, rhi, ylo, yhi);
-                        const int cw = 2 * cp + half;
-                        const bool cv = cw < ncw;
-                        const int combo2 = cb0 + (cv ? cw : 0);
-                        const int cl = combo2 / NP, pr = combo2 - cl * NP;
-                        const int ra = 2 * pr, rb = ra + 1;
-                        const float2 s2 = sc[cl];
+                        horner2<N2, ZP>(zrd + cp * 2 * CS, rlo, rhi, ylo, yhi);
+                        const int combo = cb0 + 2 * cp + half;
+                        const bool cv = combo < ncombo;
+                        const int cl = cv ? (magicNP ? (int)__umulhi((unsigned)combo, magicNP) : combo) : 0, pr = cv ? combo - cl * NP : 0;
+                        const float2 s2 = scb[cl];
+                        const int sha = 2 * pr * KK, shb = sha + KK;
+                        const bool rbv = 2 * pr + 1 < KK;
                         const float b[4] = {ylo.x, ylo.y, yhi.x, yhi.y};
-                        const bool v[4] = {cv && vlo, cv && vlo && rb < KK, cv && vhi, cv && vhi && rb < KK};
-                        const uint32_t sh[4] = {(uint32_t)(ra * KK + kk_lo), (uint32_t)(rb * KK + kk_lo), (uint32_t)(ra * KK + kk_hi),
-                                                (uint32_t)(rb * KK + kk_hi)};
+                        const bool v[4] = {cv && vlo, cv && vlo && rbv, cv && vhi, cv && vhi && rbv};
+                        const uint32_t sh[4] = {(uint32_t)(sha + kk_lo), (uint32_t)(shb + kk_lo), (uint32_t)(sha + kk_hi), (uint32_t)(shb + kk_hi)};
                         score4<DUMP>(p, st, mylist, b, v, sh, s2.x, s2.y, (uint32_t)(o * p.n_ctf + c0 + cl));
                     }
                 }
                 if (has_x && ncw > 0) {                              // dx = +16
                     const bool cv = lane < ncw;
-                    const int cw = cv ? lane : 0;
-                    const cf y = horner1<N2, ZP>(Zw + cw * N2 * ZP, rx);
-                    const int combo2 = cb0 + cw;
-                    const int cl = combo2 / NP, pr = combo2 - cl * NP;
-                    const int ra = 2 * pr, rb = ra + 1;
-                    const float2 s2 = sc[cl];
+                    const cf y = horner1<N2, ZP>(Zw + (cv ? lane : 0) * CS, rx);
+                    const int combo = cb0 + (cv ? lane : 0);
+                    const int cl = magicNP ? (int)__umulhi((unsigned)combo, magicNP) : combo, pr = combo - cl * NP, xsha = 2 * pr * KK;
+                    const float2 s2 = scb[cl];
                     const float b[4] = {y.x, y.y, 0.f, 0.f};
-                    const bool v[4] = {cv, cv && rb < KK, false, false};
-                    const uint32_t sh[4] = {(uint32_t)(ra * KK + KK - 1), (uint32_t)(rb * KK + KK - 1), 0u, 0u};
+                    const bool v[4] = {cv, cv && 2 * pr + 1 < KK, false, false};
+                    const uint32_t sh[4] = {(uint32_t)(xsha + KK - 1), (uint32_t)(xsha + 2 * KK - 1), 0u, 0u};
                     score4<DUMP>(p, st, mylist, b, v, sh, s2.x, s2.y, (uint32_t)(o * p.n_ctf + c0 + cl));
                 }
             }
-            __syncthreads();
+            if (NBUF == 1) __syncthreads();      // single G buffer: pass 2 must drain before the next group's pass 1 (with 2 buffers the next barrier orders the reuse)
         }
     }
     if (DUMP) return;
@@ -407,7 +412,7 @@ cudaError_t launch_relayout_K(int N, const float *K32, float *Kt, int n_ctf, cud
 }
 
 template <int N>
-static void rq_plan(int D, int n_ctf, int &CG, int &GP, size_t &bytes)
+static void rq_plan(int D, int n_ctf, int nbuf, int &CG, int &GP, size_t &bytes)
 {
     typedef RQ<N> C_;
     const int KK = 2 * D + 1, NP = (KK + 1) / 2;
@@ -415,9 +420,9 @@ static void rq_plan(int D, int n_ctf, int &CG, int &GP, size_t &bytes)
     CG = C_::NT / (NP * C_::N2);
     if (CG < 1) CG = 1;
     if (CG > n_ctf) CG = n_ctf;
-    const size_t budget = 220 * 1024;
+    const size_t budget = 226 * 1024;
     for (;;) {
-        bytes = (size_t)C_::NW * C_::ZW * 8 + (size_t)CG * KK * GP * 8 + (size_t)CG * 8 +
+        bytes = (size_t)C_::NW * C_::ZW * 8 + (size_t)nbuf * CG * KK * GP * 8 + 2 * (size_t)CG * 8 +
                 (size_t)C_::NW * BIOEM_TOPK * sizeof(TopEntry) + 2 * C_::NW * 4 + 64;
         if (bytes <= budget || CG == 1) break;
         --CG;
@@ -429,18 +434,21 @@ static cudaError_t launch_rq_t(const FusedParams &p, const float *Kt, bool dump,
 {
     int CG, GP;
     size_t bytes;
-    rq_plan<N>(p.D, p.n_ctf, CG, GP, bytes);
+    const int nbuf = 1;      // G buffers: 2 removes one CTA barrier per group but shrinks L1 to ~30 KB; measured equal on B200 (DESIGN 7)
+    rq_plan<N>(p.D, p.n_ctf, nbuf, CG, GP, bytes);
     if (bytes > 227 * 1024) return cudaErrorInvalidConfiguration;
+    const int NP = p.D + 1;                                                    // (2D+1+1)/2 row pairs
+    const unsigned magic = NP == 1 ? 0u : (unsigned)((0x100000000ull + NP - 1) / NP);   // exact x / NP for x < 2^16 (NP = 1 never divides: D = 0 has one combo per CTF)
     cudaError_t e;
     if (dump) {
         e = cudaFuncSetAttribute(k_fused_rq<N, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
         if (e != cudaSuccess) return e;
-        k_fused_rq<N, true><<<1, RQ<N>::NT, bytes, st>>>(p, reinterpret_cast<const float4 *>(Kt), CG, GP);
+        k_fused_rq<N, true><<<1, RQ<N>::NT, bytes, st>>>(p, reinterpret_cast<const float4 *>(Kt), CG, GP, magic, nbuf);
     } else {
         e = cudaFuncSetAttribute(k_fused_rq<N, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
         if (e != cudaSuccess) return e;
         const int items = p.n_img * p.n_model * p.chunks_per_model;
-        k_fused_rq<N, false><<<items, RQ<N>::NT, bytes, st>>>(p, reinterpret_cast<const float4 *>(Kt), CG, GP);
+        k_fused_rq<N, false><<<items, RQ<N>::NT, bytes, st>>>(p, reinterpret_cast<const float4 *>(Kt), CG, GP, magic, nbuf);
     }
     return cudaGetLastError();
 }

@@ -371,9 +371,9 @@ int bioem_run(bioem_ctx *ctx)
     CK(launch_ctf_tables(ctx->ctf_a.as<double>(), ctx->ctf_A.as<double>(), ctx->ctf_b.as<double>(), C, N, ctx->px, ctx->K64.as<double>(),
                          ctx->K32.as<float>(), st));
     ctx->launches += 1;
-    const bool use_rq = rq_supported(N, D);
-    if (use_rq) {
-        CK(ctx->Kt.ensure(rq_kt_bytes(N, C)));
+    const bool use_pk = pk_supported(N, D);
+    if (use_pk) {
+        CK(ctx->Kt.ensure(pk_kt_bytes(N, C)));
         CK(launch_relayout_K(N, ctx->K32.as<float>(), ctx->Kt.as<float>(), C, st));
         ctx->launches += 1;
     }
@@ -422,7 +422,7 @@ int bioem_run(bioem_ctx *ctx)
     p.part_m = ctx->part_m.as<float>(); p.part_s = ctx->part_s.as<float>(); p.part_top = ctx->part_top.as<TopEntry>();
     CK(cudaEventRecord(ctx->ev[1], st));
     int nl = 1;
-    if (use_rq) CK(launch_fused_rq(N, p, ctx->Kt.as<float>(), false, st));
+    if (use_pk) CK(launch_fused_pk(N, p, ctx->Kt.as<float>(), false, st));
     else CK(launch_fused(N, p, false, st, &nl));
     CK(cudaEventRecord(ctx->ev[2], st));
     ctx->launches += nl; ctx->fused_launches += nl;
@@ -525,7 +525,7 @@ int bioem_debug_shift_map(bioem_ctx *ctx, int img, int model, int orient, int ct
     p.chunks_per_model = 1;
     p.cA = (float)(-0.5 * ((double)n - 3.0) * 1.4426950408889634);
     p.dump = ctx->dump.as<float>(); p.dump_img = img; p.dump_model = model; p.dump_orient = orient; p.dump_ctf = ctf;
-    if (rq_supported(N, D)) CK(launch_fused_rq(N, p, ctx->Kt.as<float>(), true, ctx->stream));
+    if (pk_supported(N, D)) CK(launch_fused_pk(N, p, ctx->Kt.as<float>(), true, ctx->stream));
     else CK(launch_fused(N, p, true, ctx->stream, nullptr));
     std::vector<float> tmp((size_t)KK * KK);
     rc = fetch(ctx, tmp.data(), ctx->dump.p, tmp.size() * sizeof(float));

@@ -49,11 +49,11 @@ struct FusedParams {
 // host launchers (each enqueues on `st`); return cudaError_t
 cudaError_t launch_fused(int N, const FusedParams &p, bool dump, cudaStream_t st, int *n_launches);
 size_t fused_smem_bytes(int N, int D);
-// register-resident-Q variant (N = 64, 128)
-bool rq_supported(int N, int D);
-size_t rq_kt_bytes(int N, int n_ctf);
+// register-resident-Q, packed-f32x2 variant (N = 64, 128; D <= 16)
+bool pk_supported(int N, int D);
+size_t pk_kt_bytes(int N, int n_ctf);
 cudaError_t launch_relayout_K(int N, const float *K32, float *Kt, int n_ctf, cudaStream_t st);
-cudaError_t launch_fused_rq(int N, const FusedParams &p, const float *Kt, bool dump, cudaStream_t st);
+cudaError_t launch_fused_pk(int N, const FusedParams &p, const float *Kt, bool dump, cudaStream_t st);
 
 // precompute
 cudaError_t launch_image_stats(const float *img, int n_img, int N, double *centered, double *Dw, cudaStream_t st);

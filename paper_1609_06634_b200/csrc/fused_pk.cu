@@ -1,0 +1,523 @@
+// fused_pk.cu -- the hot loop for N = 64 and N = 128, D <= 16: register-resident Q,
+// PACKED f32x2 arithmetic (sm_100a FFMA2 / FADD2 / FMUL2) and a software-pipelined pass 1.
+//
+// Work item = (image w, model, chunk of orientations).  For one (w, o) the product Q(l,m) = conj(Ohat_w) F0_o (Eq. 12,
+// P:166) is formed ONCE and kept in registers (16 complex per thread; thread = (column l, residue t) of the two-step
+// factorisation m = N2 j + t).  The CTF loop then streams only the real radial table K_c (Eq. 5).
+//
+// Why packed: a complex number is one 64-bit register pair, and sm_100a issues one FFMA2/FADD2/FMUL2 per pair with free
+// operand swizzles (swap, per-half negate, scalar broadcast).  A complex add is 1 instruction instead of 2, a complex
+// multiply-add 2 instead of 4: the FP32 pipes see the same work, the ISSUE slots see half of it -- and this kernel is
+// issue-bound (DESIGN 7: profiles/r1_v4_*).
+//
+//   pass 1 (warp-local: a warp owns 32/N2 whole columns; only __syncwarp), one "slot" per CTF c:
+//       F(c)   a = Q*K_c, 16-point DIF FFT in registers, spill to the warp's private tile Z[c & 1]
+//       H(c-1) the 2D+1 pruned outputs per column by a Horner sum over the N2 residues, read from Z[(c-1) & 1] -> G[c-1]
+//     F(c) and H(c-1) sit in ONE basic block: H's shared-memory latency hides under F's register-only arithmetic.
+//     The k = +16 output (D = 16 only) is the DC bin of the 16-point transforms: a twiddle and a shuffle-reduction over
+//     the N2 lanes of a column, no shared-memory round.
+//   CTA barrier
+//   pass 2 (per pair of rows dy, also warp-local): Hermitian completion, two real rows packed as one complex transform,
+//       F'  16-point FFT, spill;  H' Horner -> B(dx,dy) for two dy at once
+//       a5  rho^2 = B^2 alpha_c^2 beta_w^2, g = cA log1p(-rho^2) + h_c (form C2; base-2 units inside the kernel)
+//       a6  running log-sum-exp in registers (branch-free), K best terms in per-warp sorted lists
+// No float atomics, fixed reduction orders: bit-reproducible.
+#include "common.cuh"
+#include <math_constants.h>
+
+namespace bioem {
+
+typedef float2 c2;
+static constexpr unsigned FULLP = 0xffffffffu;
+static constexpr float LSE_EMPTY = -3.0e38f;          // "no term yet": finite, so the running log-sum-exp needs no branch
+
+template <int N> struct PK {
+    static constexpr int N1 = 16, N2 = N / 16, NC = N / 2 + 1, NTASK = NC * N2, NW = (NTASK + 31) / 32, NT = NW * 32;
+    static constexpr int ZP = 18, CPW = 32 / N2, NR = CPW / 2;   // Z pitch (even: 16-byte aligned pairs), columns per warp, B-phase rounds
+    static constexpr int CS = N2 * ZP + 2;                        // column-tile pitch
+    static constexpr int MAXREG = (65536 / NT) / 8 * 8 > 255 ? 255 : (65536 / NT) / 8 * 8;
+    static constexpr int ZW = CPW * CS;                           // Z words (complex) per warp and buffer
+};
+
+// ---- packed complex helpers (each maps to ONE sm_100a instruction; swizzles / negations fold into the operands)
+__device__ __forceinline__ c2 pk_add(c2 a, c2 b) { return __fadd2_rn(a, b); }
+__device__ __forceinline__ c2 pk_sub(c2 a, c2 b) { return __fadd2_rn(a, make_float2(-b.x, -b.y)); }
+__device__ __forceinline__ c2 pk_bc(float s) { return make_float2(s, s); }
+__device__ __forceinline__ c2 pk_rot90(c2 a) { return make_float2(-a.y, a.x); }                                   // i a
+__device__ __forceinline__ c2 pk_cmul(c2 a, c2 w) { return __ffma2_rn(pk_rot90(a), pk_bc(w.y), __fmul2_rn(a, pk_bc(w.x))); }       // a w
+__device__ __forceinline__ c2 pk_cmadd(c2 a, c2 w, c2 z) { return __ffma2_rn(pk_rot90(a), pk_bc(w.y), __ffma2_rn(a, pk_bc(w.x), z)); }   // a w + z
+
+// a * exp(+2 pi i K32 / 32), K32 a compile-time constant after unrolling
+__device__ __forceinline__ c2 pk_twid(c2 a, int K32)
+{
+    if (K32 == 0) return a;
+    if (K32 == 8) return pk_rot90(a);
+    float c, s;
+    if (K32 < 8) { c = (float)cos32(K32); s = (float)cos32(8 - K32); }
+    else         { c = -(float)cos32(16 - K32); s = (float)cos32(K32 - 8); }
+    return __ffma2_rn(pk_rot90(a), pk_bc(s), __fmul2_rn(a, pk_bc(c)));
+}
+
+// in-place 16-point DIF, y[k] = sum_j a[j] exp(+2 pi i j k / 16); on return a[r] = y[bitrev4(r)]
+__device__ __forceinline__ void pk_fft16(c2 (&a)[16])
+{
+#pragma unroll
+    for (int half = 8; half >= 1; half /= 2)
+#pragma unroll
+        for (int base = 0; base < 16; base += 2 * half)
+#pragma unroll
+            for (int j = 0; j < half; ++j) {
+                const c2 u = a[base + j], v = a[base + j + half];
+                a[base + j] = pk_add(u, v);
+                a[base + j + half] = pk_twid(pk_sub(u, v), j * (16 / half));
+            }
+}
+
+// spill the bit-reversed FFT output as 8 16-byte stores: (a[r], a[r+8]) = (y[2b], y[2b+1]), b = bitrev3(r)
+__device__ __forceinline__ void pk_spill16(c2 *zst, const c2 (&a)[16])
+{
+#pragma unroll
+    for (int r = 0; r < 8; ++r) {
+        const int b = bitrev(r, 3);
+        *reinterpret_cast<float4 *>(zst + 2 * b) = make_float4(a[r].x, a[r].y, a[r + 8].x, a[r + 8].y);
+    }
+}
+
+// Two Horner sums over the N2 residues sharing their loads: ylo = sum_t rlo^t z[t], yhi = sum_t rhi^t z[t]
+template <int N2, int ZP>
+__device__ __forceinline__ void pk_horner2(const c2 *zc, c2 rlo, c2 rhi, c2 &ylo, c2 &yhi)
+{
+    c2 z = zc[(N2 - 1) * ZP];
+    ylo = z; yhi = z;
+#pragma unroll
+    for (int t = N2 - 2; t >= 0; --t) {
+        z = zc[t * ZP];
+        ylo = pk_cmadd(ylo, rlo, z);
+        yhi = pk_cmadd(yhi, rhi, z);
+    }
+}
+
+// sum over the N2 lanes of a column (lanes are contiguous and N2-aligned): fixed xor tree, every lane gets the sum
+template <int N2>
+__device__ __forceinline__ c2 pk_colsum(c2 v)
+{
+#pragma unroll
+    for (int off = 1; off < N2; off <<= 1) {
+        c2 w;
+        w.x = __shfl_xor_sync(FULLP, v.x, off);
+        w.y = __shfl_xor_sync(FULLP, v.y, off);
+        v = pk_add(v, w);
+    }
+    return v;
+}
+
+__device__ __forceinline__ float pk_ex2(float x)
+{
+    float y;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
+__device__ __forceinline__ bool pk_entry_before(float ga, uint32_t pa, uint32_t sa, float gb, uint32_t pb, uint32_t sb)
+{   // ranking: larger g first; ties -> lower flat index (pair, shift) first (R15)
+    return ga > gb || (ga == gb && (pa < pb || (pa == pb && sa < sb)));
+}
+
+// Insert the candidates of the lanes with `valid && g >= thr` into this warp's sorted K-list (shared memory).
+__device__ __forceinline__ void pk_topk_insert(float g, uint32_t pair, uint32_t sh, bool valid, float &thr, TopEntry *list)
+{
+    unsigned m = __ballot_sync(FULLP, valid && g >= thr);
+    const int lane = threadIdx.x & 31;
+    while (m) {
+        const int src = __ffs(m) - 1;
+        m &= m - 1;
+        const float gv = __shfl_sync(FULLP, g, src);
+        const uint32_t pv = __shfl_sync(FULLP, pair, src), sv = __shfl_sync(FULLP, sh, src);
+        TopEntry e = {0.f, 0u, 0u};
+        if (lane < BIOEM_TOPK) e = list[lane];
+        const bool before = lane < BIOEM_TOPK && pk_entry_before(e.g, e.pair, e.shift, gv, pv, sv);
+        const int pos = __popc(__ballot_sync(FULLP, before));          // sorted list: the entries ranked before form a prefix
+        if (pos < BIOEM_TOPK) {
+            __syncwarp();
+            if (lane >= pos && lane < BIOEM_TOPK - 1) list[lane + 1] = e;
+            if (lane == pos) { TopEntry n = {gv, pv, sv}; list[pos] = n; }
+            __syncwarp();
+            thr = list[BIOEM_TOPK - 1].g;
+        }
+    }
+}
+
+struct PkLse { float m, s, thr; };
+
+// a5 + a6 for the NV (2 or 4) correlations a lane holds: b[i] = (B(dx_i, dy_A), B(dx_i, dy_B)).
+// log1p(-x) = -x (1 + x/2 + x^2/3 + x^3/4 + x^4/5) for x < 2^-6 (truncation < 2e-10 relative); the accurate routine runs
+// only when some lane of the warp is near the posterior peak.
+template <bool DUMP, int NV>
+__device__ __forceinline__ void pk_score(const FusedParams &p, PkLse &st, TopEntry *mylist, const c2 (&b)[NV / 2], const bool (&v)[NV],
+                                         const uint32_t (&sh)[NV], float ab, float hterm, uint32_t pair)
+{
+    c2 x2[NV / 2], g2[NV / 2];
+    float xmax = 0.f;
+#pragma unroll
+    for (int i = 0; i < NV / 2; ++i) {
+        const c2 r = __fmul2_rn(b[i], pk_bc(ab));
+        x2[i] = __fmul2_rn(r, r);                                               // rho^2
+        xmax = fmaxf(xmax, fmaxf(x2[i].x, x2[i].y));
+        c2 q = __ffma2_rn(x2[i], pk_bc(0.2f), pk_bc(0.25f));
+        q = __ffma2_rn(x2[i], q, pk_bc(0.33333334f));
+        q = __ffma2_rn(x2[i], q, pk_bc(0.5f));
+        q = __ffma2_rn(x2[i], q, pk_bc(1.0f));
+        g2[i] = __ffma2_rn(__fmul2_rn(x2[i], q), pk_bc(-p.cA), pk_bc(hterm));   // form C2, base-2 units
+    }
+    float g[NV];
+#pragma unroll
+    for (int i = 0; i < NV / 2; ++i) { g[2 * i] = g2[i].x; g[2 * i + 1] = g2[i].y; }
+    if (__any_sync(FULLP, xmax >= 0.015625f)) {
+#pragma unroll
+        for (int i = 0; i < NV; ++i) {
+            const float x = fminf((i & 1) ? x2[i / 2].y : x2[i / 2].x, 0.99999994f);      // R14 clamp
+            if (x >= 0.015625f) g[i] = fmaf(p.cA, log1pf(-x), hterm);
+        }
+    }
+    float gmax = -CUDART_INF_F;
+#pragma unroll
+    for (int i = 0; i < NV; ++i) {
+        if (DUMP && v[i]) p.dump[sh[i]] = g[i];
+        g[i] = v[i] ? g[i] : -CUDART_INF_F;
+        gmax = fmaxf(gmax, g[i]);
+    }
+    const float mn = fmaxf(st.m, gmax);                                         // finite: st.m starts at LSE_EMPTY
+    float acc = pk_ex2(g[0] - mn) + pk_ex2(g[1] - mn);
+    if (NV == 4) acc += pk_ex2(g[2] - mn) + pk_ex2(g[3] - mn);
+    st.s = fmaf(st.s, pk_ex2(st.m - mn), acc);
+    st.m = mn;
+    if (__any_sync(FULLP, gmax >= st.thr)) {
+#pragma unroll
+        for (int i = 0; i < NV; ++i) pk_topk_insert(g[i], pair, sh[i], v[i], st.thr, mylist);
+    }
+}
+
+template <int N, bool DUMP>
+__global__ void __launch_bounds__(PK<N>::NT, 1) k_fused_pk(FusedParams p, const float4 *__restrict__ Kt, int CG, int GP)
+{
+    typedef PK<N> C_;
+    constexpr int N1 = C_::N1, N2 = C_::N2, NC = C_::NC, NTASK = C_::NTASK, NW = C_::NW, NT = C_::NT, ZP = C_::ZP, ZW = C_::ZW, CPW = C_::CPW,
+                  CS = C_::CS, NR = C_::NR;
+    constexpr size_t H = (size_t)NC * N;
+    const int D = p.D, KK = 2 * D + 1, NP = D + 1;                        // host guarantees D <= 16; NP row pairs (the last one is a single row)
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    c2 *Z = reinterpret_cast<c2 *>(smem_raw);                         // [2][NW][ZW]   warp-private tiles, double-buffered
+    c2 *G = Z + (size_t)2 * NW * ZW;                                  // [CG][KK][GP]  pass-1 output rows of a CTF group
+    float2 *sc = reinterpret_cast<float2 *>(G + (size_t)CG * KK * GP); // [2][CG]      (alpha*beta, h) of the group's CTFs
+    TopEntry *tops = reinterpret_cast<TopEntry *>(sc + 2 * CG);       // [NW][TOPK]
+    float *red = reinterpret_cast<float *>(tops + NW * BIOEM_TOPK);   // [2 NW]
+
+    int img, model, o_begin, o_end, item;
+    if (DUMP) { img = p.dump_img; model = p.dump_model; o_begin = p.dump_orient; o_end = o_begin + 1; item = 0; }
+    else {
+        item = blockIdx.x;
+        img = item % p.n_img;
+        const int chunk = item / p.n_img;
+        model = chunk / p.chunks_per_model;
+        o_begin = (chunk % p.chunks_per_model) * p.oc;
+        o_end = min(o_begin + p.oc, p.n_orient);
+    }
+    const float beta = p.beta[img];
+    if (tid < NW * BIOEM_TOPK) { TopEntry e0 = {-CUDART_INF_F, 0xffffffffu, 0xffffffffu}; tops[tid] = e0; }
+    __syncthreads();
+
+    // ---- F-phase constants: thread = (column, residue t)
+    const bool act1 = tid < NTASK;
+    const int col = act1 ? tid / N2 : 0, t = tid % N2;
+    const size_t qbase = (size_t)col * N + t;
+    c2 *const Zw = Z + (size_t)warp * ZW;                             // buffer b at Zw + b * NW * ZW
+    constexpr int ZBUF = NW * ZW;
+    const int zst_off = (lane / N2) * CS + (lane % N2) * ZP;
+    const int ncols_w = max(0, min(CPW, NC - warp * CPW));            // whole columns owned by this warp
+    const bool has_x = D == 16;
+    c2 wx;                                                            // exp(2 pi i t / N2) = w_N^{16 t}: the k = +16 output
+    sincospif(2.0f * (float)t / (float)N2, &wx.y, &wx.x);
+    const bool xlane = has_x && t == 0;
+    // ---- H-phase constants: lane = (half, k1); outputs k = k1 - 16 ("lo") and k = k1 ("hi")
+    const int half = lane >> 4, k1 = lane & 15;
+    const bool vlo = k1 >= 16 - D, vhi = k1 <= D;
+    const int kk_lo = k1 - 16 + D, kk_hi = k1 + D;                    // row / dx index of the two outputs
+    c2 rlo, rhi;
+    sincospif(2.0f * (float)(k1 - 16 + N) / (float)N, &rlo.y, &rlo.x);
+    sincospif(2.0f * (float)k1 / (float)N, &rhi.y, &rhi.x);
+    const int zrd_off = half * CS + k1;                               // + cp * 2 * CS per round
+    // ---- pass-2 task of this thread in F': (CTF in group, row pair) = a2combo, residue t
+    const int a2combo = tid / N2, a2cl = a2combo / NP, a2pr = a2combo - a2cl * NP;
+    const bool a2two = 2 * a2pr + 1 < KK;
+    const float a2bsel = a2two ? 1.f : 0.f;
+    const int a2row = 2 * a2pr * GP, a2rowb = a2two ? GP : 0;
+    const int l8 = (t == 0) ? N / 2 : N / 2 - t;                      // j = 8: l = N/2 + t, direct only for t = 0, else mirrored to N/2 - t
+    const float sg8 = (t == 0) ? 1.f : -1.f;
+    // ---- pass-2 rounds of this lane in H': combo = warp*CPW + 2 cp + half  ->  (cl, first flat shift index of row A)
+    int h2cl[NR], h2sha[NR];
+    bool h2two[NR];
+#pragma unroll
+    for (int cp = 0; cp < NR; ++cp) {
+        const int combo = warp * CPW + 2 * cp + half;
+        h2cl[cp] = combo / NP;
+        const int pr = combo - h2cl[cp] * NP;
+        h2sha[cp] = 2 * pr * KK;
+        h2two[cp] = 2 * pr + 1 < KK;
+    }
+
+    const cf *Oimg = p.Ohat + (size_t)img * H;
+    PkLse st = {LSE_EMPTY, 0.f, -CUDART_INF_F};
+    TopEntry *mylist = tops + warp * BIOEM_TOPK;
+    const int c_lo = DUMP ? p.dump_ctf : 0, c_hi = DUMP ? p.dump_ctf + 1 : p.n_ctf;
+    const float4 *Kt_t = Kt + tid;
+    constexpr size_t KSTR = (size_t)(N1 / 4) * NT;                    // float4 per CTF
+
+    float4 kq[N1 / 4];
+#pragma unroll
+    for (int g4 = 0; g4 < N1 / 4; ++g4) kq[g4] = Kt_t[(size_t)c_lo * KSTR + (size_t)g4 * NT];
+    int zb = 0, scbuf = 0;
+
+    // a = Q K_c (consumes kq), then prefetch K of CTF `cn`
+#define PK_LOAD_A(cn)                                                                                         \
+    c2 a[N1];                                                                                                 \
+    _Pragma("unroll") for (int g4 = 0; g4 < N1 / 4; ++g4) {                                                   \
+        a[4 * g4 + 0] = __fmul2_rn(q[4 * g4 + 0], pk_bc(kq[g4].x));                                           \
+        a[4 * g4 + 1] = __fmul2_rn(q[4 * g4 + 1], pk_bc(kq[g4].y));                                           \
+        a[4 * g4 + 2] = __fmul2_rn(q[4 * g4 + 2], pk_bc(kq[g4].z));                                           \
+        a[4 * g4 + 3] = __fmul2_rn(q[4 * g4 + 3], pk_bc(kq[g4].w));                                           \
+    }                                                                                                         \
+    {                                                                                                         \
+        const float4 *kp = Kt_t + (size_t)(cn) * KSTR;                                                        \
+        _Pragma("unroll") for (int g4 = 0; g4 < N1 / 4; ++g4) kq[g4] = kp[(size_t)g4 * NT];                   \
+    }
+    // H(ci): pruned outputs of the columns in tile Zr -> rows of G
+#define PK_HORNER_G(Zr, ci)                                                                                   \
+    {                                                                                                         \
+        c2 *Gc = G + (size_t)(ci) * KK * GP + warp * CPW + half;                                              \
+        _Pragma("unroll") for (int cp = 0; cp < NR; ++cp) {                                                   \
+            c2 ylo, yhi;                                                                                      \
+            pk_horner2<N2, ZP>((Zr) + zrd_off + cp * 2 * CS, rlo, rhi, ylo, yhi);                             \
+            const bool cv = 2 * cp + half < ncols_w;                                                          \
+            if (cv && vlo) Gc[kk_lo * GP + 2 * cp] = ylo;                                                     \
+            if (cv && vhi) Gc[kk_hi * GP + 2 * cp] = yhi;                                                     \
+        }                                                                                                     \
+    }
+    // F(ci) tail: FFT, the k = +16 output from the DC bins, spill to tile Zwr
+#define PK_FFT_SPILL_G(Zwr, ci)                                                                               \
+    {                                                                                                         \
+        pk_fft16(a);                                                                                          \
+        const c2 xs = pk_colsum<N2>(pk_cmul(a[0], wx));                                                       \
+        if (xlane && act1) G[(size_t)(ci) * KK * GP + (size_t)(KK - 1) * GP + col] = xs;                      \
+        pk_spill16((Zwr) + zst_off, a);                                                                       \
+    }
+
+    for (int o = o_begin; o < o_end; ++o) {
+        // ---- Q = conj(Ohat) F0 for this thread's 16 bins (Eq. 12)
+        c2 q[N1];
+        {
+            const cf *F0 = p.F0 + ((size_t)model * p.n_orient + o) * H;
+#pragma unroll
+            for (int j = 0; j < N1; ++j) {
+                const cf ov = Oimg[qbase + (size_t)N2 * j], fv = F0[qbase + (size_t)N2 * j];
+                const cf pr = cmulc(ov, fv);
+                q[j] = act1 ? make_float2(pr.x, pr.y) : make_float2(0.f, 0.f);
+            }
+        }
+        for (int c0 = c_lo; c0 < c_hi; c0 += CG) {
+            const int nc = min(CG, c_hi - c0);
+            float2 *scb = sc + scbuf * CG;
+            scbuf ^= 1;
+            if (tid < nc) {                                           // (alpha*beta, h) of CTF c0 + tid
+                const size_t moc = ((size_t)model * p.n_orient + o) * p.n_ctf + c0 + tid;
+                scb[tid] = make_float2(p.alpha[moc] * beta, p.hterm[moc]);
+            }
+            // ================= pass 1, software-pipelined over the CTFs of the group, warp-local
+            {
+                int cn = c0 + 1;
+                if (cn >= c_hi) cn = c_lo;
+                PK_LOAD_A(cn)
+                PK_FFT_SPILL_G(Zw + zb * ZBUF, 0)
+                __syncwarp();
+            }
+            for (int ci = 1; ci < nc; ++ci) {
+                int cn = c0 + ci + 1;
+                if (cn >= c_hi) cn = c_lo;
+                PK_LOAD_A(cn)
+                PK_HORNER_G(Zw + zb * ZBUF, ci - 1)
+                zb ^= 1;
+                PK_FFT_SPILL_G(Zw + zb * ZBUF, ci)
+                __syncwarp();
+            }
+            PK_HORNER_G(Zw + zb * ZBUF, nc - 1)
+            zb ^= 1;
+            __syncthreads();
+            // ================= pass 2: (CTF, row pair) combos, CPW per warp
+            c2 xs2;
+            {
+                const c2 *ga = G + (size_t)(a2cl < nc ? a2cl : 0) * KK * GP + a2row, *gb = ga + a2rowb;
+                c2 a[N1];
+#pragma unroll
+                for (int j = 0; j < N1; ++j) {
+                    // l = N2 j + t; direct for l <= N/2, mirrored (conjugate) above: a = A + i B of the two real rows
+                    if (j < 8) {
+                        const c2 va = ga[N2 * j + t], vb = gb[N2 * j + t];
+                        a[j] = __ffma2_rn(pk_rot90(vb), pk_bc(a2bsel), va);
+                    } else if (j > 8) {
+                        const c2 va = ga[N - N2 * j - t], vb = gb[N - N2 * j - t];
+                        a[j] = __ffma2_rn(make_float2(vb.y, vb.x), pk_bc(a2bsel), make_float2(va.x, -va.y));
+                    } else {
+                        const c2 va = ga[l8], vb = gb[l8];
+                        a[j] = __ffma2_rn(make_float2(-sg8 * vb.y, vb.x), pk_bc(a2bsel), make_float2(va.x, sg8 * va.y));
+                    }
+                }
+                pk_fft16(a);
+                xs2 = pk_colsum<N2>(pk_cmul(a[0], wx));               // B(dx = +16) of the two rows
+                pk_spill16(Zw + zb * ZBUF + zst_off, a);
+            }
+            __syncthreads();                                          // G consumed (next group may overwrite it), Z tile visible
+            {
+                const c2 *Zr = Zw + zb * ZBUF;
+                const uint32_t pair0 = (uint32_t)(o * p.n_ctf + c0);
+#pragma unroll
+                for (int cp = 0; cp < NR; ++cp) {
+                    c2 y[2];
+                    pk_horner2<N2, ZP>(Zr + zrd_off + cp * 2 * CS, rlo, rhi, y[0], y[1]);
+                    const int cl = h2cl[cp];
+                    const bool cv = cl < nc;
+                    const float2 s2 = scb[cv ? cl : 0];
+                    const int sha = h2sha[cp], shb = sha + KK;
+                    const bool v[4] = {cv && vlo, cv && vlo && h2two[cp], cv && vhi, cv && vhi && h2two[cp]};
+                    const uint32_t sh[4] = {(uint32_t)(sha + kk_lo), (uint32_t)(shb + kk_lo), (uint32_t)(sha + kk_hi), (uint32_t)(shb + kk_hi)};
+                    pk_score<DUMP, 4>(p, st, mylist, y, v, sh, s2.x, s2.y, pair0 + (uint32_t)cl);
+                }
+                if (has_x) {                                          // dx = +16: one lane per combo holds the two rows' values
+                    const bool cv = t == 0 && a2cl < nc;
+                    const float2 s2 = scb[a2cl < nc ? a2cl : 0];
+                    const c2 y[1] = {xs2};
+                    const int xsha = 2 * a2pr * KK + KK - 1;
+                    const bool v[2] = {cv, cv && a2two};
+                    const uint32_t sh[2] = {(uint32_t)xsha, (uint32_t)(xsha + KK)};
+                    pk_score<DUMP, 2>(p, st, mylist, y, v, sh, s2.x, s2.y, pair0 + (uint32_t)a2cl);
+                }
+            }
+            zb ^= 1;                                                  // the next F(0) must not overwrite the tile H' is still reading
+        }
+    }
+#undef PK_LOAD_A
+#undef PK_HORNER_G
+#undef PK_FFT_SPILL_G
+    if (DUMP) return;
+
+    // ---- block reduction, fixed order
+    float lse_m = st.m, lse_s = st.s;
+#pragma unroll
+    for (int off = 16; off >= 1; off >>= 1) {
+        const float m2 = __shfl_xor_sync(FULLP, lse_m, off), s2 = __shfl_xor_sync(FULLP, lse_s, off);
+        const float M = fmaxf(lse_m, m2);
+        lse_s = lse_s * pk_ex2(lse_m - M) + s2 * pk_ex2(m2 - M);
+        lse_m = M;
+    }
+    if (lane == 0) { red[2 * warp] = lse_m; red[2 * warp + 1] = lse_s; }
+    __syncthreads();
+    if (warp == 0) {
+        float m = LSE_EMPTY, s = 0.f;
+        for (int w = 0; w < NW; ++w) {
+            const float m2 = red[2 * w], s2 = red[2 * w + 1];
+            const float M = fmaxf(m, m2);
+            s = s * pk_ex2(m - M) + s2 * pk_ex2(m2 - M);
+            m = M;
+        }
+        if (!(s > 0.f)) m = -CUDART_INF_F;                            // the merge kernel's "empty partial"
+        float th0 = tops[BIOEM_TOPK - 1].g;
+        for (int w = 1; w < NW; ++w)
+            for (int k = 0; k < BIOEM_TOPK; ++k) {
+                TopEntry e = tops[w * BIOEM_TOPK + k];
+                pk_topk_insert(e.g, e.pair, e.shift, lane == 0 && e.pair != 0xffffffffu, th0, tops);
+            }
+        __syncwarp();
+        if (lane == 0) { p.part_m[item] = m; p.part_s[item] = s; }
+        if (lane < BIOEM_TOPK) p.part_top[(size_t)item * BIOEM_TOPK + lane] = tops[lane];
+    }
+}
+
+// ------------------------------------------------------------------------------------------------ K in task order
+// Kt[c][g4][tid][e] = K_c(l = tid / N2, m = N2 (4 g4 + e) + tid % N2): the 16 values a thread needs are 4 coalesced float4.
+template <int N>
+__global__ void k_relayout_K(const float *K32, float4 *Kt, int n_ctf)
+{
+    typedef PK<N> C_;
+    const int c = blockIdx.y, i = blockIdx.x * blockDim.x + threadIdx.x;       // i = g4 * NT + tid
+    if (i >= (C_::N1 / 4) * C_::NT) return;
+    const int g4 = i / C_::NT, tid = i % C_::NT;
+    float v[4] = {0.f, 0.f, 0.f, 0.f};
+    if (tid < C_::NTASK) {
+        const int col = tid / C_::N2, t = tid % C_::N2;
+        for (int e = 0; e < 4; ++e) v[e] = K32[(size_t)c * C_::NC * N + (size_t)col * N + C_::N2 * (4 * g4 + e) + t];
+    }
+    Kt[(size_t)c * (C_::N1 / 4) * C_::NT + i] = make_float4(v[0], v[1], v[2], v[3]);
+}
+
+bool pk_supported(int N, int D) { return (N == 64 || N == 128) && D <= 16; }
+size_t pk_kt_bytes(int N, int n_ctf) { return N == 64 ? (size_t)n_ctf * 4 * PK<64>::NT * 16 : (size_t)n_ctf * 4 * PK<128>::NT * 16; }
+
+cudaError_t launch_relayout_K(int N, const float *K32, float *Kt, int n_ctf, cudaStream_t st)
+{
+    if (N == 64) {
+        dim3 g((4 * PK<64>::NT + 255) / 256, n_ctf);
+        k_relayout_K<64><<<g, 256, 0, st>>>(K32, reinterpret_cast<float4 *>(Kt), n_ctf);
+    } else {
+        dim3 g((4 * PK<128>::NT + 255) / 256, n_ctf);
+        k_relayout_K<128><<<g, 256, 0, st>>>(K32, reinterpret_cast<float4 *>(Kt), n_ctf);
+    }
+    return cudaGetLastError();
+}
+
+template <int N>
+static void pk_plan(int D, int n_ctf, int &CG, int &GP, size_t &bytes)
+{
+    typedef PK<N> C_;
+    const int KK = 2 * D + 1, NP = D + 1;
+    GP = C_::NC | 1;
+    CG = C_::NT / (NP * C_::N2);                        // CTFs per group: every (CTF, row pair, residue) task of pass 2 has a thread
+    if (CG < 1) CG = 1;
+    if (CG > n_ctf) CG = n_ctf;
+    const size_t budget = 227 * 1024;
+    for (;;) {
+        bytes = (size_t)2 * C_::NW * C_::ZW * 8 + (size_t)CG * KK * GP * 8 + 2 * (size_t)CG * 8 +
+                (size_t)C_::NW * BIOEM_TOPK * sizeof(TopEntry) + 2 * C_::NW * 4 + 64;
+        if (bytes <= budget || CG == 1) break;
+        --CG;
+    }
+}
+
+template <int N>
+static cudaError_t launch_pk_t(const FusedParams &p, const float *Kt, bool dump, cudaStream_t st)
+{
+    int CG, GP;
+    size_t bytes;
+    pk_plan<N>(p.D, p.n_ctf, CG, GP, bytes);
+    if (bytes > 227 * 1024) return cudaErrorInvalidConfiguration;
+    cudaError_t e;
+    if (dump) {
+        e = cudaFuncSetAttribute(k_fused_pk<N, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+        if (e != cudaSuccess) return e;
+        k_fused_pk<N, true><<<1, PK<N>::NT, bytes, st>>>(p, reinterpret_cast<const float4 *>(Kt), CG, GP);
+    } else {
+        e = cudaFuncSetAttribute(k_fused_pk<N, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+        if (e != cudaSuccess) return e;
+        const int items = p.n_img * p.n_model * p.chunks_per_model;
+        k_fused_pk<N, false><<<items, PK<N>::NT, bytes, st>>>(p, reinterpret_cast<const float4 *>(Kt), CG, GP);
+    }
+    return cudaGetLastError();
+}
+
+cudaError_t launch_fused_pk(int N, const FusedParams &p, const float *Kt, bool dump, cudaStream_t st)
+{
+    if (N == 64) return launch_pk_t<64>(p, Kt, dump, st);
+    if (N == 128) return launch_pk_t<128>(p, Kt, dump, st);
+    return cudaErrorInvalidValue;
+}
+
+}  // namespace bioem

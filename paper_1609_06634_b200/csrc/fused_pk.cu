@@ -1,5 +1,5 @@
 // fused_pk.cu -- the hot loop for N = 64 and N = 128, D <= 16: register-resident Q,
-// PACKED f32x2 arithmetic (sm_100a FFMA2 / FADD2 / FMUL2) and a software-pipelined pass 1.
+// PACKED f32x2 arithmetic (sm_100a FFMA2 / FADD2 / FMUL2) and ONE software pipeline over CTF groups.
 //
 // Work item = (image w, model, chunk of orientations).  For one (w, o) the product Q(l,m) = conj(Ohat_w) F0_o (Eq. 12,
 // P:166) is formed ONCE and kept in registers (16 complex per thread; thread = (column l, residue t) of the two-step
@@ -7,20 +7,24 @@
 //
 // Why packed: a complex number is one 64-bit register pair, and sm_100a issues one FFMA2/FADD2/FMUL2 per pair with free
 // operand swizzles (swap, per-half negate, scalar broadcast).  A complex add is 1 instruction instead of 2, a complex
-// multiply-add 2 instead of 4: the FP32 pipes see the same work, the ISSUE slots see half of it -- and this kernel is
-// issue-bound (DESIGN 7: profiles/r1_v4_*).
+// multiply-add 2 instead of 4: the FP32 pipes see the same work, the ISSUE slots see half of it (DESIGN 7).
 //
-//   pass 1 (warp-local: a warp owns 32/N2 whole columns; only __syncwarp), one "slot" per CTF c:
-//       F(c)   a = Q*K_c, 16-point DIF FFT in registers, spill to the warp's private tile Z[c & 1]
-//       H(c-1) the 2D+1 pruned outputs per column by a Horner sum over the N2 residues, read from Z[(c-1) & 1] -> G[c-1]
-//     F(c) and H(c-1) sit in ONE basic block: H's shared-memory latency hides under F's register-only arithmetic.
-//     The k = +16 output (D = 16 only) is the DC bin of the 16-point transforms: a twiddle and a shuffle-reduction over
-//     the N2 lanes of a column, no shared-memory round.
-//   CTA barrier
-//   pass 2 (per pair of rows dy, also warp-local): Hermitian completion, two real rows packed as one complex transform,
-//       F'  16-point FFT, spill;  H' Horner -> B(dx,dy) for two dy at once
-//       a5  rho^2 = B^2 alpha_c^2 beta_w^2, g = cA log1p(-rho^2) + h_c (form C2; base-2 units inside the kernel)
-//       a6  running log-sum-exp in registers (branch-free), K best terms in per-warp sorted lists
+// Why N/2 columns: the CTA is N/2 * N2 threads = 16 warps at N = 128, i.e. exactly 4 warps on each of the SM's 4
+// schedulers with 128 registers each (17 warps put 5 on one scheduler: 96 registers, spills, and 3 schedulers waiting
+// for the 4th at every barrier -- profiles/r1_v5_*).  The Nyquist column l = N/2 rides on column 0: both are Hermitian
+// in m, so the transform of Q(0,.)K(0,.) + i Q(N/2,.)K(N/2,.) is G(.,0) + i G(.,N/2) with both parts real.
+//
+// Every "slot" is [A-op: 16 complex into registers, 16-point DIF FFT] || [H-op: Horner sums over the Z tile the previous
+// slot spilled], then __syncwarp, spill, __syncwarp.  The two halves of a slot share no data, sit in one basic block, and
+// the H-op's shared-memory latency hides under the A-op's register-only arithmetic:
+//   slot A   F(0)   a = Q K_c0                 ||  H'(group gi-2): B(dx,dy) -> a5 likelihood -> a6 log-sum-exp, candidates
+//   slot B   F(ci)  a = Q K_ci                 ||  H(ci-1): the 2D+1 pruned outputs per column -> rows of G[gi & 1]
+//   slot C   F'(group gi-1): rows of G[gi-1 & 1], Hermitian completion, two real rows per transform  ||  H(nc-1)
+//   one CTA barrier per group (G is double-buffered over groups; the Z tiles are warp-private).
+// The k = +16 output (D = 16 only) is the DC bin of the 16-point transforms: a twiddle and a shuffle-reduction over the
+// N2 lanes of a column.  The pipeline is primed and drained with masked groups (2 per work item, < 1 % of the work).
+//   a5  rho^2 = B^2 alpha_c^2 beta_w^2, g = cA log1p(-rho^2) + h_c (form C2; base-2 units inside the kernel)
+//   a6  running log-sum-exp in registers (branch-free), K best terms in per-warp sorted lists
 // No float atomics, fixed reduction orders: bit-reproducible.
 #include "common.cuh"
 #include <math_constants.h>
@@ -32,11 +36,11 @@ static constexpr unsigned FULLP = 0xffffffffu;
 static constexpr float LSE_EMPTY = -3.0e38f;          // "no term yet": finite, so the running log-sum-exp needs no branch
 
 template <int N> struct PK {
-    static constexpr int N1 = 16, N2 = N / 16, NC = N / 2 + 1, NTASK = NC * N2, NW = (NTASK + 31) / 32, NT = NW * 32;
-    static constexpr int ZP = 18, CPW = 32 / N2, NR = CPW / 2;   // Z pitch (even: 16-byte aligned pairs), columns per warp, B-phase rounds
+    static constexpr int N1 = 16, N2 = N / 16, NCH = N / 2, NT = NCH * N2, NW = NT / 32;   // NCH columns: l = 0 carries l = N/2 packed with it
+    static constexpr int ZP = 18, CPW = 32 / N2, NR = CPW / 2;   // Z pitch (even: 16-byte aligned pairs), columns per warp, H-phase rounds
     static constexpr int CS = N2 * ZP + 2;                        // column-tile pitch
-    static constexpr int MAXREG = (65536 / NT) / 8 * 8 > 255 ? 255 : (65536 / NT) / 8 * 8;
-    static constexpr int ZW = CPW * CS;                           // Z words (complex) per warp and buffer
+    static constexpr int ZW = CPW * CS;                           // Z words (complex) per warp
+    static constexpr int NCOMBO = NT / N2;                        // (CTF, row pair) tasks of pass 2 per sweep
 };
 
 // ---- packed complex helpers (each maps to ONE sm_100a instruction; swizzles / negations fold into the operands)
@@ -197,21 +201,33 @@ __device__ __forceinline__ void pk_score(const FusedParams &p, PkLse &st, TopEnt
     }
 }
 
+// 16-byte asynchronous global -> shared copy (LDGSTS); completion is awaited by the issuing thread itself
+__device__ __forceinline__ void pk_cp_async16(void *smem_dst, const void *gsrc)
+{
+    const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(gsrc) : "memory");
+}
+__device__ __forceinline__ void pk_cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void pk_cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
+
 template <int N, bool DUMP>
-__global__ void __launch_bounds__(PK<N>::NT, 1) k_fused_pk(FusedParams p, const float4 *__restrict__ Kt, int CG, int GP)
+__global__ void __launch_bounds__(PK<N>::NT, 1) k_fused_pk(FusedParams p, const float4 *__restrict__ Kt, const float4 *__restrict__ KtN, int CG, int GP)
 {
     typedef PK<N> C_;
-    constexpr int N1 = C_::N1, N2 = C_::N2, NC = C_::NC, NTASK = C_::NTASK, NW = C_::NW, NT = C_::NT, ZP = C_::ZP, ZW = C_::ZW, CPW = C_::CPW,
-                  CS = C_::CS, NR = C_::NR;
-    constexpr size_t H = (size_t)NC * N;
-    const int D = p.D, KK = 2 * D + 1, NP = D + 1;                        // host guarantees D <= 16; NP row pairs (the last one is a single row)
+    constexpr int N1 = C_::N1, N2 = C_::N2, NW = C_::NW, NT = C_::NT, ZP = C_::ZP, ZW = C_::ZW, CPW = C_::CPW, CS = C_::CS,
+                  NR = C_::NR;
+    constexpr size_t H = (size_t)(N / 2 + 1) * N;
+    const int D = p.D, KK = 2 * D + 1, NP = D + 1;                    // host guarantees D <= 16; NP row pairs (the last one is a single row)
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
 
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    c2 *Z = reinterpret_cast<c2 *>(smem_raw);                         // [2][NW][ZW]   warp-private tiles, double-buffered
-    c2 *G = Z + (size_t)2 * NW * ZW;                                  // [CG][KK][GP]  pass-1 output rows of a CTF group
-    float2 *sc = reinterpret_cast<float2 *>(G + (size_t)CG * KK * GP); // [2][CG]      (alpha*beta, h) of the group's CTFs
-    TopEntry *tops = reinterpret_cast<TopEntry *>(sc + 2 * CG);       // [NW][TOPK]
+    c2 *Z = reinterpret_cast<c2 *>(smem_raw);                         // [NW][ZW]         warp-private tiles
+    c2 *G = Z + (size_t)NW * ZW;                                      // [2][CG][KK][GP]  pass-1 output rows of a CTF group, double-buffered over groups
+    const int GSZ = CG * KK * GP;
+    c2 *qn = G + (size_t)2 * GSZ;                                     // [8][N2][2]       Q of the Nyquist column l = N/2 (warp 0, lanes < N2)
+    float4 *kn = reinterpret_cast<float4 *>(qn + 16 * N2);            // [2][4][N2]       K_c(N/2, .) of the current / next CTF  (+ one zero float4)
+    float2 *sc = reinterpret_cast<float2 *>(kn + 8 * N2 + 1);         // [4][CG]          (alpha*beta, h) of the CTFs of the last 4 groups
+    TopEntry *tops = reinterpret_cast<TopEntry *>(sc + 4 * CG);       // [NW][TOPK]
     float *red = reinterpret_cast<float *>(tops + NW * BIOEM_TOPK);   // [2 NW]
 
     int img, model, o_begin, o_end, item;
@@ -225,21 +241,26 @@ __global__ void __launch_bounds__(PK<N>::NT, 1) k_fused_pk(FusedParams p, const 
         o_end = min(o_begin + p.oc, p.n_orient);
     }
     const float beta = p.beta[img];
+    // the pipeline runs two masked warm-up / drain groups: everything it may read must be finite
+    for (int i = tid; i < (NW * ZW + 2 * GSZ + 16 * N2) * 2; i += NT) reinterpret_cast<float *>(Z)[i] = 0.f;
+    for (int i = tid; i < (8 * N2 + 1) * 4; i += NT) reinterpret_cast<float *>(kn)[i] = 0.f;
+    for (int i = tid; i < 4 * CG; i += NT) sc[i] = make_float2(0.f, 0.f);
     if (tid < NW * BIOEM_TOPK) { TopEntry e0 = {-CUDART_INF_F, 0xffffffffu, 0xffffffffu}; tops[tid] = e0; }
     __syncthreads();
 
-    // ---- F-phase constants: thread = (column, residue t)
-    const bool act1 = tid < NTASK;
-    const int col = act1 ? tid / N2 : 0, t = tid % N2;
+    // ---- F-phase constants: thread = (column, residue t); column 0 also carries column N/2 (both are Hermitian in m, so
+    //      the transform of Q(0,.) + i Q(N/2,.) has G(.,0) as its real and G(.,N/2) as its imaginary part)
+    const int col = tid / N2, t = tid % N2;
     const size_t qbase = (size_t)col * N + t;
-    c2 *const Zw = Z + (size_t)warp * ZW;                             // buffer b at Zw + b * NW * ZW
-    constexpr int ZBUF = NW * ZW;
+    c2 *const Zw = Z + (size_t)warp * ZW;
     const int zst_off = (lane / N2) * CS + (lane % N2) * ZP;
-    const int ncols_w = max(0, min(CPW, NC - warp * CPW));            // whole columns owned by this warp
     const bool has_x = D == 16;
     c2 wx;                                                            // exp(2 pi i t / N2) = w_N^{16 t}: the k = +16 output
     sincospif(2.0f * (float)t / (float)N2, &wx.y, &wx.x);
     const bool xlane = has_x && t == 0;
+    const bool nyq = warp == 0 && lane < N2;                          // threads of column 0
+    const float4 *knp = nyq ? kn + t : kn + 8 * N2;                   // other lanes of warp 0 read the zero float4
+    const int kn_str = nyq ? N2 : 0, kn_boff = nyq ? 4 * N2 : 0;
     // ---- H-phase constants: lane = (half, k1); outputs k = k1 - 16 ("lo") and k = k1 ("hi")
     const int half = lane >> 4, k1 = lane & 15;
     const bool vlo = k1 >= 16 - D, vhi = k1 <= D;
@@ -253,8 +274,7 @@ __global__ void __launch_bounds__(PK<N>::NT, 1) k_fused_pk(FusedParams p, const 
     const bool a2two = 2 * a2pr + 1 < KK;
     const float a2bsel = a2two ? 1.f : 0.f;
     const int a2row = 2 * a2pr * GP, a2rowb = a2two ? GP : 0;
-    const int l8 = (t == 0) ? N / 2 : N / 2 - t;                      // j = 8: l = N/2 + t, direct only for t = 0, else mirrored to N/2 - t
-    const float sg8 = (t == 0) ? 1.f : -1.f;
+    const int l8 = (t == 0) ? 0 : N / 2 - t;                          // j = 8: l = N/2 + t -> mirrored N/2 - t; t = 0: the packed entry
     // ---- pass-2 rounds of this lane in H': combo = warp*CPW + 2 cp + half  ->  (cl, first flat shift index of row A)
     int h2cl[NR], h2sha[NR];
     bool h2two[NR];
@@ -273,13 +293,20 @@ __global__ void __launch_bounds__(PK<N>::NT, 1) k_fused_pk(FusedParams p, const 
     const int c_lo = DUMP ? p.dump_ctf : 0, c_hi = DUMP ? p.dump_ctf + 1 : p.n_ctf;
     const float4 *Kt_t = Kt + tid;
     constexpr size_t KSTR = (size_t)(N1 / 4) * NT;                    // float4 per CTF
+    const int gpo = (c_hi - c_lo + CG - 1) / CG;                      // groups per orientation
+    const int total = (o_end - o_begin) * gpo;
 
     float4 kq[N1 / 4];
 #pragma unroll
     for (int g4 = 0; g4 < N1 / 4; ++g4) kq[g4] = Kt_t[(size_t)c_lo * KSTR + (size_t)g4 * NT];
-    int zb = 0, scbuf = 0;
+    int knb = 0;
+    if (nyq) {
+#pragma unroll
+        for (int g4 = 0; g4 < 4; ++g4) pk_cp_async16(kn + g4 * N2 + t, KtN + ((size_t)c_lo * 4 + g4) * N2 + t);
+    }
+    pk_cp_async_commit();
 
-    // a = Q K_c (consumes kq), then prefetch K of CTF `cn`
+    // a = Q K_c (consumes kq; column 0 adds i Q(N/2,.) K_c(N/2,.)), then prefetch K of CTF `cn`
 #define PK_LOAD_A(cn)                                                                                         \
     c2 a[N1];                                                                                                 \
     _Pragma("unroll") for (int g4 = 0; g4 < N1 / 4; ++g4) {                                                   \
@@ -291,123 +318,163 @@ __global__ void __launch_bounds__(PK<N>::NT, 1) k_fused_pk(FusedParams p, const 
     {                                                                                                         \
         const float4 *kp = Kt_t + (size_t)(cn) * KSTR;                                                        \
         _Pragma("unroll") for (int g4 = 0; g4 < N1 / 4; ++g4) kq[g4] = kp[(size_t)g4 * NT];                   \
+    }                                                                                                         \
+    if (warp == 0) {                                                                                          \
+        pk_cp_async_wait_all();                                                                               \
+        _Pragma("unroll") for (int g4 = 0; g4 < 4; ++g4) {                                                    \
+            const float4 k4 = knp[knb * kn_boff + g4 * kn_str];                                                \
+            const float4 qa = *reinterpret_cast<const float4 *>(qn + ((2 * g4) * N2 + t) * 2);                \
+            const float4 qb = *reinterpret_cast<const float4 *>(qn + ((2 * g4 + 1) * N2 + t) * 2);            \
+            a[4 * g4 + 0] = __ffma2_rn(make_float2(-qa.y, qa.x), pk_bc(k4.x), a[4 * g4 + 0]);                 \
+            a[4 * g4 + 1] = __ffma2_rn(make_float2(-qa.w, qa.z), pk_bc(k4.y), a[4 * g4 + 1]);                 \
+            a[4 * g4 + 2] = __ffma2_rn(make_float2(-qb.y, qb.x), pk_bc(k4.z), a[4 * g4 + 2]);                 \
+            a[4 * g4 + 3] = __ffma2_rn(make_float2(-qb.w, qb.z), pk_bc(k4.w), a[4 * g4 + 3]);                 \
+        }                                                                                                     \
+        knb ^= 1;                                                                                             \
+        if (nyq) {                                                                                            \
+            _Pragma("unroll") for (int g4 = 0; g4 < 4; ++g4)                                                  \
+                pk_cp_async16(kn + (knb * 4 + g4) * N2 + t, KtN + ((size_t)(cn) * 4 + g4) * N2 + t);          \
+        }                                                                                                     \
+        pk_cp_async_commit();                                                                                 \
     }
-    // H(ci): pruned outputs of the columns in tile Zr -> rows of G
-#define PK_HORNER_G(Zr, ci)                                                                                   \
+    // H(ci): pruned outputs of the columns in the Z tile -> rows of G
+#define PK_HORNER_G(Gb, ci)                                                                                   \
     {                                                                                                         \
-        c2 *Gc = G + (size_t)(ci) * KK * GP + warp * CPW + half;                                              \
+        c2 *Gc = (Gb) + (size_t)(ci) * KK * GP + warp * CPW + half;                                           \
         _Pragma("unroll") for (int cp = 0; cp < NR; ++cp) {                                                   \
             c2 ylo, yhi;                                                                                      \
-            pk_horner2<N2, ZP>((Zr) + zrd_off + cp * 2 * CS, rlo, rhi, ylo, yhi);                             \
-            const bool cv = 2 * cp + half < ncols_w;                                                          \
-            if (cv && vlo) Gc[kk_lo * GP + 2 * cp] = ylo;                                                     \
-            if (cv && vhi) Gc[kk_hi * GP + 2 * cp] = yhi;                                                     \
+            pk_horner2<N2, ZP>(Zw + zrd_off + cp * 2 * CS, rlo, rhi, ylo, yhi);                               \
+            if (vlo) Gc[kk_lo * GP + 2 * cp] = ylo;                                                           \
+            if (vhi) Gc[kk_hi * GP + 2 * cp] = yhi;                                                           \
         }                                                                                                     \
     }
-    // F(ci) tail: FFT, the k = +16 output from the DC bins, spill to tile Zwr
-#define PK_FFT_SPILL_G(Zwr, ci)                                                                               \
-    {                                                                                                         \
-        pk_fft16(a);                                                                                          \
-        const c2 xs = pk_colsum<N2>(pk_cmul(a[0], wx));                                                       \
-        if (xlane && act1) G[(size_t)(ci) * KK * GP + (size_t)(KK - 1) * GP + col] = xs;                      \
-        pk_spill16((Zwr) + zst_off, a);                                                                       \
-    }
+    // tail of a slot: FFT of a, the k = +16 output from the DC bins (xs), then the tile hand-over
+#define PK_FFT_XS()                                                                                           \
+    pk_fft16(a);                                                                                              \
+    const c2 xs = pk_colsum<N2>(pk_cmul(a[0], wx));
+#define PK_SPILL()                                                                                            \
+    __syncwarp();                         /* every lane has read the previous tile */                         \
+    pk_spill16(Zw + zst_off, a);                                                                              \
+    __syncwarp();
 
-    for (int o = o_begin; o < o_end; ++o) {
-        // ---- Q = conj(Ohat) F0 for this thread's 16 bins (Eq. 12)
-        c2 q[N1];
-        {
+    // ---- the flat, software-pipelined loop over CTF groups (group gi: pass 1 now, F' one group later, H' two groups later)
+    int o = o_begin, c0 = c_lo;
+    int nc1 = 0, nc2 = 0;                                             // CTFs in groups gi-1, gi-2 (0 = no such group)
+    uint32_t pair1 = 0, pair2 = 0;                                    // o * n_ctf + c0 of those groups
+    c2 xs2 = make_float2(0.f, 0.f);                                   // B(dx = +16) of this thread's pass-2 task, from F' to H'
+    c2 q[N1];
+#pragma unroll
+    for (int j = 0; j < N1; ++j) q[j] = make_float2(0.f, 0.f);
+    for (int gi = 0; gi < total + 2; ++gi) {
+        const bool live = gi < total;
+        const int nc = live ? min(CG, c_hi - c0) : 1;
+        c2 *const Gw = G + (size_t)(gi & 1) * GSZ;                    // written by this group's pass 1
+        const c2 *const Gr = G + (size_t)((gi & 1) ^ 1) * GSZ;        // group gi-1: read by F'
+        if (live && c0 == c_lo) {
+            // ---- Q = conj(Ohat) F0 for this thread's 16 bins (Eq. 12), new orientation
             const cf *F0 = p.F0 + ((size_t)model * p.n_orient + o) * H;
 #pragma unroll
             for (int j = 0; j < N1; ++j) {
                 const cf ov = Oimg[qbase + (size_t)N2 * j], fv = F0[qbase + (size_t)N2 * j];
                 const cf pr = cmulc(ov, fv);
-                q[j] = act1 ? make_float2(pr.x, pr.y) : make_float2(0.f, 0.f);
+                q[j] = make_float2(pr.x, pr.y);
             }
-        }
-        for (int c0 = c_lo; c0 < c_hi; c0 += CG) {
-            const int nc = min(CG, c_hi - c0);
-            float2 *scb = sc + scbuf * CG;
-            scbuf ^= 1;
-            if (tid < nc) {                                           // (alpha*beta, h) of CTF c0 + tid
-                const size_t moc = ((size_t)model * p.n_orient + o) * p.n_ctf + c0 + tid;
-                scb[tid] = make_float2(p.alpha[moc] * beta, p.hterm[moc]);
-            }
-            // ================= pass 1, software-pipelined over the CTFs of the group, warp-local
-            {
-                int cn = c0 + 1;
-                if (cn >= c_hi) cn = c_lo;
-                PK_LOAD_A(cn)
-                PK_FFT_SPILL_G(Zw + zb * ZBUF, 0)
-                __syncwarp();
-            }
-            for (int ci = 1; ci < nc; ++ci) {
-                int cn = c0 + ci + 1;
-                if (cn >= c_hi) cn = c_lo;
-                PK_LOAD_A(cn)
-                PK_HORNER_G(Zw + zb * ZBUF, ci - 1)
-                zb ^= 1;
-                PK_FFT_SPILL_G(Zw + zb * ZBUF, ci)
-                __syncwarp();
-            }
-            PK_HORNER_G(Zw + zb * ZBUF, nc - 1)
-            zb ^= 1;
-            __syncthreads();
-            // ================= pass 2: (CTF, row pair) combos, CPW per warp
-            c2 xs2;
-            {
-                const c2 *ga = G + (size_t)(a2cl < nc ? a2cl : 0) * KK * GP + a2row, *gb = ga + a2rowb;
-                c2 a[N1];
+            if (nyq) {
 #pragma unroll
                 for (int j = 0; j < N1; ++j) {
-                    // l = N2 j + t; direct for l <= N/2, mirrored (conjugate) above: a = A + i B of the two real rows
-                    if (j < 8) {
-                        const c2 va = ga[N2 * j + t], vb = gb[N2 * j + t];
-                        a[j] = __ffma2_rn(pk_rot90(vb), pk_bc(a2bsel), va);
-                    } else if (j > 8) {
-                        const c2 va = ga[N - N2 * j - t], vb = gb[N - N2 * j - t];
-                        a[j] = __ffma2_rn(make_float2(vb.y, vb.x), pk_bc(a2bsel), make_float2(va.x, -va.y));
-                    } else {
-                        const c2 va = ga[l8], vb = gb[l8];
-                        a[j] = __ffma2_rn(make_float2(-sg8 * vb.y, vb.x), pk_bc(a2bsel), make_float2(va.x, sg8 * va.y));
-                    }
+                    const size_t e = (size_t)(N / 2) * N + N2 * j + t;
+                    const cf pr = cmulc(Oimg[e], F0[e]);
+                    qn[((j >> 1) * N2 + t) * 2 + (j & 1)] = make_float2(pr.x, pr.y);
                 }
-                pk_fft16(a);
-                xs2 = pk_colsum<N2>(pk_cmul(a[0], wx));               // B(dx = +16) of the two rows
-                pk_spill16(Zw + zb * ZBUF + zst_off, a);
             }
-            __syncthreads();                                          // G consumed (next group may overwrite it), Z tile visible
+            __syncwarp();
+        }
+        if (tid < nc && live) {                                       // (alpha*beta, h) of CTF c0 + tid
+            const size_t moc = ((size_t)model * p.n_orient + o) * p.n_ctf + c0 + tid;
+            sc[(gi & 3) * CG + tid] = make_float2(p.alpha[moc] * beta, p.hterm[moc]);
+        }
+        // ================= slot A: F(0) of this group  ||  H' of group gi-2 (a5 + a6)
+        {
+            int cn = c0 + 1;
+            if (cn >= c_hi) cn = c_lo;
+            PK_LOAD_A(cn)
+            PK_FFT_XS()
+            if (xlane) Gw[(size_t)(KK - 1) * GP + col] = xs;
             {
-                const c2 *Zr = Zw + zb * ZBUF;
-                const uint32_t pair0 = (uint32_t)(o * p.n_ctf + c0);
+                const float2 *scb = sc + ((gi + 2) & 3) * CG;
 #pragma unroll
                 for (int cp = 0; cp < NR; ++cp) {
                     c2 y[2];
-                    pk_horner2<N2, ZP>(Zr + zrd_off + cp * 2 * CS, rlo, rhi, y[0], y[1]);
+                    pk_horner2<N2, ZP>(Zw + zrd_off + cp * 2 * CS, rlo, rhi, y[0], y[1]);
                     const int cl = h2cl[cp];
-                    const bool cv = cl < nc;
+                    const bool cv = cl < nc2;
                     const float2 s2 = scb[cv ? cl : 0];
                     const int sha = h2sha[cp], shb = sha + KK;
                     const bool v[4] = {cv && vlo, cv && vlo && h2two[cp], cv && vhi, cv && vhi && h2two[cp]};
                     const uint32_t sh[4] = {(uint32_t)(sha + kk_lo), (uint32_t)(shb + kk_lo), (uint32_t)(sha + kk_hi), (uint32_t)(shb + kk_hi)};
-                    pk_score<DUMP, 4>(p, st, mylist, y, v, sh, s2.x, s2.y, pair0 + (uint32_t)cl);
+                    pk_score<DUMP, 4>(p, st, mylist, y, v, sh, s2.x, s2.y, pair2 + (uint32_t)cl);
                 }
                 if (has_x) {                                          // dx = +16: one lane per combo holds the two rows' values
-                    const bool cv = t == 0 && a2cl < nc;
-                    const float2 s2 = scb[a2cl < nc ? a2cl : 0];
+                    const bool cv = t == 0 && a2cl < nc2;
+                    const float2 s2 = scb[a2cl < nc2 ? a2cl : 0];
                     const c2 y[1] = {xs2};
                     const int xsha = 2 * a2pr * KK + KK - 1;
                     const bool v[2] = {cv, cv && a2two};
                     const uint32_t sh[2] = {(uint32_t)xsha, (uint32_t)(xsha + KK)};
-                    pk_score<DUMP, 2>(p, st, mylist, y, v, sh, s2.x, s2.y, pair0 + (uint32_t)a2cl);
+                    pk_score<DUMP, 2>(p, st, mylist, y, v, sh, s2.x, s2.y, pair2 + (uint32_t)a2cl);
                 }
             }
-            zb ^= 1;                                                  // the next F(0) must not overwrite the tile H' is still reading
+            PK_SPILL()
         }
+        // ================= slots B: F(ci)  ||  H(ci-1) -> G
+        for (int ci = 1; ci < nc; ++ci) {
+            int cn = c0 + ci + 1;
+            if (cn >= c_hi) cn = c_lo;
+            PK_LOAD_A(cn)
+            PK_HORNER_G(Gw, ci - 1)
+            PK_FFT_XS()
+            if (xlane) Gw[(size_t)ci * KK * GP + (size_t)(KK - 1) * GP + col] = xs;
+            PK_SPILL()
+        }
+        // ================= slot C: F' of group gi-1 (rows of Gr)  ||  H(nc-1) -> G
+        {
+            const c2 *ga = Gr + (size_t)(a2cl < nc1 ? a2cl : 0) * KK * GP + a2row, *gb = ga + a2rowb;
+            c2 a[N1];
+#pragma unroll
+            for (int j = 0; j < N1; ++j) {
+                // l = N2 j + t; direct for l < N/2, mirrored (conjugate) above: a = A + i B of the two real rows
+                if (j > 0 && j < 8) {
+                    const c2 va = ga[N2 * j + t], vb = gb[N2 * j + t];
+                    a[j] = __ffma2_rn(pk_rot90(vb), pk_bc(a2bsel), va);
+                } else if (j > 8) {
+                    const c2 va = ga[N - N2 * j - t], vb = gb[N - N2 * j - t];
+                    a[j] = __ffma2_rn(make_float2(vb.y, vb.x), pk_bc(a2bsel), make_float2(va.x, -va.y));
+                } else if (j == 0) {                                  // t = 0: the packed entry holds (G(.,0), G(.,N/2)), both real
+                    const c2 va = ga[t], vb = gb[t];
+                    const c2 gen = __ffma2_rn(pk_rot90(vb), pk_bc(a2bsel), va);
+                    a[j] = (t == 0) ? make_float2(va.x, a2bsel * vb.x) : gen;
+                } else {
+                    const c2 va = ga[l8], vb = gb[l8];
+                    const c2 gen = __ffma2_rn(make_float2(vb.y, vb.x), pk_bc(a2bsel), make_float2(va.x, -va.y));
+                    a[j] = (t == 0) ? make_float2(va.y, a2bsel * vb.y) : gen;
+                }
+            }
+            PK_HORNER_G(Gw, nc - 1)
+            PK_FFT_XS()
+            xs2 = xs;
+            PK_SPILL()
+        }
+        __syncthreads();                                              // G[gi & 1] complete; every warp is done reading G[(gi-1) & 1]
+        nc2 = nc1; pair2 = pair1;
+        nc1 = live ? nc : 0; pair1 = (uint32_t)(o * p.n_ctf + c0);
+        c0 += CG;
+        if (c0 >= c_hi) { c0 = c_lo; ++o; }
     }
 #undef PK_LOAD_A
 #undef PK_HORNER_G
-#undef PK_FFT_SPILL_G
+#undef PK_FFT_XS
+#undef PK_SPILL
+    pk_cp_async_wait_all();
     if (DUMP) return;
 
     // ---- block reduction, fixed order
@@ -443,33 +510,48 @@ __global__ void __launch_bounds__(PK<N>::NT, 1) k_fused_pk(FusedParams p, const 
 }
 
 // ------------------------------------------------------------------------------------------------ K in task order
-// Kt[c][g4][tid][e] = K_c(l = tid / N2, m = N2 (4 g4 + e) + tid % N2): the 16 values a thread needs are 4 coalesced float4.
+// Kt[c][g4][tid][e]  = K_c(l = tid / N2, m = N2 (4 g4 + e) + tid % N2): the 16 values a thread needs are 4 coalesced float4.
+// KtN[c][g4][t][e]   = K_c(l = N/2,      m = N2 (4 g4 + e) + t): the Nyquist column, read by the threads of column 0.
 template <int N>
-__global__ void k_relayout_K(const float *K32, float4 *Kt, int n_ctf)
+__global__ void k_relayout_K(const float *K32, float4 *Kt, float4 *KtN, int n_ctf)
 {
     typedef PK<N> C_;
     const int c = blockIdx.y, i = blockIdx.x * blockDim.x + threadIdx.x;       // i = g4 * NT + tid
     if (i >= (C_::N1 / 4) * C_::NT) return;
     const int g4 = i / C_::NT, tid = i % C_::NT;
-    float v[4] = {0.f, 0.f, 0.f, 0.f};
-    if (tid < C_::NTASK) {
-        const int col = tid / C_::N2, t = tid % C_::N2;
-        for (int e = 0; e < 4; ++e) v[e] = K32[(size_t)c * C_::NC * N + (size_t)col * N + C_::N2 * (4 * g4 + e) + t];
-    }
+    const int col = tid / C_::N2, t = tid % C_::N2;
+    const float *Kc = K32 + (size_t)c * (N / 2 + 1) * N;
+    float v[4];
+    for (int e = 0; e < 4; ++e) v[e] = Kc[(size_t)col * N + C_::N2 * (4 * g4 + e) + t];
     Kt[(size_t)c * (C_::N1 / 4) * C_::NT + i] = make_float4(v[0], v[1], v[2], v[3]);
+    if (col == 0) {
+        for (int e = 0; e < 4; ++e) v[e] = Kc[(size_t)(N / 2) * N + C_::N2 * (4 * g4 + e) + t];
+        KtN[((size_t)c * 4 + g4) * C_::N2 + t] = make_float4(v[0], v[1], v[2], v[3]);
+    }
 }
 
 bool pk_supported(int N, int D) { return (N == 64 || N == 128) && D <= 16; }
-size_t pk_kt_bytes(int N, int n_ctf) { return N == 64 ? (size_t)n_ctf * 4 * PK<64>::NT * 16 : (size_t)n_ctf * 4 * PK<128>::NT * 16; }
+// Kt followed by KtN
+size_t pk_kt_bytes(int N, int n_ctf)
+{
+    const size_t nt = N == 64 ? PK<64>::NT : PK<128>::NT, n2 = N / 16;
+    return (size_t)n_ctf * 4 * nt * 16 + (size_t)n_ctf * 4 * n2 * 16;
+}
+static const float *pk_ktn(int N, const float *Kt, int n_ctf)
+{
+    const size_t nt = N == 64 ? PK<64>::NT : PK<128>::NT;
+    return Kt + (size_t)n_ctf * 4 * nt * 4;
+}
 
 cudaError_t launch_relayout_K(int N, const float *K32, float *Kt, int n_ctf, cudaStream_t st)
 {
+    float4 *ktn = reinterpret_cast<float4 *>(const_cast<float *>(pk_ktn(N, Kt, n_ctf)));
     if (N == 64) {
         dim3 g((4 * PK<64>::NT + 255) / 256, n_ctf);
-        k_relayout_K<64><<<g, 256, 0, st>>>(K32, reinterpret_cast<float4 *>(Kt), n_ctf);
+        k_relayout_K<64><<<g, 256, 0, st>>>(K32, reinterpret_cast<float4 *>(Kt), ktn, n_ctf);
     } else {
         dim3 g((4 * PK<128>::NT + 255) / 256, n_ctf);
-        k_relayout_K<128><<<g, 256, 0, st>>>(K32, reinterpret_cast<float4 *>(Kt), n_ctf);
+        k_relayout_K<128><<<g, 256, 0, st>>>(K32, reinterpret_cast<float4 *>(Kt), ktn, n_ctf);
     }
     return cudaGetLastError();
 }
@@ -479,13 +561,13 @@ static void pk_plan(int D, int n_ctf, int &CG, int &GP, size_t &bytes)
 {
     typedef PK<N> C_;
     const int KK = 2 * D + 1, NP = D + 1;
-    GP = C_::NC | 1;
-    CG = C_::NT / (NP * C_::N2);                        // CTFs per group: every (CTF, row pair, residue) task of pass 2 has a thread
+    GP = C_::NCH | 1;
+    CG = C_::NCOMBO / NP;                               // CTFs per group: every (CTF, row pair, residue) task of pass 2 has a thread
     if (CG < 1) CG = 1;
     if (CG > n_ctf) CG = n_ctf;
     const size_t budget = 227 * 1024;
     for (;;) {
-        bytes = (size_t)2 * C_::NW * C_::ZW * 8 + (size_t)CG * KK * GP * 8 + 2 * (size_t)CG * 8 +
+        bytes = (size_t)C_::NW * C_::ZW * 8 + (size_t)2 * CG * KK * GP * 8 + 16 * C_::N2 * 8 + (8 * C_::N2 + 1) * 16 + 4 * (size_t)CG * 8 +
                 (size_t)C_::NW * BIOEM_TOPK * sizeof(TopEntry) + 2 * C_::NW * 4 + 64;
         if (bytes <= budget || CG == 1) break;
         --CG;
@@ -499,16 +581,17 @@ static cudaError_t launch_pk_t(const FusedParams &p, const float *Kt, bool dump,
     size_t bytes;
     pk_plan<N>(p.D, p.n_ctf, CG, GP, bytes);
     if (bytes > 227 * 1024) return cudaErrorInvalidConfiguration;
+    const float4 *kt = reinterpret_cast<const float4 *>(Kt), *ktn = reinterpret_cast<const float4 *>(pk_ktn(N, Kt, p.n_ctf));
     cudaError_t e;
     if (dump) {
         e = cudaFuncSetAttribute(k_fused_pk<N, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
         if (e != cudaSuccess) return e;
-        k_fused_pk<N, true><<<1, PK<N>::NT, bytes, st>>>(p, reinterpret_cast<const float4 *>(Kt), CG, GP);
+        k_fused_pk<N, true><<<1, PK<N>::NT, bytes, st>>>(p, kt, ktn, CG, GP);
     } else {
         e = cudaFuncSetAttribute(k_fused_pk<N, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
         if (e != cudaSuccess) return e;
         const int items = p.n_img * p.n_model * p.chunks_per_model;
-        k_fused_pk<N, false><<<items, PK<N>::NT, bytes, st>>>(p, reinterpret_cast<const float4 *>(Kt), CG, GP);
+        k_fused_pk<N, false><<<items, PK<N>::NT, bytes, st>>>(p, kt, ktn, CG, GP);
     }
     return cudaGetLastError();
 }

@@ -120,13 +120,24 @@ def oracle_sample_rate(wl, n_img, n_orient, n_ctf):
     return pairs * s.n_shifts / dt, dt, oracle.num_threads(), f"{n_img} images x {n_orient} orientations x {n_ctf} CTFs x {s.n_shifts} shifts of '{s.name}' (direct summation, model 0)"
 
 
+def oracle_sample_shape(wl, target_s):
+    """Size the bounded sample for about `target_s` seconds of oracle time: all CTFs, up to 16 images (the oracle's OpenMP
+    loop runs over images), and as many orientations as a one-orientation probe says fit."""
+    s = wl["spec"]
+    ni, nc = min(s.n_images, 16), s.n_ctf
+    oracle_sample_rate(wl, ni, 1, nc)                             # build / load / page in / thread start-up, untimed
+    _, dt, _, _ = oracle_sample_rate(wl, ni, 1, nc)
+    no = int(max(1, min(s.n_orient, target_s / max(dt, 1e-6))))
+    return ni, no, nc
+
+
 def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
     wl = build_inputs(args.config, 0)
     s = wl["spec"]
-    ni, no, nc = min(s.n_images, 8), min(s.n_orient, 2), min(s.n_ctf, 4)
+    ni, no, nc = oracle_sample_shape(wl, 6.0)                    # ~6 s of oracle time per step
     for _ in range(args.warmup):
         oracle_sample_rate(wl, 1, 1, 1)
     t_tot, ev = 0.0, 0.0
@@ -238,7 +249,7 @@ def run_ours(args):
             "hbm_alt": {"bytes_per_launch_if_streamed": hbm_bytes, "gbs_equivalent": hbm_bytes / (fused_ms * 1e-3) / 1e9,
                         "peak_gbs": peaks.get("hbm_gbs")},
         }
-        ni, no, nc = min(s.n_images, 8), min(s.n_orient, 2), min(s.n_ctf, 4)
+        ni, no, nc = oracle_sample_shape(wl, 15.0)               # 10-30 s of oracle time
         rate, dt, cores, sample = oracle_sample_rate(wl, ni, no, nc)
         line = {
             "metric": METRIC, "value": evals_job / t_dev, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,

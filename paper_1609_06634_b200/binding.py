@@ -212,6 +212,9 @@ class BioEM:
         self._ck(fn(self._h, img, model, orient, ctf, out.ctypes.data_as(_dp)))
         return out
 
+    def debug_shift_map_f64(self, img, model, orient, ctf):
+        return self.debug_shift_map(img, model, orient, ctf, f64=True)
+
     def debug_log_posterior_f32(self):
         out = np.empty((self.n_img, self.n_models))
         self._ck(self._L.bioem_debug_log_posterior_f32(self._h, out.ctypes.data_as(_dp)))

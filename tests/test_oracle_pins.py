@@ -370,3 +370,43 @@ def test_equal_terms_sum_to_the_term():
     one = oracle.run_model(model, N, 1.0, 0, quats[:1], np.array([[0.0, 1.0, 0.0]]), img)
     assert abs(st.log_posterior()[0] - one.log_posterior()[0]) < 1e-10
     assert st.best_flat[0] == 0            # exact ties keep the lowest flat index (R15)
+
+
+# ------------------------------------------------------------------ stored fixtures (tests/golden/, each file cites its source)
+GOLDEN = __import__("pathlib").Path(__file__).resolve().parent / "golden"
+
+
+def _rows(name):
+    return [ln for ln in (GOLDEN / name).read_text().splitlines() if ln.strip() and not ln.startswith("#")]
+
+
+def test_golden_ctf_constants():
+    g = {r.split()[0]: (float(r.split()[1]), float(r.split()[2])) for r in _rows("ctf_constants.txt")}
+    for kv in (100, 200, 300):
+        v, tol = g[f"lambda_A_{kv}kV"]
+        assert abs(W.generate.electron_wavelength_A(float(kv)) - v) <= tol
+    a, b = W.ctf_from_defocus(1.0, 50.0, 300.0)
+    assert abs(a - g["a_A2_1um_300kV"][0]) <= g["a_A2_1um_300kV"][1]
+    assert abs(b - g["b_A2_B50"][0]) <= g["b_A2_B50"][1]
+    # ... and the oracle's CTF*Env (Eq. 4-5) at that (a, b): first zero of the pure phase CTF (A = 0) at a s^2 / 2 = pi
+    s2 = 2 * np.pi / a
+    assert abs(oracle.ctf_env(s2, a, 0.0, 0.0)) < 1e-12
+    assert abs(oracle.ctf_env(s2, a, 0.0, b) / np.exp(-b * s2 / 2) ) < 1e-12
+    assert abs(oracle.ctf_env(0.5 * s2, a, 0.0, b) - (-np.exp(-b * s2 / 4))) < 1e-12      # a s^2/2 = pi/2: -sin = -1 (R9 sign)
+
+
+def test_golden_closed_form_vs_stored_quadrature_of_eq8():
+    """(C1) and (C2) against the brute-force triple integral of the un-marginalised Eq. 8 on fixed inputs; the
+    expected values were written by tests/golden/make_closed_form_golden.py, which imports nothing of the oracle."""
+    rows = _rows("closed_form_quadrature.txt")
+    assert len(rows) >= 3
+    for r in rows:
+        a, b, c = r.split("|")
+        n = int(a.split()[0])
+        io = np.array([float(x) for x in a.split()[1:]])
+        ic = np.array([float(x) for x in b.split()])
+        want = float(c)
+        assert io.size == n and ic.size == n
+        args = (n, io.sum(), (io * io).sum(), ic.sum(), (ic * ic).sum(), (io * ic).sum())
+        assert abs(oracle.log_post_c1(*args) - want) <= 2e-7
+        assert abs(oracle.log_post_c2(*args) - want) <= 2e-7

@@ -28,6 +28,7 @@
 // No float atomics, fixed reduction orders: bit-reproducible.
 #include "common.cuh"
 #include <math_constants.h>
+#include <vector>
 
 namespace bioem {
 
@@ -153,6 +154,11 @@ __device__ __forceinline__ void pk_topk_insert(float g, uint32_t pair, uint32_t 
 
 struct PkLse { float m, s, thr; };
 
+// Pass-2 task table: slot (= tid / N2) -> (CTF in group << 8 | row pair), 0xffff = idle.  Built on the host (pk_plan) so that
+// the slots of a half-warp read rows whose shared-memory bank offsets tile the 16 eight-byte banks (conflict-free G loads),
+// and so that the idle slots fill whole warps starting at warp 0 (which carries the extra Nyquist-column work of pass 1).
+struct PkMap { uint16_t e[64]; };
+
 // a5 + a6 for the NV (2 or 4) correlations a lane holds: b[i] = (B(dx_i, dy_A), B(dx_i, dy_B)).
 // log1p(-x) = -x (1 + x/2 + x^2/3 + x^3/4 + x^4/5) for x < 2^-6 (truncation < 2e-10 relative); the accurate routine runs
 // only when some lane of the warp is near the posterior peak.
@@ -211,7 +217,7 @@ __device__ __forceinline__ void pk_cp_async_commit() { asm volatile("cp.async.co
 __device__ __forceinline__ void pk_cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 
 template <int N, bool DUMP>
-__global__ void __launch_bounds__(PK<N>::NT, 1) k_fused_pk(FusedParams p, const float4 *__restrict__ Kt, const float4 *__restrict__ KtN, int CG, int GP)
+__global__ void __launch_bounds__(PK<N>::NT, 1) k_fused_pk(FusedParams p, const float4 *__restrict__ Kt, const float4 *__restrict__ KtN, int CG, int GP, const __grid_constant__ PkMap map)
 {
     typedef PK<N> C_;
     constexpr int N1 = C_::N1, N2 = C_::N2, NW = C_::NW, NT = C_::NT, ZP = C_::ZP, ZW = C_::ZW, CPW = C_::CPW, CS = C_::CS,
@@ -270,19 +276,22 @@ __global__ void __launch_bounds__(PK<N>::NT, 1) k_fused_pk(FusedParams p, const 
     sincospif(2.0f * (float)k1 / (float)N, &rhi.y, &rhi.x);
     const int zrd_off = half * CS + k1;                               // + cp * 2 * CS per round
     // ---- pass-2 task of this thread in F': (CTF in group, row pair) = a2combo, residue t
-    const int a2combo = tid / N2, a2cl = a2combo / NP, a2pr = a2combo - a2cl * NP;
+    const int a2combo = tid / N2, a2e = map.e[a2combo], a2cl = a2e >> 8, a2pr = a2e == 0xffff ? 0 : a2e & 255;    // idle: cl = 255
     const bool a2two = 2 * a2pr + 1 < KK;
     const float a2bsel = a2two ? 1.f : 0.f;
     const int a2row = 2 * a2pr * GP, a2rowb = a2two ? GP : 0;
+    bool warp_p2 = false;                                             // does this warp have any pass-2 task at all? (warp-uniform)
+#pragma unroll
+    for (int i = 0; i < CPW; ++i) warp_p2 = warp_p2 || map.e[warp * CPW + i] != 0xffff;
     const int l8 = (t == 0) ? 0 : N / 2 - t;                          // j = 8: l = N/2 + t -> mirrored N/2 - t; t = 0: the packed entry
     // ---- pass-2 rounds of this lane in H': combo = warp*CPW + 2 cp + half  ->  (cl, first flat shift index of row A)
     int h2cl[NR], h2sha[NR];
     bool h2two[NR];
 #pragma unroll
     for (int cp = 0; cp < NR; ++cp) {
-        const int combo = warp * CPW + 2 * cp + half;
-        h2cl[cp] = combo / NP;
-        const int pr = combo - h2cl[cp] * NP;
+        const int he = map.e[warp * CPW + 2 * cp + half];
+        h2cl[cp] = he >> 8;
+        const int pr = he == 0xffff ? 0 : he & 255;
         h2sha[cp] = 2 * pr * KK;
         h2two[cp] = 2 * pr + 1 < KK;
     }
@@ -400,7 +409,7 @@ __global__ void __launch_bounds__(PK<N>::NT, 1) k_fused_pk(FusedParams p, const 
             PK_LOAD_A(cn)
             PK_FFT_XS()
             if (xlane) Gw[(size_t)(KK - 1) * GP + col] = xs;
-            {
+            if (warp_p2) {
                 const float2 *scb = sc + ((gi + 2) & 3) * CG;
 #pragma unroll
                 for (int cp = 0; cp < NR; ++cp) {
@@ -437,7 +446,9 @@ __global__ void __launch_bounds__(PK<N>::NT, 1) k_fused_pk(FusedParams p, const 
             PK_SPILL()
         }
         // ================= slot C: F' of group gi-1 (rows of Gr)  ||  H(nc-1) -> G
-        {
+        if (!warp_p2) {
+            PK_HORNER_G(Gw, nc - 1)
+        } else {
             const c2 *ga = Gr + (size_t)(a2cl < nc1 ? a2cl : 0) * KK * GP + a2row, *gb = ga + a2rowb;
             c2 a[N1];
 #pragma unroll
@@ -556,8 +567,36 @@ cudaError_t launch_relayout_K(int N, const float *K32, float *Kt, int n_ctf, cud
     return cudaGetLastError();
 }
 
+// Assign the CG * NP pass-2 tasks (CTF in group, row pair) to the NCOMBO slots.  A half-warp holds G = 16 / N2 slots, each
+// reading N2 consecutive complex words of one G row per load: the load is conflict-free when the rows' offsets (in 8-byte
+// banks, mod 16) are o, o + N2, o + 2 N2, ...  Tasks are bucketed by offset and drawn accordingly; leftovers fill up in any
+// order.  Groups are placed at the END of the slot range, so the idle slots make warps 0, 1, ... idle in pass 2.
+static bool pk_build_map(int N2, int NCOMBO, int CG, int NP, int KK, int GP, PkMap &map)
+{
+    const int G = 16 / N2;
+    std::vector<std::vector<uint16_t>> bucket(16);
+    for (int cl = 0; cl < CG; ++cl)
+        for (int pr = 0; pr < NP; ++pr) bucket[((long)cl * KK * GP + 2L * pr * GP) % 16].push_back((uint16_t)(cl << 8 | pr));
+    std::vector<uint16_t> slots;
+    for (int o = 0; o < 16; ++o)
+        for (;;) {
+            bool full = true;
+            for (int e = 0; e < G; ++e) full = full && !bucket[(o + e * N2) % 16].empty();
+            if (!full) break;
+            for (int e = 0; e < G; ++e) { auto &b = bucket[(o + e * N2) % 16]; slots.push_back(b.back()); b.pop_back(); }
+        }
+    for (auto &b : bucket)
+        for (uint16_t v : b) slots.push_back(v);
+    while (slots.size() % G) slots.push_back(0xffff);
+    if ((int)slots.size() > NCOMBO) return false;
+    const int idle = NCOMBO - (int)slots.size();
+    for (int i = 0; i < 64; ++i) map.e[i] = 0xffff;
+    for (size_t i = 0; i < slots.size(); ++i) map.e[idle + i] = slots[i];
+    return true;
+}
+
 template <int N>
-static void pk_plan(int D, int n_ctf, int &CG, int &GP, size_t &bytes)
+static void pk_plan(int D, int n_ctf, int &CG, int &GP, size_t &bytes, PkMap &map)
 {
     typedef PK<N> C_;
     const int KK = 2 * D + 1, NP = D + 1;
@@ -569,9 +608,10 @@ static void pk_plan(int D, int n_ctf, int &CG, int &GP, size_t &bytes)
     for (;;) {
         bytes = (size_t)C_::NW * C_::ZW * 8 + (size_t)2 * CG * KK * GP * 8 + 16 * C_::N2 * 8 + (8 * C_::N2 + 1) * 16 + 4 * (size_t)CG * 8 +
                 (size_t)C_::NW * BIOEM_TOPK * sizeof(TopEntry) + 2 * C_::NW * 4 + 64;
-        if (bytes <= budget || CG == 1) break;
+        if ((bytes <= budget && pk_build_map(C_::N2, C_::NCOMBO, CG, NP, KK, GP, map)) || CG == 1) break;
         --CG;
     }
+    if (CG == 1) pk_build_map(C_::N2, C_::NCOMBO, CG, NP, KK, GP, map);
 }
 
 template <int N>
@@ -579,19 +619,20 @@ static cudaError_t launch_pk_t(const FusedParams &p, const float *Kt, bool dump,
 {
     int CG, GP;
     size_t bytes;
-    pk_plan<N>(p.D, p.n_ctf, CG, GP, bytes);
+    PkMap map;
+    pk_plan<N>(p.D, p.n_ctf, CG, GP, bytes, map);
     if (bytes > 227 * 1024) return cudaErrorInvalidConfiguration;
     const float4 *kt = reinterpret_cast<const float4 *>(Kt), *ktn = reinterpret_cast<const float4 *>(pk_ktn(N, Kt, p.n_ctf));
     cudaError_t e;
     if (dump) {
         e = cudaFuncSetAttribute(k_fused_pk<N, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
         if (e != cudaSuccess) return e;
-        k_fused_pk<N, true><<<1, PK<N>::NT, bytes, st>>>(p, kt, ktn, CG, GP);
+        k_fused_pk<N, true><<<1, PK<N>::NT, bytes, st>>>(p, kt, ktn, CG, GP, map);
     } else {
         e = cudaFuncSetAttribute(k_fused_pk<N, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
         if (e != cudaSuccess) return e;
         const int items = p.n_img * p.n_model * p.chunks_per_model;
-        k_fused_pk<N, false><<<items, PK<N>::NT, bytes, st>>>(p, kt, ktn, CG, GP);
+        k_fused_pk<N, false><<<items, PK<N>::NT, bytes, st>>>(p, kt, ktn, CG, GP, map);
     }
     return cudaGetLastError();
 }

@@ -216,6 +216,30 @@ __device__ __forceinline__ void pk_cp_async16(void *smem_dst, const void *gsrc)
 __device__ __forceinline__ void pk_cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void pk_cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 
+// ---- split-phase CTA synchronisation on shared-memory mbarriers (one arrival per warp): a warp ARRIVES when its part of a
+// hand-over is done and WAITS only where it needs the other warps' part, so warps drift by up to a slot instead of meeting
+// at a CTA barrier once per group.
+__device__ __forceinline__ void pk_mbar_init(uint64_t *bar, int count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"((unsigned)__cvta_generic_to_shared(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void pk_mbar_arrive(uint64_t *bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"((unsigned)__cvta_generic_to_shared(bar)) : "memory");
+}
+__device__ __forceinline__ void pk_mbar_wait(uint64_t *bar, unsigned parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred P1;\n"
+        "PK_WAIT:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n"
+        "@P1 bra PK_DONE;\n"
+        "bra PK_WAIT;\n"
+        "PK_DONE:\n"
+        "}" ::"r"((unsigned)__cvta_generic_to_shared(bar)), "r"(parity) : "memory");
+}
+
 template <int N, bool DUMP>
 __global__ void __launch_bounds__(PK<N>::NT, 1) k_fused_pk(FusedParams p, const float4 *__restrict__ Kt, const float4 *__restrict__ KtN, int CG, int GP, const __grid_constant__ PkMap map)
 {
@@ -235,6 +259,7 @@ __global__ void __launch_bounds__(PK<N>::NT, 1) k_fused_pk(FusedParams p, const 
     float2 *sc = reinterpret_cast<float2 *>(kn + 8 * N2 + 1);         // [4][CG]          (alpha*beta, h) of the CTFs of the last 4 groups
     TopEntry *tops = reinterpret_cast<TopEntry *>(sc + 4 * CG);       // [NW][TOPK]
     float *red = reinterpret_cast<float *>(tops + NW * BIOEM_TOPK);   // [2 NW]
+    __shared__ uint64_t mbar[2];                                      // [0] "G rows of group gi written", [1] "G rows of group gi-1 read"
 
     int img, model, o_begin, o_end, item;
     if (DUMP) { img = p.dump_img; model = p.dump_model; o_begin = p.dump_orient; o_end = o_begin + 1; item = 0; }
@@ -252,6 +277,7 @@ __global__ void __launch_bounds__(PK<N>::NT, 1) k_fused_pk(FusedParams p, const 
     for (int i = tid; i < (8 * N2 + 1) * 4; i += NT) reinterpret_cast<float *>(kn)[i] = 0.f;
     for (int i = tid; i < 4 * CG; i += NT) sc[i] = make_float2(0.f, 0.f);
     if (tid < NW * BIOEM_TOPK) { TopEntry e0 = {-CUDART_INF_F, 0xffffffffu, 0xffffffffu}; tops[tid] = e0; }
+    if (tid == 0) { pk_mbar_init(&mbar[0], NW); pk_mbar_init(&mbar[1], NW); }
     __syncthreads();
 
     // ---- F-phase constants: thread = (column, residue t); column 0 also carries column N/2 (both are Hermitian in m, so
@@ -408,7 +434,6 @@ __global__ void __launch_bounds__(PK<N>::NT, 1) k_fused_pk(FusedParams p, const 
             if (cn >= c_hi) cn = c_lo;
             PK_LOAD_A(cn)
             PK_FFT_XS()
-            if (xlane) Gw[(size_t)(KK - 1) * GP + col] = xs;
             if (warp_p2) {
                 const float2 *scb = sc + ((gi + 2) & 3) * CG;
 #pragma unroll
@@ -433,6 +458,8 @@ __global__ void __launch_bounds__(PK<N>::NT, 1) k_fused_pk(FusedParams p, const 
                     pk_score<DUMP, 2>(p, st, mylist, y, v, sh, s2.x, s2.y, pair2 + (uint32_t)a2cl);
                 }
             }
+            if (gi > 0) pk_mbar_wait(&mbar[1], (unsigned)(gi - 1) & 1u);   // every warp has read G[gi & 1] (F' of group gi-2): first write below
+            if (xlane) Gw[(size_t)(KK - 1) * GP + col] = xs;
             PK_SPILL()
         }
         // ================= slots B: F(ci)  ||  H(ci-1) -> G
@@ -446,8 +473,12 @@ __global__ void __launch_bounds__(PK<N>::NT, 1) k_fused_pk(FusedParams p, const 
             PK_SPILL()
         }
         // ================= slot C: F' of group gi-1 (rows of Gr)  ||  H(nc-1) -> G
+        if (gi > 0) pk_mbar_wait(&mbar[0], (unsigned)(gi - 1) & 1u);       // G rows of group gi-1 are complete
         if (!warp_p2) {
+            if (lane == 0) pk_mbar_arrive(&mbar[1]);
             PK_HORNER_G(Gw, nc - 1)
+            __syncwarp();
+            if (lane == 0) pk_mbar_arrive(&mbar[0]);
         } else {
             const c2 *ga = Gr + (size_t)(a2cl < nc1 ? a2cl : 0) * KK * GP + a2row, *gb = ga + a2rowb;
             c2 a[N1];
@@ -470,12 +501,14 @@ __global__ void __launch_bounds__(PK<N>::NT, 1) k_fused_pk(FusedParams p, const 
                     a[j] = (t == 0) ? make_float2(va.y, a2bsel * vb.y) : gen;
                 }
             }
+            __syncwarp();                                             // every lane's loads of G[(gi-1) & 1] are in registers
+            if (lane == 0) pk_mbar_arrive(&mbar[1]);
             PK_HORNER_G(Gw, nc - 1)
             PK_FFT_XS()
             xs2 = xs;
-            PK_SPILL()
+            PK_SPILL()                                                // its __syncwarp orders every lane's G writes before the arrival
+            if (lane == 0) pk_mbar_arrive(&mbar[0]);
         }
-        __syncthreads();                                              // G[gi & 1] complete; every warp is done reading G[(gi-1) & 1]
         nc2 = nc1; pair2 = pair1;
         nc1 = live ? nc : 0; pair1 = (uint32_t)(o * p.n_ctf + c0);
         c0 += CG;

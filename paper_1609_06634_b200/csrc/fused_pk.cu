@@ -157,7 +157,7 @@ struct PkLse { float m, s, thr; };
 // Pass-2 task table: slot (= tid / N2) -> (CTF in group << 8 | row pair), 0xffff = idle.  Built on the host (pk_plan) so that
 // the slots of a half-warp read rows whose shared-memory bank offsets tile the 16 eight-byte banks (conflict-free G loads),
 // and so that the idle slots fill whole warps starting at warp 0 (which carries the extra Nyquist-column work of pass 1).
-struct PkMap { uint16_t e[64]; };
+struct PkMap { uint16_t e[3][64]; int nvar; };     // nvar variants, used round-robin over the CTF groups (see pk_build_map)
 
 // a5 + a6 for the NV (2 or 4) correlations a lane holds: b[i] = (B(dx_i, dy_A), B(dx_i, dy_B)).
 // log1p(-x) = -x (1 + x/2 + x^2/3 + x^3/4 + x^4/5) for x < 2^-6 (truncation < 2e-10 relative); the accurate routine runs
@@ -301,26 +301,12 @@ __global__ void __launch_bounds__(PK<N>::NT, 1) k_fused_pk(FusedParams p, const 
     sincospif(2.0f * (float)(k1 - 16 + N) / (float)N, &rlo.y, &rlo.x);
     sincospif(2.0f * (float)k1 / (float)N, &rhi.y, &rhi.x);
     const int zrd_off = half * CS + k1;                               // + cp * 2 * CS per round
-    // ---- pass-2 task of this thread in F': (CTF in group, row pair) = a2combo, residue t
-    const int a2combo = tid / N2, a2e = map.e[a2combo], a2cl = a2e >> 8, a2pr = a2e == 0xffff ? 0 : a2e & 255;    // idle: cl = 255
-    const bool a2two = 2 * a2pr + 1 < KK;
-    const float a2bsel = a2two ? 1.f : 0.f;
-    const int a2row = 2 * a2pr * GP, a2rowb = a2two ? GP : 0;
-    bool warp_p2 = false;                                             // does this warp have any pass-2 task at all? (warp-uniform)
-#pragma unroll
-    for (int i = 0; i < CPW; ++i) warp_p2 = warp_p2 || map.e[warp * CPW + i] != 0xffff;
+    // ---- pass-2 tasks come from the task table, variant (group index mod nvar): slot a2combo is this thread's F' task, slots
+    //      warp * CPW + 2 cp + half are this lane's H' tasks.  Entry = CTF in group << 8 | row pair; 0xffff = idle (cl = 255).
+    const int a2combo = tid / N2;
     const int l8 = (t == 0) ? 0 : N / 2 - t;                          // j = 8: l = N/2 + t -> mirrored N/2 - t; t = 0: the packed entry
-    // ---- pass-2 rounds of this lane in H': combo = warp*CPW + 2 cp + half  ->  (cl, first flat shift index of row A)
-    int h2cl[NR], h2sha[NR];
-    bool h2two[NR];
-#pragma unroll
-    for (int cp = 0; cp < NR; ++cp) {
-        const int he = map.e[warp * CPW + 2 * cp + half];
-        h2cl[cp] = he >> 8;
-        const int pr = he == 0xffff ? 0 : he & 255;
-        h2sha[cp] = 2 * pr * KK;
-        h2two[cp] = 2 * pr + 1 < KK;
-    }
+    int var0 = 0, var1 = 0, var2 = 0;                                 // variants of groups gi, gi-1, gi-2
+    int eX = 0xffff;                                                  // this thread's F' entry of group gi-2 (owner of xs2)
 
     const cf *Oimg = p.Ohat + (size_t)img * H;
     PkLse st = {LSE_EMPTY, 0.f, -CUDART_INF_F};
@@ -400,6 +386,11 @@ __global__ void __launch_bounds__(PK<N>::NT, 1) k_fused_pk(FusedParams p, const 
     c2 q[N1];
 #pragma unroll
     for (int j = 0; j < N1; ++j) q[j] = make_float2(0.f, 0.f);
+    float2 scn = make_float2(0.f, 0.f);                               // (alpha, h) of the NEXT group's CTF c0 + tid (threads tid < CG)
+    if (tid < CG && total > 0 && c_lo + tid < c_hi) {
+        const size_t moc = ((size_t)model * p.n_orient + o_begin) * p.n_ctf + c_lo + tid;
+        scn = make_float2(p.alpha[moc], p.hterm[moc]);
+    }
     for (int gi = 0; gi < total + 2; ++gi) {
         const bool live = gi < total;
         const int nc = live ? min(CG, c_hi - c0) : 1;
@@ -424,9 +415,14 @@ __global__ void __launch_bounds__(PK<N>::NT, 1) k_fused_pk(FusedParams p, const 
             }
             __syncwarp();
         }
-        if (tid < nc && live) {                                       // (alpha*beta, h) of CTF c0 + tid
-            const size_t moc = ((size_t)model * p.n_orient + o) * p.n_ctf + c0 + tid;
-            sc[(gi & 3) * CG + tid] = make_float2(p.alpha[moc] * beta, p.hterm[moc]);
+        if (tid < CG) {                                               // (alpha*beta, h) of CTF c0 + tid: stored now, fetched a group ahead
+            if (tid < nc && live) sc[(gi & 3) * CG + tid] = make_float2(scn.x * beta, scn.y);
+            int c0n = c0 + CG, on = o;
+            if (c0n >= c_hi) { c0n = c_lo; ++on; }
+            if (gi + 1 < total && c0n + tid < c_hi) {
+                const size_t moc = ((size_t)model * p.n_orient + on) * p.n_ctf + c0n + tid;
+                scn = make_float2(p.alpha[moc], p.hterm[moc]);
+            }
         }
         // ================= slot A: F(0) of this group  ||  H' of group gi-2 (a5 + a6)
         {
@@ -434,28 +430,35 @@ __global__ void __launch_bounds__(PK<N>::NT, 1) k_fused_pk(FusedParams p, const 
             if (cn >= c_hi) cn = c_lo;
             PK_LOAD_A(cn)
             PK_FFT_XS()
-            if (warp_p2) {
+            int h2e[NR];
+#pragma unroll
+            for (int cp = 0; cp < NR; ++cp) h2e[cp] = map.e[var2][warp * CPW + 2 * cp + half];
+            int h2all = 0xffff;
+#pragma unroll
+            for (int cp = 0; cp < NR; ++cp) h2all &= h2e[cp];
+            if (nc2 > 0 && __any_sync(FULLP, h2all != 0xffff)) {      // warp-uniform: some H' task in this warp
                 const float2 *scb = sc + ((gi + 2) & 3) * CG;
 #pragma unroll
                 for (int cp = 0; cp < NR; ++cp) {
                     c2 y[2];
                     pk_horner2<N2, ZP>(Zw + zrd_off + cp * 2 * CS, rlo, rhi, y[0], y[1]);
-                    const int cl = h2cl[cp];
-                    const bool cv = cl < nc2;
+                    const int cl = h2e[cp] >> 8, pr = h2e[cp] == 0xffff ? 0 : h2e[cp] & 255;
+                    const bool cv = cl < nc2, two = 2 * pr + 1 < KK;
                     const float2 s2 = scb[cv ? cl : 0];
-                    const int sha = h2sha[cp], shb = sha + KK;
-                    const bool v[4] = {cv && vlo, cv && vlo && h2two[cp], cv && vhi, cv && vhi && h2two[cp]};
+                    const int sha = 2 * pr * KK, shb = sha + KK;
+                    const bool v[4] = {cv && vlo, cv && vlo && two, cv && vhi, cv && vhi && two};
                     const uint32_t sh[4] = {(uint32_t)(sha + kk_lo), (uint32_t)(shb + kk_lo), (uint32_t)(sha + kk_hi), (uint32_t)(shb + kk_hi)};
                     pk_score<DUMP, 4>(p, st, mylist, y, v, sh, s2.x, s2.y, pair2 + (uint32_t)cl);
                 }
-                if (has_x) {                                          // dx = +16: one lane per combo holds the two rows' values
-                    const bool cv = t == 0 && a2cl < nc2;
-                    const float2 s2 = scb[a2cl < nc2 ? a2cl : 0];
+                if (has_x) {                                          // dx = +16: one lane per task holds the two rows' values
+                    const int xcl = eX >> 8, xpr = eX == 0xffff ? 0 : eX & 255;
+                    const bool cv = t == 0 && xcl < nc2;
+                    const float2 s2 = scb[xcl < nc2 ? xcl : 0];
                     const c2 y[1] = {xs2};
-                    const int xsha = 2 * a2pr * KK + KK - 1;
-                    const bool v[2] = {cv, cv && a2two};
+                    const int xsha = 2 * xpr * KK + KK - 1;
+                    const bool v[2] = {cv, cv && 2 * xpr + 1 < KK};
                     const uint32_t sh[2] = {(uint32_t)xsha, (uint32_t)(xsha + KK)};
-                    pk_score<DUMP, 2>(p, st, mylist, y, v, sh, s2.x, s2.y, pair2 + (uint32_t)a2cl);
+                    pk_score<DUMP, 2>(p, st, mylist, y, v, sh, s2.x, s2.y, pair2 + (uint32_t)xcl);
                 }
             }
             if (gi > 0) pk_mbar_wait(&mbar[1], (unsigned)(gi - 1) & 1u);   // every warp has read G[gi & 1] (F' of group gi-2): first write below
@@ -474,13 +477,17 @@ __global__ void __launch_bounds__(PK<N>::NT, 1) k_fused_pk(FusedParams p, const 
         }
         // ================= slot C: F' of group gi-1 (rows of Gr)  ||  H(nc-1) -> G
         if (gi > 0) pk_mbar_wait(&mbar[0], (unsigned)(gi - 1) & 1u);       // G rows of group gi-1 are complete
-        if (!warp_p2) {
+        const int eF = map.e[var1][a2combo];                          // this thread's F' task of group gi-1
+        if (!(nc1 > 0 && __any_sync(FULLP, eF != 0xffff))) {
             if (lane == 0) pk_mbar_arrive(&mbar[1]);
             PK_HORNER_G(Gw, nc - 1)
             __syncwarp();
             if (lane == 0) pk_mbar_arrive(&mbar[0]);
         } else {
-            const c2 *ga = Gr + (size_t)(a2cl < nc1 ? a2cl : 0) * KK * GP + a2row, *gb = ga + a2rowb;
+            const int a2cl = eF >> 8, a2pr = eF == 0xffff ? 0 : eF & 255;
+            const bool a2two = 2 * a2pr + 1 < KK;
+            const float a2bsel = a2two ? 1.f : 0.f;
+            const c2 *ga = Gr + (size_t)(a2cl < nc1 ? a2cl : 0) * KK * GP + 2 * a2pr * GP, *gb = ga + (a2two ? GP : 0);
             c2 a[N1];
 #pragma unroll
             for (int j = 0; j < N1; ++j) {
@@ -509,7 +516,8 @@ __global__ void __launch_bounds__(PK<N>::NT, 1) k_fused_pk(FusedParams p, const 
             PK_SPILL()                                                // its __syncwarp orders every lane's G writes before the arrival
             if (lane == 0) pk_mbar_arrive(&mbar[0]);
         }
-        nc2 = nc1; pair2 = pair1;
+        nc2 = nc1; pair2 = pair1; eX = eF;
+        var2 = var1; var1 = var0; var0 = var0 + 1 == map.nvar ? 0 : var0 + 1;
         nc1 = live ? nc : 0; pair1 = (uint32_t)(o * p.n_ctf + c0);
         c0 += CG;
         if (c0 >= c_hi) { c0 = c_lo; ++o; }
@@ -622,9 +630,27 @@ static bool pk_build_map(int N2, int NCOMBO, int CG, int NP, int KK, int GP, PkM
         for (uint16_t v : b) slots.push_back(v);
     while (slots.size() % G) slots.push_back(0xffff);
     if ((int)slots.size() > NCOMBO) return false;
-    const int idle = NCOMBO - (int)slots.size();
-    for (int i = 0; i < 64; ++i) map.e[i] = 0xffff;
-    for (size_t i = 0; i < slots.size(); ++i) map.e[idle + i] = slots[i];
+    // Idle slots: whole warps are idle in pass 2.  With 16 warps (4 per scheduler) warp 0 is always one of them (it carries the
+    // Nyquist column in pass 1) and the others rotate over warps 1..3 from group to group (3 variants), so that over three
+    // groups every scheduler sees the same pass-2 load; otherwise one variant with the idle warps first.
+    const int CPW = 32 / N2, NW = NCOMBO / CPW, idle = NCOMBO - (int)slots.size(), idle_w = idle / CPW, rem = idle % CPW;
+    map.nvar = (NW == 16 && idle_w >= 2 && idle_w <= 4) ? 3 : 1;
+    for (int v = 0; v < 3; ++v) {
+        bool iw[64] = {false};
+        if (map.nvar == 3) {
+            iw[0] = true;
+            for (int i = 0; i + 1 < idle_w; ++i) iw[1 + (v + i) % 3] = true;
+        } else
+            for (int w = 0; w < idle_w; ++w) iw[w] = true;
+        for (int i = 0; i < 64; ++i) map.e[v][i] = 0xffff;
+        int skip = rem;
+        size_t k = 0;
+        for (int i = 0; i < NCOMBO; ++i) {
+            if (iw[i / CPW]) continue;
+            if (skip > 0) { --skip; continue; }
+            map.e[v][i] = slots[k++];
+        }
+    }
     return true;
 }
 

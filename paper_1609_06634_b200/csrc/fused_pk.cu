@@ -88,17 +88,25 @@ __device__ __forceinline__ void pk_spill16(c2 *zst, const c2 (&a)[16])
     }
 }
 
-// Two Horner sums over the N2 residues sharing their loads: ylo = sum_t rlo^t z[t], yhi = sum_t rhi^t z[t]
+// Two sums over the N2 residues sharing their loads: ylo = sum_t rlo^t z[t], yhi = sum_t rhi^t z[t], where rlo = rhi w_N^-16, so
+// that rlo^(N2/2) = -rhi^(N2/2) =: -rh.  With P_a = z_a + rh z_(a+N2/2) and M_a = z_a - rh z_(a+N2/2) = 2 z_a - P_a:
+// yhi = sum_a rhi^a P_a, ylo = sum_a rlo^a M_a: two half-length Horner chains (24 instead of 28 packed instructions at N2 = 8).
 template <int N2, int ZP>
-__device__ __forceinline__ void pk_horner2(const c2 *zc, c2 rlo, c2 rhi, c2 &ylo, c2 &yhi)
+__device__ __forceinline__ void pk_horner2(const c2 *zc, c2 rlo, c2 rhi, c2 rh, c2 &ylo, c2 &yhi)
 {
-    c2 z = zc[(N2 - 1) * ZP];
-    ylo = z; yhi = z;
+    constexpr int HF = N2 / 2;
+    c2 P[HF], M[HF];
 #pragma unroll
-    for (int t = N2 - 2; t >= 0; --t) {
-        z = zc[t * ZP];
-        ylo = pk_cmadd(ylo, rlo, z);
-        yhi = pk_cmadd(yhi, rhi, z);
+    for (int a = 0; a < HF; ++a) {
+        const c2 z0 = zc[a * ZP], z1 = zc[(a + HF) * ZP];
+        P[a] = pk_cmadd(z1, rh, z0);
+        M[a] = __ffma2_rn(z0, pk_bc(2.0f), make_float2(-P[a].x, -P[a].y));
+    }
+    yhi = P[HF - 1]; ylo = M[HF - 1];
+#pragma unroll
+    for (int a = HF - 2; a >= 0; --a) {
+        yhi = pk_cmadd(yhi, rhi, P[a]);
+        ylo = pk_cmadd(ylo, rlo, M[a]);
     }
 }
 
@@ -233,11 +241,11 @@ __device__ __forceinline__ void pk_mbar_wait(uint64_t *bar, unsigned parity)
         "{\n"
         ".reg .pred P1;\n"
         "PK_WAIT:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1, %2;\n"
         "@P1 bra PK_DONE;\n"
         "bra PK_WAIT;\n"
         "PK_DONE:\n"
-        "}" ::"r"((unsigned)__cvta_generic_to_shared(bar)), "r"(parity) : "memory");
+        "}" ::"r"((unsigned)__cvta_generic_to_shared(bar)), "r"(parity), "r"(20000u) : "memory");   // suspend-time hint (ns): sleep, do not spin
 }
 
 template <int N, bool DUMP>
@@ -300,6 +308,8 @@ __global__ void __launch_bounds__(PK<N>::NT, 1) k_fused_pk(FusedParams p, const 
     c2 rlo, rhi;
     sincospif(2.0f * (float)(k1 - 16 + N) / (float)N, &rlo.y, &rlo.x);
     sincospif(2.0f * (float)k1 / (float)N, &rhi.y, &rhi.x);
+    c2 rh;                                                            // rhi^(N2/2) = exp(2 pi i k1 / 32)
+    sincospif(2.0f * (float)k1 / 32.0f, &rh.y, &rh.x);
     const int zrd_off = half * CS + k1;                               // + cp * 2 * CS per round
     // ---- pass-2 tasks come from the task table, variant (group index mod nvar): slot a2combo is this thread's F' task, slots
     //      warp * CPW + 2 cp + half are this lane's H' tasks.  Entry = CTF in group << 8 | row pair; 0xffff = idle (cl = 255).
@@ -364,7 +374,7 @@ __global__ void __launch_bounds__(PK<N>::NT, 1) k_fused_pk(FusedParams p, const 
         c2 *Gc = (Gb) + (size_t)(ci) * KK * GP + warp * CPW + half;                                           \
         _Pragma("unroll") for (int cp = 0; cp < NR; ++cp) {                                                   \
             c2 ylo, yhi;                                                                                      \
-            pk_horner2<N2, ZP>(Zw + zrd_off + cp * 2 * CS, rlo, rhi, ylo, yhi);                               \
+            pk_horner2<N2, ZP>(Zw + zrd_off + cp * 2 * CS, rlo, rhi, rh, ylo, yhi);                               \
             if (vlo) Gc[kk_lo * GP + 2 * cp] = ylo;                                                           \
             if (vhi) Gc[kk_hi * GP + 2 * cp] = yhi;                                                           \
         }                                                                                                     \
@@ -441,7 +451,7 @@ __global__ void __launch_bounds__(PK<N>::NT, 1) k_fused_pk(FusedParams p, const 
 #pragma unroll
                 for (int cp = 0; cp < NR; ++cp) {
                     c2 y[2];
-                    pk_horner2<N2, ZP>(Zw + zrd_off + cp * 2 * CS, rlo, rhi, y[0], y[1]);
+                    pk_horner2<N2, ZP>(Zw + zrd_off + cp * 2 * CS, rlo, rhi, rh, y[0], y[1]);
                     const int cl = h2e[cp] >> 8, pr = h2e[cp] == 0xffff ? 0 : h2e[cp] & 255;
                     const bool cv = cl < nc2, two = 2 * pr + 1 < KK;
                     const float2 s2 = scb[cv ? cl : 0];

@@ -235,17 +235,23 @@ __device__ __forceinline__ void pk_mbar_arrive(uint64_t *bar)
 {
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"((unsigned)__cvta_generic_to_shared(bar)) : "memory");
 }
-__device__ __forceinline__ void pk_mbar_wait(uint64_t *bar, unsigned parity)
+__device__ __forceinline__ bool pk_mbar_test(unsigned bar, unsigned parity)
 {
+    unsigned ok;
     asm volatile(
         "{\n"
         ".reg .pred P1;\n"
-        "PK_WAIT:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1, %2;\n"
-        "@P1 bra PK_DONE;\n"
-        "bra PK_WAIT;\n"
-        "PK_DONE:\n"
-        "}" ::"r"((unsigned)__cvta_generic_to_shared(bar)), "r"(parity), "r"(20000u) : "memory");   // suspend-time hint (ns): sleep, do not spin
+        "mbarrier.test_wait.parity.shared::cta.b64 P1, [%1], %2;\n"
+        "selp.u32 %0, 1, 0, P1;\n"
+        "}" : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+    return ok != 0;
+}
+// Usually the phase is already complete (the wait sits about a slot after the last arrival).  A warp that is early -- the
+// warps without a pass-2 task are -- sleeps between probes instead of spinning in the issue slots of its scheduler.
+__device__ __forceinline__ void pk_mbar_wait(uint64_t *bar, unsigned parity)
+{
+    const unsigned b = (unsigned)__cvta_generic_to_shared(bar);
+    while (!pk_mbar_test(b, parity)) __nanosleep(200);
 }
 
 template <int N, bool DUMP>

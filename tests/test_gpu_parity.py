@@ -125,3 +125,51 @@ def test_edge_cases_and_errors():
         b.run()
         dev = b.get_log_posterior()
     assert np.array_equal(dev, _gpu_full(wl)["logp"])
+
+
+@pytest.mark.parametrize("name", ["small"])
+def test_full_size_sampled(name):
+    """BASELINE.json's full size, in the launch configuration bench.py times (same calls, same grid): the full-grid
+    oracle is out of reach (2.6e12 MACs per image), so outputs are checked on samples the oracle computes
+    one by one -- whole shift maps of sampled (image, orientation, CTF) tuples and of every sampled image's reported
+    argmax -- plus properties that hold at any size."""
+    import oracle
+    from paper_1609_06634_b200 import BioEM
+    wl = W.build_workload(name)
+    s = wl["spec"]
+    n = s.n_pix ** 2
+    KK = 2 * s.max_shift + 1
+    model = oracle.prepare_model(wl["models"][0])
+    logw = oracle.uniform_logw(len(wl["quats"]), len(wl["ctfs"]), s.max_shift)
+    rng = np.random.default_rng(7)
+    with BioEM() as b:
+        b.load_workload(wl)
+        b.run()
+        logp, best = b.get_log_posterior(), b.get_best()
+        # (1) random tuples: the whole (2D+1)^2 map against direct summation
+        for _ in range(6):
+            img, o, c = int(rng.integers(s.n_images)), int(rng.integers(s.n_orient)), int(rng.integers(s.n_ctf))
+            I1 = oracle.calc_image(model, wl["quats"][o], wl["ctfs"][c], s.n_pix, s.pixel_A)
+            ref = oracle.shift_map(wl["images"][img], I1, s.max_shift, logw)
+            assert np.abs(b.debug_shift_map(img, 0, o, c, f64=True) - ref).max() <= 1e-6
+            assert np.abs(b.debug_shift_map(img, 0, o, c) - ref).max() <= 5e-7 * n + 1e-3
+        # (2) sampled images: the reported argmax is the maximum of the oracle's map of that (orientation, CTF), at the
+        #     reported shift, with the reported value
+        for img in rng.choice(s.n_images, size=8, replace=False):
+            o, c = int(best["orient"][img, 0]), int(best["ctf"][img, 0])
+            I1 = oracle.calc_image(model, wl["quats"][o], wl["ctfs"][c], s.n_pix, s.pixel_A)
+            ref = np.asarray(oracle.shift_map(wl["images"][img], I1, s.max_shift, logw)).reshape(KK, KK)
+            iy, ix = np.unravel_index(np.argmax(ref), ref.shape)
+            assert (ix - s.max_shift, iy - s.max_shift) == (int(best["dx"][img, 0]), int(best["dy"][img, 0]))
+            assert abs(ref[iy, ix] - best["log_p"][img, 0]) <= TOL_LOGP
+            # the posterior holds at least this map's mass and at most every term at the maximum
+            m = ref.max()
+            assert logp[img, 0] >= m + math.log(np.exp(ref - m).sum()) - TOL_LOGP
+    # (3) properties at any size: max term <= sum <= (number of terms) x max term
+    n_terms = s.n_orient * s.n_ctf * s.n_shifts
+    assert np.all(logp >= best["log_p"] - 1e-9) and np.all(logp <= best["log_p"] + math.log(n_terms) + 1e-9)
+    assert np.all(np.isfinite(logp))
+    # planted parameters (SNR 0.1 at 128^2): the generating orientation and shift are recovered
+    t = wl["truth"]
+    hit = (best["orient"][:, 0] == t["orient"]) & (best["dx"][:, 0] == t["dx"]) & (best["dy"][:, 0] == t["dy"])
+    assert hit.mean() >= 0.95, hit.mean()

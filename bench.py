@@ -35,7 +35,7 @@ UNIT = "evaluations/s"
 SM_COUNT, FP32_LANES = 148, 128
 # dram__bytes_read.sum + dram__bytes_write.sum of the fused kernel, per launch, from the committed `ncu --set full`
 # capture (profiles/); None until a capture of the current kernel exists for that config.
-NCU_TRAFFIC_BYTES = {"small": None}
+NCU_TRAFFIC_BYTES = {"small": 341270528 + 10024960}        # profiles/r1_v11_fused_small_full.csv
 
 
 def algorithmic_flops_per_pair(N: int, D: int) -> float:
@@ -241,7 +241,7 @@ def run_ours(args):
         achieved = fl / (fused_ms * 1e-3) / 1e12
         hbm_bytes = s.n_pairs * 8.0 * s.n_pix * (s.n_pix // 2 + 1)               # streaming Ohat once per pair
         roof = {
-            "bound": "alu", "kernel": "k_fused (a4+a5+a6)", "achieved": achieved, "peak": fp32_peak, "unit": "TFLOP/s",
+            "bound": "alu", "kernel": "k_fused_pk (a4+a5+a6)" if s.n_pix in (64, 128) and s.max_shift <= 16 else "k_fused (a4+a5+a6)", "achieved": achieved, "peak": fp32_peak, "unit": "TFLOP/s",
             "frac": achieved / fp32_peak, "traffic": NCU_TRAFFIC_BYTES.get(s.name),
             "peak_source": f"148 SM x 128 lanes x 2 x {peaks.get('sm_max_mhz', 1965.0):.0f} MHz (formula, {peak_src})",
             "measured_ffma_tflops": fma_meas, "frac_of_measured_ffma": achieved / fma_meas,

@@ -351,8 +351,10 @@ int bioem_run(bioem_ctx *ctx)
     CK(ctx->h64.ensure(MOC * sizeof(double)));
     CK(ctx->alpha32.ensure(MOC * sizeof(float)));
     CK(ctx->h32.ensure(MOC * sizeof(float)));
+    const bool use_pk = pk_supported(N, D), use_c2 = !use_pk && c2_supported(N, D);
     const int oc = choose_oc(I, M, O), cpm = (O + oc - 1) / oc;
-    const size_t items = (size_t)I * M * cpm, IM = (size_t)I * M;
+    const int ppi = use_c2 ? 2 : 1;                                       // partials per work item (the cluster kernel writes one per CTA)
+    const size_t items = (size_t)I * M * cpm * ppi, IM = (size_t)I * M;
     CK(ctx->part_m.ensure(items * sizeof(float)));
     CK(ctx->part_s.ensure(items * sizeof(float)));
     CK(ctx->part_top.ensure(items * BIOEM_TOPK * sizeof(TopEntry)));
@@ -371,10 +373,13 @@ int bioem_run(bioem_ctx *ctx)
     CK(launch_ctf_tables(ctx->ctf_a.as<double>(), ctx->ctf_A.as<double>(), ctx->ctf_b.as<double>(), C, N, ctx->px, ctx->K64.as<double>(),
                          ctx->K32.as<float>(), st));
     ctx->launches += 1;
-    const bool use_pk = pk_supported(N, D);
     if (use_pk) {
         CK(ctx->Kt.ensure(pk_kt_bytes(N, C)));
         CK(launch_relayout_K(N, ctx->K32.as<float>(), ctx->Kt.as<float>(), C, st));
+        ctx->launches += 1;
+    } else if (use_c2) {
+        CK(ctx->Kt.ensure(c2_kt_bytes(C)));
+        CK(launch_relayout_K_c2(ctx->K32.as<float>(), ctx->Kt.as<float>(), C, st));
         ctx->launches += 1;
     }
 
@@ -423,12 +428,13 @@ int bioem_run(bioem_ctx *ctx)
     CK(cudaEventRecord(ctx->ev[1], st));
     int nl = 1;
     if (use_pk) CK(launch_fused_pk(N, p, ctx->Kt.as<float>(), false, st));
+    else if (use_c2) CK(launch_fused_c2(p, ctx->Kt.as<float>(), false, st));
     else CK(launch_fused(N, p, false, st, &nl));
     CK(cudaEventRecord(ctx->ev[2], st));
     ctx->launches += nl; ctx->fused_launches += nl;
 
     // ---- a6 combine, a7 re-score, results
-    CK(launch_merge(p.part_m, p.part_s, p.part_top, I, M, cpm, ctx->m32.as<double>(), ctx->s32.as<double>(), ctx->top.as<TopEntry>(), st));
+    CK(launch_merge(p.part_m, p.part_s, p.part_top, I, M, cpm * ppi, ctx->m32.as<double>(), ctx->s32.as<double>(), ctx->top.as<TopEntry>(), st));
     CK(launch_rescore(ctx->Ohat64.as<cd>(), ctx->F064.as<cd>(), ctx->K64.as<double>(), ctx->Tc64.as<double>(), ctx->h64.as<double>(),
                       ctx->Dw.as<double>(), ctx->top.as<TopEntry>(), BIOEM_TOPK, I, M, O, C, N, D, -1, ctx->g64.as<double>(), st));
     const double nn = (double)n;
@@ -526,6 +532,7 @@ int bioem_debug_shift_map(bioem_ctx *ctx, int img, int model, int orient, int ct
     p.cA = (float)(-0.5 * ((double)n - 3.0) * 1.4426950408889634);
     p.dump = ctx->dump.as<float>(); p.dump_img = img; p.dump_model = model; p.dump_orient = orient; p.dump_ctf = ctf;
     if (pk_supported(N, D)) CK(launch_fused_pk(N, p, ctx->Kt.as<float>(), true, ctx->stream));
+    else if (c2_supported(N, D)) CK(launch_fused_c2(p, ctx->Kt.as<float>(), true, ctx->stream));
     else CK(launch_fused(N, p, true, ctx->stream, nullptr));
     std::vector<float> tmp((size_t)KK * KK);
     rc = fetch(ctx, tmp.data(), ctx->dump.p, tmp.size() * sizeof(float));

@@ -54,6 +54,11 @@ bool pk_supported(int N, int D);
 size_t pk_kt_bytes(int N, int n_ctf);
 cudaError_t launch_relayout_K(int N, const float *K32, float *Kt, int n_ctf, cudaStream_t st);
 cudaError_t launch_fused_pk(int N, const FusedParams &p, const float *Kt, bool dump, cudaStream_t st);
+// two-CTA-cluster variant (N = 224; D <= 31): Q register-resident across a CTA pair; writes TWO partials per work item
+bool c2_supported(int N, int D);
+size_t c2_kt_bytes(int n_ctf);
+cudaError_t launch_relayout_K_c2(const float *K32, float *Kt, int n_ctf, cudaStream_t st);
+cudaError_t launch_fused_c2(const FusedParams &p, const float *Kt, bool dump, cudaStream_t st);
 
 // precompute
 cudaError_t launch_image_stats(const float *img, int n_img, int N, double *centered, double *Dw, cudaStream_t st);

@@ -43,28 +43,26 @@ __device__ __forceinline__ unsigned c2_map(const void *smem_ptr, unsigned rank) 
     asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(a), "r"(rank));
     return r;
 }
-__device__ __forceinline__ void c2_st(unsigned cluster_addr, c2 v)
+// 8-byte store into the shared memory of a CTA of the cluster that also counts its bytes on an mbarrier OF THAT CTA: the
+// barrier's phase completes when every expected byte has landed, so the hand-over needs no fence (a release at cluster scope
+// costs MEMBAR.ALL.GPU per arrival, an acquire at cluster scope an L1 invalidation per wait).
+__device__ __forceinline__ void c2_st_async(unsigned cluster_addr, c2 v, unsigned cluster_mbar)
 {
-    asm volatile("st.shared::cluster.v2.f32 [%0], {%1, %2};" ::"r"(cluster_addr), "f"(v.x), "f"(v.y) : "memory");
+    asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.v2.f32 [%0], {%1, %2}, [%3];" ::"r"(cluster_addr), "f"(v.x),
+                 "f"(v.y), "r"(cluster_mbar) : "memory");
 }
-__device__ __forceinline__ void c2_arrive(unsigned cluster_addr)                       // release at cluster scope: prior (remote) stores are visible to the waiter
+__device__ __forceinline__ void c2_expect_tx(uint64_t *bar, unsigned bytes)            // one arrival + the bytes this phase will receive
 {
-    asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr) : "memory");
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"((unsigned)__cvta_generic_to_shared(bar)), "r"(bytes) : "memory");
 }
-__device__ __forceinline__ void c2_wait(uint64_t *bar, unsigned parity)                // acquire at cluster scope; sleeps between probes
+__device__ __forceinline__ void c2_arrive(unsigned cluster_addr)                       // "my reads are done": no data flows with it
+{
+    asm volatile("mbarrier.arrive.relaxed.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr) : "memory");
+}
+__device__ __forceinline__ void c2_wait(uint64_t *bar, unsigned parity)                // sleeps between probes
 {
     const unsigned b = (unsigned)__cvta_generic_to_shared(bar);
-    for (;;) {
-        unsigned ok;
-        asm volatile(
-            "{\n"
-            ".reg .pred P1;\n"
-            "mbarrier.test_wait.parity.acquire.cluster.shared::cta.b64 P1, [%1], %2;\n"
-            "selp.u32 %0, 1, 0, P1;\n"
-            "}" : "=r"(ok) : "r"(b), "r"(parity) : "memory");
-        if (ok) break;
-        __nanosleep(100);
-    }
+    while (!pk_mbar_test(b, parity)) __nanosleep(200);
 }
 __device__ __forceinline__ void c2_cluster_sync()
 {
@@ -196,7 +194,7 @@ k_fused_c2(FusedParams p, const float4 *__restrict__ Kt, const float *__restrict
     for (int i = tid; i < (NW * ZW + 2 * GSZ + 224) * 2; i += NT) reinterpret_cast<float *>(Z)[i] = 0.f;
     if (tid < NW * BIOEM_TOPK) { TopEntry e0 = {-CUDART_INF_F, 0xffffffffu, 0xffffffffu}; tops[tid] = e0; }
     if (tid == 0) {
-        pk_mbar_init(&bar_full[0], 2 * NW); pk_mbar_init(&bar_full[1], 2 * NW);
+        pk_mbar_init(&bar_full[0], 1); pk_mbar_init(&bar_full[1], 1);
         pk_mbar_init(&bar_empty[0], 2 * P2W); pk_mbar_init(&bar_empty[1], 2 * P2W);
     }
     __syncthreads();
@@ -221,8 +219,10 @@ k_fused_c2(FusedParams p, const float4 *__restrict__ Kt, const float *__restrict
     const unsigned own_lo = (kk_lo >> 1) >= P0, own_hi = (kk_hi >> 1) >= P0;
     const unsigned g_lo = c2_map(G, own_lo) + 8u * (unsigned)(kk_lo - (own_lo ? 2 * P0 : 0));
     const unsigned g_hi = c2_map(G, own_hi) + 8u * (unsigned)(kk_hi - (own_hi ? 2 * P0 : 0));
-    const unsigned full_l[2] = {c2_map(&bar_full[0], rank), c2_map(&bar_full[1], rank)}, full_p[2] = {c2_map(&bar_full[0], peer), c2_map(&bar_full[1], peer)};
+    const unsigned f_lo[2] = {c2_map(&bar_full[0], own_lo), c2_map(&bar_full[1], own_lo)}, f_hi[2] = {c2_map(&bar_full[0], own_hi), c2_map(&bar_full[1], own_hi)};
     const unsigned empty_l[2] = {c2_map(&bar_empty[0], rank), c2_map(&bar_empty[1], rank)}, empty_p[2] = {c2_map(&bar_empty[0], peer), c2_map(&bar_empty[1], peer)};
+    const int rows0 = min(2 * P0, KK);
+    const unsigned full_bytes = 8u * 112u * (unsigned)(rank ? KK - rows0 : rows0);      // bytes one step stores into this CTA's G_T tile
 
     const cf *Oimg = p.Ohat + (size_t)img * H;
     PkLse st = {LSE_EMPTY, 0.f, -CUDART_INF_F};
@@ -271,12 +271,10 @@ k_fused_c2(FusedParams p, const float4 *__restrict__ Kt, const float *__restrict
                 for (int cw = 0; cw < 4; ++cw) {
                     c2 ylo, yhi;
                     c2_horner7(Zw + cw * 7 * ZP + zpos, rlo, rhi, ylo, yhi);
-                    if (vlo) c2_st(g_lo + cb + 8u * (unsigned)(cw * RP), ylo);
-                    if (vhi) c2_st(g_hi + cb + 8u * (unsigned)(cw * RP), yhi);
+                    if (vlo) c2_st_async(g_lo + cb + 8u * (unsigned)(cw * RP), ylo, f_lo[b]);
+                    if (vhi) c2_st_async(g_hi + cb + 8u * (unsigned)(cw * RP), yhi, f_hi[b]);
                 }
             }
-            __syncwarp();                                             // orders every lane's stores before lane 0's release
-            if (lane == 0) { c2_arrive(full_l[b]); c2_arrive(full_p[b]); }
         }
         // ---- pass 2 of step s - 1 (a4 along l, a5, a6) on P2W warps, rotating with the step
         if (s >= 1) {
@@ -288,6 +286,7 @@ k_fused_c2(FusedParams p, const float4 *__restrict__ Kt, const float *__restrict
                 const bool pv = has_col && pl < my_np;
                 const int prf = my_p0 + (pv ? pl : 0);
                 const float bsel = 2 * prf + 1 < KK ? 1.f : 0.f;
+                if (w2 == 0 && lane == 0) c2_expect_tx(&bar_full[b1], full_bytes);   // this phase: one arrival + every byte of the tile
                 c2_wait(&bar_full[b1], (unsigned)(s1 >> 1) & 1u);     // all 28 warps of the cluster have stored their part of buffer b1
                 __syncwarp();                                         // the H-phase reads of this warp's tile are done
                 c2_pass2_f(G + (size_t)b1 * GSZ + 2 * (pv ? pl : 0), t, bsel, zrow);

@@ -28,6 +28,7 @@ struct C2 {
     static constexpr int RP = 34;                                                 // G_T row pitch: [column][local row]
     static constexpr int GSZ = 2 * NCOL * RP;                                     // one G_T buffer: 112 packed columns
     static constexpr int P2W = 4;                                                 // warps running pass 2 in a step
+    static constexpr int NB = 2;                                                  // G_T buffers (3 fits shared memory too; measured no faster: the L1 left for the register spills shrinks)
 };
 
 // ---- cluster helpers
@@ -62,7 +63,7 @@ __device__ __forceinline__ void c2_arrive(unsigned cluster_addr)                
 __device__ __forceinline__ void c2_wait(uint64_t *bar, unsigned parity)                // sleeps between probes
 {
     const unsigned b = (unsigned)__cvta_generic_to_shared(bar);
-    while (!pk_mbar_test(b, parity)) __nanosleep(200);
+    while (!pk_mbar_test(b, parity)) __nanosleep(1000);
 }
 __device__ __forceinline__ void c2_cluster_sync()
 {
@@ -165,7 +166,7 @@ template <bool DUMP>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(C2::NT, 1)
 k_fused_c2(FusedParams p, const float4 *__restrict__ Kt, const float *__restrict__ KtN, int P0)
 {
-    constexpr int N = C2::N, NW = C2::NW, NT = C2::NT, ZP = C2::ZP, ZW = C2::ZW, RP = C2::RP, GSZ = C2::GSZ, P2W = C2::P2W;
+    constexpr int N = C2::N, NW = C2::NW, NT = C2::NT, ZP = C2::ZP, ZW = C2::ZW, RP = C2::RP, GSZ = C2::GSZ, P2W = C2::P2W, NB = C2::NB;
     constexpr size_t H = (size_t)(N / 2 + 1) * N;
     const int D = p.D, KK = 2 * D + 1, NP = D + 1;                    // host guarantees D <= 31; NP row pairs (the last one is a single row)
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -174,11 +175,11 @@ k_fused_c2(FusedParams p, const float4 *__restrict__ Kt, const float *__restrict
 
     extern __shared__ __align__(16) unsigned char smem_raw[];
     c2 *Z = reinterpret_cast<c2 *>(smem_raw);                         // [NW][32][ZP]   warp-private tiles, one row per lane
-    c2 *G = Z + (size_t)NW * ZW;                                      // [2][112][RP]   G_T: pass-1 outputs of this CTA's rows, all columns
-    c2 *qn = G + (size_t)2 * GSZ;                                     // [32][7]        Q of the Nyquist column (rank 0, warp 0)
+    c2 *G = Z + (size_t)NW * ZW;                                      // [NB][112][RP]  G_T: pass-1 outputs of this CTA's rows, all columns
+    c2 *qn = G + (size_t)NB * GSZ;                                    // [32][7]        Q of the Nyquist column (rank 0, warp 0)
     TopEntry *tops = reinterpret_cast<TopEntry *>(qn + 224);          // [NW][TOPK]
     float *red = reinterpret_cast<float *>(tops + NW * BIOEM_TOPK);   // [2 NW]
-    __shared__ uint64_t bar_full[2], bar_empty[2];
+    __shared__ uint64_t bar_full[NB], bar_empty[NB];
 
     int img, model, o_begin, o_end, item;
     if (DUMP) { img = p.dump_img; model = p.dump_model; o_begin = p.dump_orient; o_end = o_begin + 1; item = 0; }
@@ -191,11 +192,10 @@ k_fused_c2(FusedParams p, const float4 *__restrict__ Kt, const float *__restrict
         o_end = min(o_begin + p.oc, p.n_orient);
     }
     const float beta = p.beta[img];
-    for (int i = tid; i < (NW * ZW + 2 * GSZ + 224) * 2; i += NT) reinterpret_cast<float *>(Z)[i] = 0.f;
+    for (int i = tid; i < (NW * ZW + NB * GSZ + 224) * 2; i += NT) reinterpret_cast<float *>(Z)[i] = 0.f;
     if (tid < NW * BIOEM_TOPK) { TopEntry e0 = {-CUDART_INF_F, 0xffffffffu, 0xffffffffu}; tops[tid] = e0; }
     if (tid == 0) {
-        pk_mbar_init(&bar_full[0], 1); pk_mbar_init(&bar_full[1], 1);
-        pk_mbar_init(&bar_empty[0], 2 * P2W); pk_mbar_init(&bar_empty[1], 2 * P2W);
+        for (int i = 0; i < NB; ++i) { pk_mbar_init(&bar_full[i], 1); pk_mbar_init(&bar_empty[i], 2 * P2W); }
     }
     __syncthreads();
     c2_cluster_sync();                                                // both CTAs' tiles are zeroed and barriers initialised before any remote access
@@ -219,8 +219,8 @@ k_fused_c2(FusedParams p, const float4 *__restrict__ Kt, const float *__restrict
     const unsigned own_lo = (kk_lo >> 1) >= P0, own_hi = (kk_hi >> 1) >= P0;
     const unsigned g_lo = c2_map(G, own_lo) + 8u * (unsigned)(kk_lo - (own_lo ? 2 * P0 : 0));
     const unsigned g_hi = c2_map(G, own_hi) + 8u * (unsigned)(kk_hi - (own_hi ? 2 * P0 : 0));
-    const unsigned f_lo[2] = {c2_map(&bar_full[0], own_lo), c2_map(&bar_full[1], own_lo)}, f_hi[2] = {c2_map(&bar_full[0], own_hi), c2_map(&bar_full[1], own_hi)};
-    const unsigned empty_l[2] = {c2_map(&bar_empty[0], rank), c2_map(&bar_empty[1], rank)}, empty_p[2] = {c2_map(&bar_empty[0], peer), c2_map(&bar_empty[1], peer)};
+    const unsigned f_lo = c2_map(&bar_full[0], own_lo), f_hi = c2_map(&bar_full[0], own_hi);       // + 8 b: "full" barrier of buffer b in the owning CTA
+    const unsigned empty_l = c2_map(&bar_empty[0], rank), empty_p = c2_map(&bar_empty[0], peer);
     const int rows0 = min(2 * P0, KK);
     const unsigned full_bytes = 8u * 112u * (unsigned)(rank ? KK - rows0 : rows0);      // bytes one step stores into this CTA's G_T tile
 
@@ -236,9 +236,9 @@ k_fused_c2(FusedParams p, const float4 *__restrict__ Kt, const float *__restrict
 #pragma unroll
     for (int j = 0; j < 32; ++j) q[j] = make_float2(0.f, 0.f);
     int o = o_begin, c = c_lo, o1 = o_begin, c1 = c_lo;               // (o, c) of step s; (o1, c1) of step s - 1
+    unsigned b = 0, ph = 0, b1 = 0, ph1 = 0;                          // buffer s % NB and phase parity (s / NB) & 1 of steps s and s - 1
     for (int s = 0; s <= S; ++s) {
         if (s < S) {
-            const int b = s & 1;
             if (c == c_lo) {
                 // ---- Q = conj(Ohat) F0 for this thread's 32 bins (Eq. 12), new orientation
                 const cf *F0 = p.F0 + ((size_t)model * p.n_orient + o) * H;
@@ -264,21 +264,21 @@ k_fused_c2(FusedParams p, const float4 *__restrict__ Kt, const float *__restrict
             else c2_pass1_f<false>(q, kt, zrow, false, nullptr, nullptr);
             __syncwarp();
             // ---- pass 1, H-phase: the 2D+1 needed outputs of each of the warp's 4 columns -> G_T of the owning CTA
-            if (s >= 2) c2_wait(&bar_empty[b], (unsigned)((s >> 1) - 1) & 1u);      // both CTAs have read buffer b (step s - 2)
+            if (s >= NB) c2_wait(&bar_empty[b], ph ^ 1u);                    // both CTAs have read buffer b (step s - NB)
             {
-                const unsigned cb = 8u * (unsigned)(b * GSZ + (56 * (int)rank + 4 * warp) * RP);
+                const unsigned cb = 8u * (b * (unsigned)GSZ + (unsigned)((56 * (int)rank + 4 * warp) * RP));
 #pragma unroll
                 for (int cw = 0; cw < 4; ++cw) {
                     c2 ylo, yhi;
                     c2_horner7(Zw + cw * 7 * ZP + zpos, rlo, rhi, ylo, yhi);
-                    if (vlo) c2_st_async(g_lo + cb + 8u * (unsigned)(cw * RP), ylo, f_lo[b]);
-                    if (vhi) c2_st_async(g_hi + cb + 8u * (unsigned)(cw * RP), yhi, f_hi[b]);
+                    if (vlo) c2_st_async(g_lo + cb + 8u * (unsigned)(cw * RP), ylo, f_lo + 8u * b);
+                    if (vhi) c2_st_async(g_hi + cb + 8u * (unsigned)(cw * RP), yhi, f_hi + 8u * b);
                 }
             }
         }
         // ---- pass 2 of step s - 1 (a4 along l, a5, a6) on P2W warps, rotating with the step
         if (s >= 1) {
-            const int s1 = s - 1, b1 = s1 & 1;
+            const int s1 = s - 1;
             int w2 = warp - (P2W * s1) % NW;
             if (w2 < 0) w2 += NW;
             if (w2 < P2W) {
@@ -287,11 +287,11 @@ k_fused_c2(FusedParams p, const float4 *__restrict__ Kt, const float *__restrict
                 const int prf = my_p0 + (pv ? pl : 0);
                 const float bsel = 2 * prf + 1 < KK ? 1.f : 0.f;
                 if (w2 == 0 && lane == 0) c2_expect_tx(&bar_full[b1], full_bytes);   // this phase: one arrival + every byte of the tile
-                c2_wait(&bar_full[b1], (unsigned)(s1 >> 1) & 1u);     // all 28 warps of the cluster have stored their part of buffer b1
+                c2_wait(&bar_full[b1], ph1);    // all 28 warps of the cluster have stored their part of buffer b1
                 __syncwarp();                                         // the H-phase reads of this warp's tile are done
                 c2_pass2_f(G + (size_t)b1 * GSZ + 2 * (pv ? pl : 0), t, bsel, zrow);
                 __syncwarp();                                         // tile complete; every lane's G_T loads are in registers
-                if (lane == 0) { c2_arrive(empty_l[b1]); c2_arrive(empty_p[b1]); }
+                if (lane == 0) { c2_arrive(empty_l + 8u * b1); c2_arrive(empty_p + 8u * b1); }
                 const size_t moc = ((size_t)model * p.n_orient + o1) * p.n_ctf + c1;
                 const float ab = p.alpha[moc] * beta, hterm = p.hterm[moc];
                 const uint32_t pair = (uint32_t)(o1 * p.n_ctf + c1);
@@ -308,8 +308,9 @@ k_fused_c2(FusedParams p, const float4 *__restrict__ Kt, const float *__restrict
                 }
             }
         }
-        o1 = o; c1 = c;
+        o1 = o; c1 = c; b1 = b; ph1 = ph;
         if (++c >= c_hi) { c = c_lo; ++o; }
+        if (++b == NB) { b = 0; ph ^= 1u; }
     }
     c2_cluster_sync();                                                // no CTA leaves while its peer may still store to it or arrive on its barriers
     if (DUMP) return;
@@ -382,7 +383,7 @@ cudaError_t launch_relayout_K_c2(const float *K32, float *Kt, int n_ctf, cudaStr
 // Work items: one cluster (2 CTAs) per (image, model, chunk); partial results: 2 per work item (see the kernel's epilogue).
 cudaError_t launch_fused_c2(const FusedParams &p, const float *Kt, bool dump, cudaStream_t st)
 {
-    const size_t bytes = ((size_t)C2::NW * C2::ZW + 2 * C2::GSZ + 224) * 8 + (size_t)C2::NW * BIOEM_TOPK * sizeof(TopEntry) + 2 * C2::NW * 4 + 64;
+    const size_t bytes = ((size_t)C2::NW * C2::ZW + C2::NB * C2::GSZ + 224) * 8 + (size_t)C2::NW * BIOEM_TOPK * sizeof(TopEntry) + 2 * C2::NW * 4 + 64;
     const int P0 = (p.D + 2) / 2;                                     // rank 0 takes ceil(NP / 2) of the NP = D + 1 row pairs
     const float4 *kt = reinterpret_cast<const float4 *>(Kt);
     const float *ktn = c2_ktn(Kt, p.n_ctf);

@@ -241,7 +241,7 @@ def run_ours(args):
         achieved = fl / (fused_ms * 1e-3) / 1e12
         hbm_bytes = s.n_pairs * 8.0 * s.n_pix * (s.n_pix // 2 + 1)               # streaming Ohat once per pair
         roof = {
-            "bound": "alu", "kernel": "k_fused_pk (a4+a5+a6)" if s.n_pix in (64, 128) and s.max_shift <= 16 else "k_fused (a4+a5+a6)", "achieved": achieved, "peak": fp32_peak, "unit": "TFLOP/s",
+            "bound": "alu", "kernel": ("k_fused_pk" if s.n_pix in (64, 128) and s.max_shift <= 16 else "k_fused_c2" if s.n_pix == 224 and s.max_shift <= 31 else "k_fused") + " (a4+a5+a6)", "achieved": achieved, "peak": fp32_peak, "unit": "TFLOP/s",
             "frac": achieved / fp32_peak, "traffic": NCU_TRAFFIC_BYTES.get(s.name),
             "peak_source": f"148 SM x 128 lanes x 2 x {peaks.get('sm_max_mhz', 1965.0):.0f} MHz (formula, {peak_src})",
             "measured_ffma_tflops": fma_meas, "frac_of_measured_ffma": achieved / fma_meas,

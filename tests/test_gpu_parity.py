@@ -174,3 +174,33 @@ def test_full_size_sampled(name):
     ii, mm = np.arange(s.n_images), np.asarray(t["model"])
     hit = (best["orient"][ii, mm] == t["orient"]) & (best["dx"][ii, mm] == t["dx"]) & (best["dy"][ii, mm] == t["dy"])
     assert hit.mean() >= 0.95, hit.mean()
+
+
+# Shift ranges and grid shapes at the edges of each fused kernel's plan: D = 0 and 1 (one CTA of the 224 cluster owns no or a
+# single row), the largest D of the tuned kernels (16 at 64/128, 31 at 224: odd, so the last row pair is a single row of the
+# other CTA), D just above it (generic fallback), a single CTF, a single orientation, odd image counts.
+@pytest.mark.parametrize("base,D,n_img,stride,nctf", [
+    ("tiny_mini", 0, 3, 13, 4), ("tiny_mini", 1, 2, 21, 1), ("tiny_mini", 16, 3, 32, 3), ("tiny_mini", 17, 2, 32, 2),
+    ("small_mini", 0, 2, 2304, 4), ("small_mini", 5, 3, 1536, 3), ("small_mini", 17, 2, 2304, 2),
+    ("paper_mini", 0, 2, 2048, 2), ("paper_mini", 1, 3, 2048, 1), ("paper_mini", 7, 2, 4095, 2), ("paper_mini", 31, 2, 2048, 1),
+])
+def test_kernel_plan_edges(base, D, n_img, stride, nctf):
+    import oracle
+    from paper_1609_06634_b200 import BioEM
+    wl = W.build_workload(W.get_spec(base, n_images=n_img, orient_stride=stride))
+    s = wl["spec"]
+    quats, ctfs, imgs = wl["quats"], wl["ctfs"][:nctf], wl["images"]
+    with BioEM() as b:
+        b.load_workload(wl, images=False)
+        b.set_ctf_grid(ctfs[:, 0], ctfs[:, 1], ctfs[:, 2])
+        b.set_shift_range(D)
+        b.push_images(imgs)
+        b.run()
+        got, best = b.get_log_posterior(), b.get_best()
+    st = oracle.run_model(wl["models"][0], s.n_pix, s.pixel_A, D, quats, ctfs, imgs)
+    assert np.abs(got[:, 0] - st.log_posterior()).max() <= TOL_LOGP
+    o, c, dx, dy = oracle.unflatten(st.best_flat, len(ctfs), D)
+    tie = (st.best - st.second) < 1e-6
+    for k, ref in (("orient", o), ("ctf", c), ("dx", dx), ("dy", dy)):
+        assert np.all((best[k][:, 0] == ref) | tie), (k, best[k][:, 0], ref)
+    assert np.abs(best["log_p"][:, 0] - st.best).max() <= TOL_LOGP

@@ -92,6 +92,17 @@ int bioem_get_log_posterior(bioem_ctx *ctx, double *out);
 int bioem_get_best(bioem_ctx *ctx, int32_t *orient_idx, int32_t *ctf_idx, int32_t *dx, int32_t *dy,
                    double *best_log_p);
 
+/* Posterior as a function of the orientation (the paper's third output):
+ *   out[img][model][o] = log sum_{ctf, d} w(o, ctf, d) P_m,omega(o, ctf, d)      (log-sum-exp over o gives log_posterior).
+ * Off by default.  When enabled before bioem_run, every work item covers ONE orientation, so the per-item partial sums are
+ * the per-orientation sums (same kernels, O x more work items: the per-item prologue and epilogue are no longer amortised over a
+ * chunk of 32 orientations -- measured 2.0x the run time on Small, 32 CTFs per orientation).  The terms that the FP64
+ * re-scoring replaces (the 8 largest per image and model) are replaced here too; the others keep FP32 accuracy
+ * (R24).  enable: 0 | 1.  get_: caller-allocated [n_img][n_model][n_orient] doubles; BIOEM_EBADSTATE if the
+ * last run was made without the option. */
+int bioem_set_orientation_posterior(bioem_ctx *ctx, int enable);
+int bioem_get_orientation_log_posterior(bioem_ctx *ctx, double *out);
+
 /* ---- test / debug entry points (not on the measured path) ---- */
 /* real-space calculated image I1 of (model, orient, ctf) [N][N] ("synthetic map"). */
 int bioem_debug_calc_image(bioem_ctx *ctx, int model, int orient, int ctf, float *out_real);

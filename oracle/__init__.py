@@ -274,6 +274,16 @@ def run_model(model, N, px, D, quats, ctfs, images, lp_orient=None, lp_ctf=None,
     return st
 
 
+def orientation_log_posterior(model, N, px, D, quats, ctfs, images, lp_orient=None, lp_ctf=None):
+    """Posterior as a function of the orientation (the paper's third output): for every image and orientation o,
+    log sum_{ctf, d} w(o, ctf, d) P(o, ctf, d) -- Eq. 9's sum restricted to one orientation, weights of the FULL grid, so that
+    the log-sum-exp over o is log_posterior.  Returns [I][O].  Plain restatement: one run of the loop nest per orientation."""
+    out = np.empty((np.asarray(images).shape[0], len(quats)))
+    for o in range(len(quats)):
+        out[:, o] = run_model(model, N, px, D, quats, ctfs, images, lp_orient, lp_ctf, o_begin=o, o_end=o + 1).log_posterior()
+    return out
+
+
 def shift_map(image, I1, D, logw, tier=0):
     """log P(C1) + logw for every shift of one (image, calc image) pair: [dy+D][dx+D]."""
     image = np.ascontiguousarray(image, dtype=np.float32)

@@ -16,6 +16,7 @@ EXPORTED_SYMBOLS = [
     "bioem_ctf_from_defocus", "bioem_set_shift_range", "bioem_push_images", "bioem_run", "bioem_get_log_posterior",
     "bioem_get_best", "bioem_debug_calc_image", "bioem_debug_shift_map", "bioem_debug_shift_map_f64",
     "bioem_debug_log_posterior_f32", "bioem_get_timing", "bioem_get_launch_count", "bioem_measure_fp32_peak",
+    "bioem_set_orientation_posterior", "bioem_get_orientation_log_posterior",
 ]
 
 _fp = C.POINTER(C.c_float)
@@ -199,6 +200,14 @@ class BioEM:
         self._ck(self._L.bioem_get_best(self._h, o.ctypes.data_as(_ip), c.ctypes.data_as(_ip), dx.ctypes.data_as(_ip),
                                         dy.ctypes.data_as(_ip), lp.ctypes.data_as(_dp)))
         return dict(orient=o, ctf=c, dx=dx, dy=dy, log_p=lp)
+
+    def set_orientation_posterior(self, enable=True):
+        self._ck(self._L.bioem_set_orientation_posterior(self._h, int(bool(enable))))
+
+    def get_orientation_log_posterior(self):
+        out = np.empty((self.n_img, self.n_models, self.n_orient))
+        self._ck(self._L.bioem_get_orientation_log_posterior(self._h, out.ctypes.data_as(_dp)))
+        return out
 
     def debug_calc_image(self, model, orient, ctf):
         out = np.empty((self.n_pix, self.n_pix), dtype=np.float32)

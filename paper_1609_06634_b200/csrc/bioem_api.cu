@@ -58,6 +58,8 @@ struct bioem_ctx {
     DBuf Ohat64, Ohat32, Dw, beta;
     // run state
     bool ran = false;
+    bool want_orient = false, ran_orient = false;      // per-orientation posterior: requested / produced by the last run
+    DBuf logp_orient;
     int run_models = 0, run_orient = 0, run_ctf = 0, run_D = 0, run_img = 0;
     DBuf F064, F032, K64, K32, Kt, Tc64, h64, alpha32, h32;
     DBuf part_m, part_s, part_top, m32, s32, top, g64;
@@ -111,7 +113,7 @@ int bioem_destroy(bioem_ctx *ctx)
     for (auto &m : ctx->models) { m.xyz.release(); m.rad.release(); m.wt.release(); m.rho.release(); }
     DBuf *all[] = {&ctx->rot, &ctx->lp_orient, &ctx->ctf_a, &ctx->ctf_A, &ctx->ctf_b, &ctx->lp_ctf, &ctx->Ohat64, &ctx->Ohat32, &ctx->Dw,
                    &ctx->beta, &ctx->F064, &ctx->F032, &ctx->K64, &ctx->K32, &ctx->Kt, &ctx->Tc64, &ctx->h64, &ctx->alpha32, &ctx->h32,
-                   &ctx->part_m, &ctx->part_s, &ctx->part_top, &ctx->m32, &ctx->s32, &ctx->top, &ctx->g64, &ctx->logp, &ctx->logp32,
+                   &ctx->part_m, &ctx->part_s, &ctx->part_top, &ctx->m32, &ctx->s32, &ctx->top, &ctx->g64, &ctx->logp, &ctx->logp_orient, &ctx->logp32,
                    &ctx->best, &ctx->best_logp, &ctx->scratch_a, &ctx->scratch_b, &ctx->scratch_c, &ctx->dump};
     for (DBuf *b : all) b->release();
     for (int i = 0; i < 4; ++i) if (ctx->ev[i]) cudaEventDestroy(ctx->ev[i]);
@@ -352,7 +354,7 @@ int bioem_run(bioem_ctx *ctx)
     CK(ctx->alpha32.ensure(MOC * sizeof(float)));
     CK(ctx->h32.ensure(MOC * sizeof(float)));
     const bool use_pk = pk_supported(N, D), use_c2 = !use_pk && c2_supported(N, D);
-    const int oc = choose_oc(I, M, O), cpm = (O + oc - 1) / oc;
+    const int oc = ctx->want_orient ? 1 : choose_oc(I, M, O), cpm = (O + oc - 1) / oc;     // one orientation per work item when its posterior is wanted
     const int ppi = use_c2 ? 2 : 1;                                       // partials per work item (the cluster kernel writes one per CTA)
     const size_t items = (size_t)I * M * cpm * ppi, IM = (size_t)I * M;
     CK(ctx->part_m.ensure(items * sizeof(float)));
@@ -442,6 +444,14 @@ int bioem_run(bioem_ctx *ctx)
     CK(launch_final(ctx->m32.as<double>(), ctx->s32.as<double>(), ctx->top.as<TopEntry>(), ctx->g64.as<double>(), ctx->Dw.as<double>(), I, M,
                     C, N, D, const_n, ctx->logp.as<double>(), ctx->logp32.as<double>(), ctx->best.as<int32_t>(), ctx->best_logp.as<double>(), st));
     ctx->launches += 3;
+    ctx->ran_orient = false;
+    if (ctx->want_orient) {
+        CK(ctx->logp_orient.ensure(IM * O * sizeof(double)));
+        CK(launch_orient_final(p.part_m, p.part_s, ppi, ctx->top.as<TopEntry>(), ctx->g64.as<double>(), ctx->Dw.as<double>(), I, M, O, C, N,
+                               const_n, ctx->logp_orient.as<double>(), st));
+        ctx->launches += 1;
+        ctx->ran_orient = true;
+    }
     CK(cudaEventRecord(ctx->ev[3], st));
     ctx->ran = true;
     ctx->run_models = M; ctx->run_orient = O; ctx->run_ctf = C; ctx->run_D = D; ctx->run_img = I;
@@ -461,6 +471,21 @@ int bioem_get_log_posterior(bioem_ctx *ctx, double *out)
     if (!ctx || !out) return BIOEM_EBADARG;
     if (!ctx->ran) FAIL(BIOEM_EBADSTATE, "get_log_posterior: no completed run");
     return fetch(ctx, out, ctx->logp.p, (size_t)ctx->run_img * ctx->run_models * sizeof(double));
+}
+
+int bioem_set_orientation_posterior(bioem_ctx *ctx, int enable)
+{
+    if (!ctx) return BIOEM_EBADARG;
+    if (enable != 0 && enable != 1) FAIL(BIOEM_EBADARG, "set_orientation_posterior: enable must be 0 or 1");
+    ctx->want_orient = enable != 0;
+    return BIOEM_OK;
+}
+
+int bioem_get_orientation_log_posterior(bioem_ctx *ctx, double *out)
+{
+    if (!ctx || !out) return BIOEM_EBADARG;
+    if (!ctx->ran || !ctx->ran_orient) FAIL(BIOEM_EBADSTATE, "get_orientation_log_posterior: no completed run with the option enabled");
+    return fetch(ctx, out, ctx->logp_orient.p, (size_t)ctx->run_img * ctx->run_models * ctx->run_orient * sizeof(double));
 }
 
 int bioem_debug_log_posterior_f32(bioem_ctx *ctx, double *out)

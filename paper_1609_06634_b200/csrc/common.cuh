@@ -85,6 +85,9 @@ cudaError_t launch_rescore(const cd *Ohat64, const cd *F064, const double *K64, 
 cudaError_t launch_final(const double *m32, const double *s32, const TopEntry *top, const double *g64, const double *Dw,
                          int n_img, int n_model, int n_ctf, int N, int D, double const_n, double *logp, double *logp32,
                          int32_t *best, double *best_logp, cudaStream_t st);
+cudaError_t launch_orient_final(const float *part_m, const float *part_s, int parts_per_orient, const TopEntry *top, const double *g64,
+                                const double *Dw, int n_img, int n_model, int n_orient, int n_ctf, int N, double const_n,
+                                double *logp_orient, cudaStream_t st);
 cudaError_t launch_calc_image(const cd *F0, const double *K64, int N, double *out, cudaStream_t st);
 cudaError_t launch_fp32_peak(float *sink, int iters, cudaStream_t st);
 

@@ -167,4 +167,51 @@ cudaError_t launch_final(const double *m32, const double *s32, const TopEntry *t
     return cudaGetLastError();
 }
 
+// Posterior per orientation: with one orientation per work item the per-item partials ARE the per-orientation sums.
+// One thread per (image, model, orientation): combine the item's partials in order (the cluster kernel writes two), replace
+// the re-scored terms of this orientation by their FP64 values, add the constants.
+__global__ void k_orient_final(const float *part_m, const float *part_s, int ppo, const TopEntry *top, const double *g64, const double *Dw,
+                               int n_img, int n_model, int n_orient, int n_ctf, int N, double const_n, double *out)
+{
+    const size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= (size_t)n_img * n_model * n_orient) return;
+    const int o = (int)(idx % n_orient), im = (int)(idx / n_orient), img = im / n_model, model = im % n_model;
+    const double LN2 = 0.6931471805599453, n = (double)N * N;
+    double M = -CUDART_INF, S = 0.0;                       // base-2 units, as the fused kernels write them
+    for (int k = 0; k < ppo; ++k) {
+        const size_t item = (((size_t)model * n_orient + o) * ppo + k) * n_img + img;
+        const double m = part_m[item], s = part_s[item];
+        if (m == -CUDART_INF) continue;
+        if (M == -CUDART_INF) { M = m; S = s; }
+        else if (m > M) { S = S * exp2(M - m) + s; M = m; }
+        else S += s * exp2(m - M);
+    }
+    if (M == -CUDART_INF) { out[idx] = -CUDART_INF; return; }
+    double Mn = M * LN2;
+    const TopEntry *t = top + (size_t)im * BIOEM_TOPK;
+    const double *g = g64 + (size_t)im * BIOEM_TOPK;
+    double ref = Mn;
+    for (int k = 0; k < BIOEM_TOPK; ++k)
+        if (t[k].pair != 0xffffffffu && (int)(t[k].pair / n_ctf) == o && g[k] > ref) ref = g[k];
+    double tot = S * exp(Mn - ref), t32 = 0.0, t64 = 0.0;
+    for (int k = 0; k < BIOEM_TOPK; ++k)
+        if (t[k].pair != 0xffffffffu && (int)(t[k].pair / n_ctf) == o) {
+            t32 += exp((double)t[k].g * LN2 - ref);
+            t64 += exp(g[k] - ref);
+        }
+    double rest = tot - t32;
+    if (rest < 0.0) rest = 0.0;
+    out[idx] = const_n - 0.5 * (n - 3.0) * log(Dw[img]) + ref + log(t64 + rest);
+}
+
+cudaError_t launch_orient_final(const float *part_m, const float *part_s, int parts_per_orient, const TopEntry *top, const double *g64,
+                                const double *Dw, int n_img, int n_model, int n_orient, int n_ctf, int N, double const_n,
+                                double *logp_orient, cudaStream_t st)
+{
+    const size_t n = (size_t)n_img * n_model * n_orient;
+    k_orient_final<<<(unsigned)((n + 127) / 128), 128, 0, st>>>(part_m, part_s, parts_per_orient, top, g64, Dw, n_img, n_model, n_orient, n_ctf, N,
+                                                                const_n, logp_orient);
+    return cudaGetLastError();
+}
+
 }  // namespace bioem

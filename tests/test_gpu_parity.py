@@ -204,3 +204,38 @@ def test_kernel_plan_edges(base, D, n_img, stride, nctf):
     for k, ref in (("orient", o), ("ctf", c), ("dx", dx), ("dy", dy)):
         assert np.all((best[k][:, 0] == ref) | tie), (k, best[k][:, 0], ref)
     assert np.abs(best["log_p"][:, 0] - st.best).max() <= TOL_LOGP
+
+
+@pytest.mark.parametrize("name", ["tiny_mini", "small_mini", "paper_mini", "density_mini", "ensemble_mini"])
+def test_orientation_posterior(name):
+    """posterior per orientation.  Bar: entries that matter (within 30 log-units of the image's
+    maximum) within the FP32 shift-map tolerance of DESIGN 6 / R24; their log-sum-exp over orientations within 1e-3 of the
+    oracle's full log-posterior; the other outputs of the run unchanged (bit-identical argmax, log-posterior within 1e-3)."""
+    import oracle
+    from paper_1609_06634_b200 import BioEM, BioEMError
+    wl = W.build_workload(name)
+    s = wl["spec"]
+    n = s.n_pix ** 2
+    with BioEM() as b:
+        b.load_workload(wl)
+        b.run()
+        with pytest.raises(BioEMError):
+            b.get_orientation_log_posterior()                      # option was off for that run
+        base_lp, base_best = b.get_log_posterior(), b.get_best()
+        b.set_orientation_posterior(True)
+        b.run()
+        po, lp, best = b.get_orientation_log_posterior(), b.get_log_posterior(), b.get_best()
+    assert po.shape == (s.n_images, s.n_models, len(wl["quats"]))
+    assert np.abs(lp - base_lp).max() <= 1e-3
+    for k in ("orient", "ctf", "dx", "dy"):
+        assert np.array_equal(best[k], base_best[k])
+    tol = 5e-7 * n + 1e-3
+    for mi, model in enumerate(wl["models"]):
+        ref = oracle.orientation_log_posterior(model, s.n_pix, s.pixel_A, s.max_shift, wl["quats"], wl["ctfs"], wl["images"])
+        got = po[:, mi, :]
+        rel = ref >= ref.max(axis=1, keepdims=True) - 30.0
+        assert np.abs(got - ref)[rel].max() <= tol, np.abs(got - ref)[rel].max()
+        assert np.abs(got - ref).max() <= 10 * tol                    # the negligible ones too, loosely
+        m = got.max(axis=1)
+        full = oracle.run_model(model, s.n_pix, s.pixel_A, s.max_shift, wl["quats"], wl["ctfs"], wl["images"]).log_posterior()
+        assert np.abs(m + np.log(np.exp(got - m[:, None]).sum(axis=1)) - full).max() <= TOL_LOGP

@@ -410,3 +410,27 @@ def test_golden_closed_form_vs_stored_quadrature_of_eq8():
         args = (n, io.sum(), (io * io).sum(), ic.sum(), (ic * ic).sum(), (io * ic).sum())
         assert abs(oracle.log_post_c1(*args) - want) <= 2e-7
         assert abs(oracle.log_post_c2(*args) - want) <= 2e-7
+
+
+def test_orientation_posterior_pins():
+    """P:225 'posterior as a function of orientation': (i) its log-sum-exp over orientations is the full log-posterior
+    (Eq. 9 is a sum over the grid, so any partition of the grid adds up); (ii) each entry equals the log-sum-exp of the
+    per-shift maps of that orientation's calculated images, built through a different oracle entry point (calc_image +
+    shift_map) and numpy."""
+    import bioem_workloads as W
+    wl = W.build_workload("tiny_mini")
+    s = wl["spec"]
+    quats, ctfs, imgs = wl["quats"][:3], wl["ctfs"][:2], wl["images"][:2]
+    D = 2
+    po = oracle.orientation_log_posterior(wl["models"][0], s.n_pix, s.pixel_A, D, quats, ctfs, imgs)
+    full = oracle.run_model(wl["models"][0], s.n_pix, s.pixel_A, D, quats, ctfs, imgs).log_posterior()
+    m = po.max(axis=1)
+    assert np.abs(m + np.log(np.exp(po - m[:, None]).sum(axis=1)) - full).max() <= 1e-10
+    model = oracle.prepare_model(wl["models"][0])
+    logw = oracle.uniform_logw(len(quats), len(ctfs), D)
+    for i in range(len(imgs)):
+        for o in range(len(quats)):
+            maps = np.stack([oracle.shift_map(imgs[i], oracle.calc_image(model, quats[o], ctfs[c], s.n_pix, s.pixel_A), D, logw)
+                             for c in range(len(ctfs))])
+            mm = maps.max()
+            assert abs(mm + math.log(np.exp(maps - mm).sum()) - po[i, o]) <= 1e-9

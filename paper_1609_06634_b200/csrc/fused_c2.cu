@@ -15,8 +15,9 @@
 // residues for the two needed outputs k1 - 32 and k1 (|k| <= D <= 31), written into the G tile OF THE CTA THAT OWNS THE ROW
 // (rank 0: row pairs 0..P0-1, rank 1: the rest), locally or with st.shared::cluster.  Pass 2 (along l, two real rows per complex
 // transform, Hermitian completion on load) runs one step later on 4 of the 14 warps, rotating from step to step, and scores
-// its outputs at once (a5, a6).  Hand-over: per buffer a "full" mbarrier (28 arrivals: every warp of both CTAs, release at
-// cluster scope after its stores) and an "empty" mbarrier (8 arrivals: the pass-2 warps of both CTAs).
+// its outputs at once (a5, a6).  Hand-over: per buffer a "full" mbarrier whose phase completes when every byte of the tile has
+// landed (the stores are st.async with complete_tx on the owner's barrier: no fence; a release at cluster scope costs a
+// MEMBAR.ALL.GPU per arrival) and an "empty" mbarrier (8 relaxed arrivals: the pass-2 warps of both CTAs).
 // No float atomics, fixed reduction orders: bit-reproducible.
 #include "pk_math.cuh"
 
@@ -339,7 +340,8 @@ k_fused_c2(FusedParams p, const float4 *__restrict__ Kt, const float *__restrict
         for (int w = 1; w < NW; ++w)
             for (int k = 0; k < BIOEM_TOPK; ++k) {
                 TopEntry e = tops[w * BIOEM_TOPK + k];
-                pk_topk_insert(e.g, e.pair, e.shift, lane == 0 && e.pair != 0xffffffffu, th0, tops);
+                if (e.pair == 0xffffffffu || e.g < th0) break;        // lists are sorted: nothing further down can enter (warp-uniform)
+                pk_topk_insert(e.g, e.pair, e.shift, lane == 0, th0, tops);
             }
         __syncwarp();
         // the two CTAs of the cluster are two partials of the same (image, model): chunk' = 2 chunk + rank

@@ -393,7 +393,8 @@ __global__ void __launch_bounds__(PK<N>::NT, 1) k_fused_pk(FusedParams p, const 
         for (int w = 1; w < NW; ++w)
             for (int k = 0; k < BIOEM_TOPK; ++k) {
                 TopEntry e = tops[w * BIOEM_TOPK + k];
-                pk_topk_insert(e.g, e.pair, e.shift, lane == 0 && e.pair != 0xffffffffu, th0, tops);
+                if (e.pair == 0xffffffffu || e.g < th0) break;        // lists are sorted: nothing further down can enter (warp-uniform)
+                pk_topk_insert(e.g, e.pair, e.shift, lane == 0, th0, tops);
             }
         __syncwarp();
         if (lane == 0) { p.part_m[item] = m; p.part_s[item] = s; }

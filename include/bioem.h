@@ -103,6 +103,12 @@ int bioem_get_best(bioem_ctx *ctx, int32_t *orient_idx, int32_t *ctf_idx, int32_
 int bioem_set_orientation_posterior(bioem_ctx *ctx, int enable);
 int bioem_get_orientation_log_posterior(bioem_ctx *ctx, double *out);
 
+/* Ensemble posterior, Eq. 10: log P(M|Omega) = sum_omega log sum_m w_m P_m,omega (up to the constant
+ * the paper drops), from the log-posteriors of the last bioem_run.  weights: host, [n_model], w_m >= 0 (the paper normalises
+ * sum_m w_m = 1; not enforced), NULL = uniform 1/n_model.  out_total: one double.  out_per_image: [n_img] doubles (the
+ * inner log-sums) or NULL.  FP64, fixed summation order. */
+int bioem_get_ensemble_log_posterior(bioem_ctx *ctx, const double *weights, double *out_total, double *out_per_image);
+
 /* ---- test / debug entry points (not on the measured path) ---- */
 /* real-space calculated image I1 of (model, orient, ctf) [N][N] ("synthetic map"). */
 int bioem_debug_calc_image(bioem_ctx *ctx, int model, int orient, int ctf, float *out_real);

@@ -284,6 +284,20 @@ def orientation_log_posterior(model, N, px, D, quats, ctfs, images, lp_orient=No
     return out
 
 
+def ensemble_log_posterior(logp, weights=None):
+    """Eq. 10: log P(M|Omega) = sum_omega log sum_m w_m P_m,omega up to the constant the paper drops.
+    logp: [I][M] log-posteriors; weights: [M] (None = 1/M).  Returns (total, per_image)."""
+    logp = np.asarray(logp, dtype=np.float64)
+    w = np.full(logp.shape[1], 1.0 / logp.shape[1]) if weights is None else np.asarray(weights, dtype=np.float64)
+    per = np.empty(logp.shape[0])
+    for i in range(logp.shape[0]):
+        with np.errstate(divide="ignore"):
+            t = logp[i] + np.log(w)
+        m = t.max()
+        per[i] = m + math.log(sum(math.exp(x - m) for x in t)) if m > -np.inf else -np.inf
+    return float(per.sum()), per
+
+
 def shift_map(image, I1, D, logw, tier=0):
     """log P(C1) + logw for every shift of one (image, calc image) pair: [dy+D][dx+D]."""
     image = np.ascontiguousarray(image, dtype=np.float32)

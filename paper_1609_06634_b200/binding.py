@@ -16,7 +16,7 @@ EXPORTED_SYMBOLS = [
     "bioem_ctf_from_defocus", "bioem_set_shift_range", "bioem_push_images", "bioem_run", "bioem_get_log_posterior",
     "bioem_get_best", "bioem_debug_calc_image", "bioem_debug_shift_map", "bioem_debug_shift_map_f64",
     "bioem_debug_log_posterior_f32", "bioem_get_timing", "bioem_get_launch_count", "bioem_measure_fp32_peak",
-    "bioem_set_orientation_posterior", "bioem_get_orientation_log_posterior",
+    "bioem_set_orientation_posterior", "bioem_get_orientation_log_posterior", "bioem_get_ensemble_log_posterior",
 ]
 
 _fp = C.POINTER(C.c_float)
@@ -208,6 +208,17 @@ class BioEM:
         out = np.empty((self.n_img, self.n_models, self.n_orient))
         self._ck(self._L.bioem_get_orientation_log_posterior(self._h, out.ctypes.data_as(_dp)))
         return out
+
+    def get_ensemble_log_posterior(self, weights=None):
+        """Eq. 10: (total, per_image)."""
+        tot, per = np.empty(1), np.empty(self.n_img)
+        wp = None
+        if weights is not None:
+            w = np.ascontiguousarray(weights, dtype=np.float64)
+            assert w.shape == (self.n_models,)
+            wp = w.ctypes.data_as(_dp)
+        self._ck(self._L.bioem_get_ensemble_log_posterior(self._h, wp, tot.ctypes.data_as(_dp), per.ctypes.data_as(_dp)))
+        return float(tot[0]), per
 
     def debug_calc_image(self, model, orient, ctf):
         out = np.empty((self.n_pix, self.n_pix), dtype=np.float32)

@@ -488,6 +488,32 @@ int bioem_get_orientation_log_posterior(bioem_ctx *ctx, double *out)
     return fetch(ctx, out, ctx->logp_orient.p, (size_t)ctx->run_img * ctx->run_models * ctx->run_orient * sizeof(double));
 }
 
+int bioem_get_ensemble_log_posterior(bioem_ctx *ctx, const double *weights, double *out_total, double *out_per_image)
+{
+    if (!ctx || !out_total) return BIOEM_EBADARG;
+    if (!ctx->ran) FAIL(BIOEM_EBADSTATE, "get_ensemble_log_posterior: no completed run");
+    CK(cudaSetDevice(ctx->device));
+    const int I = ctx->run_img, M = ctx->run_models;
+    std::vector<double> lw(M);
+    for (int m = 0; m < M; ++m) {
+        const double w = weights ? weights[m] : 1.0 / M;
+        if (!(w >= 0.0)) FAIL(BIOEM_EBADARG, "get_ensemble_log_posterior: weights must be >= 0");
+        lw[m] = std::log(w);                                          // w = 0 -> -inf: the model drops out of the sum
+    }
+    DBuf dlw, dpi, dt;
+    cudaError_t e = dlw.ensure(M * sizeof(double));
+    if (e == cudaSuccess) e = dpi.ensure((size_t)I * sizeof(double));
+    if (e == cudaSuccess) e = dt.ensure(sizeof(double));
+    if (e == cudaSuccess) e = cudaMemcpyAsync(dlw.p, lw.data(), M * sizeof(double), cudaMemcpyHostToDevice, ctx->stream);
+    if (e == cudaSuccess) e = launch_ensemble(ctx->logp.as<double>(), dlw.as<double>(), I, M, dpi.as<double>(), dt.as<double>(), ctx->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(out_total, dt.p, sizeof(double), cudaMemcpyDeviceToHost, ctx->stream);
+    if (e == cudaSuccess && out_per_image) e = cudaMemcpyAsync(out_per_image, dpi.p, (size_t)I * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+    dlw.release(); dpi.release(); dt.release();
+    CK(e);
+    return BIOEM_OK;
+}
+
 int bioem_debug_log_posterior_f32(bioem_ctx *ctx, double *out)
 {
     if (!ctx || !out) return BIOEM_EBADARG;

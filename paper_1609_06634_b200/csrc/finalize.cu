@@ -214,4 +214,38 @@ cudaError_t launch_orient_final(const float *part_m, const float *part_s, int pa
     return cudaGetLastError();
 }
 
+// Eq. 10: per image the log of the weighted sum over models, then the sum over images (the log of the product).
+// One CTA, fixed order: thread i takes images i, i + 256, ... in order, then a fixed tree over the 256 partial sums.
+__global__ void __launch_bounds__(256) k_ensemble(const double *logp, const double *logw, int n_img, int n_model, double *per_image, double *total)
+{
+    __shared__ double sh[256];
+    double acc = 0.0;
+    for (int img = threadIdx.x; img < n_img; img += 256) {
+        const double *lp = logp + (size_t)img * n_model;
+        double M = -CUDART_INF;
+        for (int m = 0; m < n_model; ++m) M = fmax(M, lp[m] + logw[m]);
+        double v = M;
+        if (M != -CUDART_INF) {
+            double S = 0.0;
+            for (int m = 0; m < n_model; ++m) S += exp(lp[m] + logw[m] - M);
+            v = M + log(S);
+        }
+        per_image[img] = v;
+        acc += v;
+    }
+    sh[threadIdx.x] = acc;
+    __syncthreads();
+    for (int st = 128; st >= 1; st >>= 1) {
+        if ((int)threadIdx.x < st) sh[threadIdx.x] += sh[threadIdx.x + st];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) *total = sh[0];
+}
+
+cudaError_t launch_ensemble(const double *logp, const double *logw, int n_img, int n_model, double *per_image, double *total, cudaStream_t st)
+{
+    k_ensemble<<<1, 256, 0, st>>>(logp, logw, n_img, n_model, per_image, total);
+    return cudaGetLastError();
+}
+
 }  // namespace bioem

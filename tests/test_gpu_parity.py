@@ -239,3 +239,20 @@ def test_orientation_posterior(name):
         m = got.max(axis=1)
         full = oracle.run_model(model, s.n_pix, s.pixel_A, s.max_shift, wl["quats"], wl["ctfs"], wl["images"]).log_posterior()
         assert np.abs(m + np.log(np.exp(got - m[:, None]).sum(axis=1)) - full).max() <= TOL_LOGP
+
+
+def test_ensemble_posterior_eq10():
+    """Eq. 10 (SURVEY 8(f) #4) from the log-posteriors of a run, against the oracle's Eq. 10 on the ORACLE's log-posteriors."""
+    import oracle
+    from paper_1609_06634_b200 import BioEM
+    wl = W.build_workload("ensemble_mini")
+    ref = _oracle_full(wl)["logp"]
+    w = np.array([0.5, 0.3, 0.2])
+    with BioEM() as b:
+        b.load_workload(wl)
+        b.run()
+        for weights in (None, w, np.array([1.0, 0.0, 0.0])):
+            tot, per = b.get_ensemble_log_posterior(weights)
+            rtot, rper = oracle.ensemble_log_posterior(ref, weights)
+            assert np.abs(per - rper).max() <= TOL_LOGP and abs(tot - rtot) <= TOL_LOGP * len(per)
+            assert abs(per.sum() - tot) <= 1e-9 * abs(tot)

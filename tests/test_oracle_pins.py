@@ -434,3 +434,21 @@ def test_orientation_posterior_pins():
                              for c in range(len(ctfs))])
             mm = maps.max()
             assert abs(mm + math.log(np.exp(maps - mm).sum()) - po[i, o]) <= 1e-9
+
+
+def test_ensemble_posterior_pins():
+    """Eq. 10: against the product of weighted sums written out with plain exp on numbers small enough not to
+    overflow; one model with weight 1 -> sum of its log-posteriors; a common offset c adds I*c; a zero-weight model drops out."""
+    rng = np.random.default_rng(3)
+    lp = rng.normal(0.0, 2.0, size=(5, 4))
+    w = np.array([0.1, 0.2, 0.3, 0.4])
+    tot, per = oracle.ensemble_log_posterior(lp, w)
+    brute = 1.0
+    for i in range(5):
+        brute *= sum(w[m] * math.exp(lp[i, m]) for m in range(4))
+    assert abs(tot - math.log(brute)) <= 1e-12 and abs(per.sum() - tot) <= 1e-12
+    assert abs(oracle.ensemble_log_posterior(lp[:, :1], [1.0])[0] - lp[:, 0].sum()) <= 1e-12
+    assert abs(oracle.ensemble_log_posterior(lp - 1e4, w)[0] - (tot - 5e4)) <= 1e-8
+    assert abs(oracle.ensemble_log_posterior(lp, [0.5, 0.5, 0.0, 0.0])[0] - oracle.ensemble_log_posterior(lp[:, :2], [0.5, 0.5])[0]) <= 1e-12
+    u, _ = oracle.ensemble_log_posterior(lp)
+    assert abs(u - oracle.ensemble_log_posterior(lp, [0.25] * 4)[0]) <= 1e-12

@@ -25,7 +25,7 @@ namespace bioem {
 
 struct C2 {
     static constexpr int N = 224, N2 = 7, NCOL = 56, NW = 14, NT = NW * 32;      // 56 packed columns per CTA, 4 columns x 7 residues per warp
-    static constexpr int ZP = 34, ZW = 32 * ZP;                                   // Z row pitch (16-byte units odd: conflict-free 128-bit rows); one row per lane (28 used)
+    static constexpr int ZP = 34, ZW = 28 * ZP;                                   // Z row pitch (16-byte units odd: conflict-free 128-bit rows); one row per lane with a column
     static constexpr int RP = 34;                                                 // G_T row pitch: [column][local row]
     static constexpr int GSZ = 2 * NCOL * RP;                                     // one G_T buffer: 112 packed columns
     static constexpr int P2W = 4;                                                 // warps running pass 2 in a step
@@ -86,37 +86,49 @@ __device__ __forceinline__ void c2_horner7(const c2 *zc, c2 rlo, c2 rhi, c2 &ylo
 
 // Second half of a 32-point transform whose first radix-2 stage has been applied: FFT16 of u -> even outputs at row words
 // 0..15, then v_j = d_j w32^j (d read back from row words 16..31), FFT16 -> odd outputs at row words 16..31.
-__device__ __forceinline__ void c2_fft32_tail(c2 (&a)[16], c2 *zrow)
+__device__ __forceinline__ void c2_spill16(c2 *zst, const c2 (&a)[16], bool act)
+{
+#pragma unroll
+    for (int r = 0; r < 8; ++r) {
+        const int b = bitrev(r, 3);
+        if (act) *reinterpret_cast<float4 *>(zst + 2 * b) = make_float4(a[r].x, a[r].y, a[r + 8].x, a[r + 8].y);
+    }
+}
+__device__ __forceinline__ void c2_fft32_tail(c2 (&a)[16], c2 *zrow, bool act)
 {
     pk_fft16(a);
-    pk_spill16(zrow, a);
+    c2_spill16(zrow, a, act);
 #pragma unroll
     for (int j = 0; j < 16; j += 2) {
-        const float4 d = *reinterpret_cast<const float4 *>(zrow + 16 + j);
+        float4 d = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (act) d = *reinterpret_cast<const float4 *>(zrow + 16 + j);
         a[j] = pk_twid(make_float2(d.x, d.y), j);
         a[j + 1] = pk_twid(make_float2(d.z, d.w), j + 1);
     }
     pk_fft16(a);
-    pk_spill16(zrow + 16, a);
+    c2_spill16(zrow + 16, a, act);
 }
 
 // F-phase of pass 1 for one CTF: x_j = Q_j K_j (m = 7 j + t), first radix-2 stage on the fly, two 16-point transforms.
 // NYQ: the threads of packed column 0 add i Q(112, m) K(112, m) (both columns are Hermitian in m, so the transform of the sum
 // is G(., 0) + i G(., 112) with both parts real).
 template <bool NYQ>
-__device__ __forceinline__ void c2_pass1_f(const c2 (&q)[32], const float4 *__restrict__ kt, c2 *zrow, bool nyq, const c2 *qn, const float *__restrict__ kn)
+__device__ __forceinline__ void c2_pass1_f(const c2 (&q)[16], const float4 *qs, const float4 *__restrict__ kt, c2 *zrow, bool act, bool nyq,
+                                           const c2 *qn, const float *__restrict__ kn)
 {
     c2 a[16];
 #pragma unroll
     for (int g = 0; g < 4; ++g) {
         const float4 kA = kt[(size_t)g * C2::NT], kB = kt[(size_t)(g + 4) * C2::NT];
+        const float4 qh0 = qs[(size_t)(2 * g) * C2::NT], qh1 = qs[(size_t)(2 * g + 1) * C2::NT];     // Q_(16 + 4g .. 16 + 4g + 3) of this thread
         const float ka[4] = {kA.x, kA.y, kA.z, kA.w}, kb[4] = {kB.x, kB.y, kB.z, kB.w};
+        const c2 qh[4] = {make_float2(qh0.x, qh0.y), make_float2(qh0.z, qh0.w), make_float2(qh1.x, qh1.y), make_float2(qh1.z, qh1.w)};
         c2 d[4];
 #pragma unroll
         for (int e = 0; e < 4; ++e) {
             const int j = 4 * g + e;
             c2 xA = __fmul2_rn(q[j], pk_bc(ka[e]));
-            c2 xB = __fmul2_rn(q[j + 16], pk_bc(kb[e]));
+            c2 xB = __fmul2_rn(qh[e], pk_bc(kb[e]));
             if (NYQ && nyq) {
                 xA = __ffma2_rn(pk_rot90(qn[j * 7]), pk_bc(kn[j * 7]), xA);
                 xB = __ffma2_rn(pk_rot90(qn[(j + 16) * 7]), pk_bc(kn[(j + 16) * 7]), xB);
@@ -124,16 +136,18 @@ __device__ __forceinline__ void c2_pass1_f(const c2 (&q)[32], const float4 *__re
             a[j] = pk_add(xA, xB);
             d[e] = pk_sub(xA, xB);
         }
-        *reinterpret_cast<float4 *>(zrow + 16 + 4 * g) = make_float4(d[0].x, d[0].y, d[1].x, d[1].y);
-        *reinterpret_cast<float4 *>(zrow + 16 + 4 * g + 2) = make_float4(d[2].x, d[2].y, d[3].x, d[3].y);
+        if (act) {
+            *reinterpret_cast<float4 *>(zrow + 16 + 4 * g) = make_float4(d[0].x, d[0].y, d[1].x, d[1].y);
+            *reinterpret_cast<float4 *>(zrow + 16 + 4 * g + 2) = make_float4(d[2].x, d[2].y, d[3].x, d[3].y);
+        }
     }
-    c2_fft32_tail(a, zrow);
+    c2_fft32_tail(a, zrow, act);
 }
 
 // F' of pass 2 for one row pair: the 224-point transform along l of A + i B (rows A, B of this CTA's G_T tile, read as one
 // 128-bit word per column), thread = (pair, residue t), l = 7 j + t.  Columns l = 1..111 are stored, l = 113..223 are their
 // conjugates (Hermitian half), packed column 0 holds (G(., 0), G(., 112)), both real.
-__device__ __forceinline__ void c2_pass2_f(const c2 *gt, int t, float bsel, c2 *zrow)
+__device__ __forceinline__ void c2_pass2_f(const c2 *gt, int t, float bsel, c2 *zrow, bool act)
 {
     c2 a[16];
     const c2 bs = pk_bc(bsel);
@@ -157,10 +171,12 @@ __device__ __forceinline__ void c2_pass2_f(const c2 *gt, int t, float bsel, c2 *
             a[j] = pk_add(xl, xh);
             d[e] = pk_sub(xl, xh);
         }
-        *reinterpret_cast<float4 *>(zrow + 16 + 4 * g) = make_float4(d[0].x, d[0].y, d[1].x, d[1].y);
-        *reinterpret_cast<float4 *>(zrow + 16 + 4 * g + 2) = make_float4(d[2].x, d[2].y, d[3].x, d[3].y);
+        if (act) {
+            *reinterpret_cast<float4 *>(zrow + 16 + 4 * g) = make_float4(d[0].x, d[0].y, d[1].x, d[1].y);
+            *reinterpret_cast<float4 *>(zrow + 16 + 4 * g + 2) = make_float4(d[2].x, d[2].y, d[3].x, d[3].y);
+        }
     }
-    c2_fft32_tail(a, zrow);
+    c2_fft32_tail(a, zrow, act);
 }
 
 template <bool DUMP>
@@ -175,9 +191,10 @@ k_fused_c2(FusedParams p, const float4 *__restrict__ Kt, const float *__restrict
     const int my_p0 = rank ? P0 : 0, my_np = rank ? NP - P0 : P0;     // this CTA's row pairs [my_p0, my_p0 + my_np)
 
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    c2 *Z = reinterpret_cast<c2 *>(smem_raw);                         // [NW][32][ZP]   warp-private tiles, one row per lane
+    c2 *Z = reinterpret_cast<c2 *>(smem_raw);                         // [NW][28][ZP]   warp-private tiles, one row per lane with a column
     c2 *G = Z + (size_t)NW * ZW;                                      // [NB][112][RP]  G_T: pass-1 outputs of this CTA's rows, all columns
-    c2 *qn = G + (size_t)NB * GSZ;                                    // [32][7]        Q of the Nyquist column (rank 0, warp 0)
+    float4 *Qs = reinterpret_cast<float4 *>(G + (size_t)NB * GSZ);    // [8][NT]        upper half of Q (j = 16..31): 2 complex per word, own thread's only
+    c2 *qn = reinterpret_cast<c2 *>(Qs + 8 * NT);                                   // [32][7]        Q of the Nyquist column (rank 0, warp 0)
     TopEntry *tops = reinterpret_cast<TopEntry *>(qn + 224);          // [NW][TOPK]
     float *red = reinterpret_cast<float *>(tops + NW * BIOEM_TOPK);   // [2 NW]
     __shared__ uint64_t bar_full[NB], bar_empty[NB];
@@ -193,7 +210,7 @@ k_fused_c2(FusedParams p, const float4 *__restrict__ Kt, const float *__restrict
         o_end = min(o_begin + p.oc, p.n_orient);
     }
     const float beta = p.beta[img];
-    for (int i = tid; i < (NW * ZW + NB * GSZ + 224) * 2; i += NT) reinterpret_cast<float *>(Z)[i] = 0.f;
+    for (int i = tid; i < (NW * ZW + NB * GSZ + 16 * NT + 224) * 2; i += NT) reinterpret_cast<float *>(Z)[i] = 0.f;
     if (tid < NW * BIOEM_TOPK) { TopEntry e0 = {-CUDART_INF_F, 0xffffffffu, 0xffffffffu}; tops[tid] = e0; }
     if (tid == 0) {
         for (int i = 0; i < NB; ++i) { pk_mbar_init(&bar_full[i], 1); pk_mbar_init(&bar_empty[i], 2 * P2W); }
@@ -206,7 +223,7 @@ k_fused_c2(FusedParams p, const float4 *__restrict__ Kt, const float *__restrict
     const int colw = has_col ? lane / 7 : 0, t = has_col ? lane % 7 : 0;
     const int l = 56 * (int)rank + 4 * warp + colw;                   // packed column 0..111
     const size_t qbase = (size_t)l * N + t;
-    c2 *const Zw = Z + (size_t)warp * ZW, *const zrow = Zw + lane * ZP;
+    c2 *const Zw = Z + (size_t)warp * ZW, *const zrow = Zw + (has_col ? lane : 0) * ZP;
     const bool warp_nyq = rank == 0 && warp == 0, nyq = warp_nyq && lane < 7;
     // ---- H-phase: lane -> output index k1 (each half-warp holds one of every pair {2k', 2k'+1} and 16 distinct k1 mod 16)
     const int hw = lane >> 4, q16 = lane & 15, k1 = q16 < 8 ? 2 * q16 + hw : 2 * q16 + 1 - hw;
@@ -233,9 +250,9 @@ k_fused_c2(FusedParams p, const float4 *__restrict__ Kt, const float *__restrict
     constexpr size_t KSTR = (size_t)2 * 8 * NT;                       // float4 per CTF in Kt: [c][rank][g 0..7][tid]
     const float4 *kt_t = Kt + (size_t)rank * 8 * NT + tid;
 
-    c2 q[32];
+    c2 q[16];
 #pragma unroll
-    for (int j = 0; j < 32; ++j) q[j] = make_float2(0.f, 0.f);
+    for (int j = 0; j < 16; ++j) q[j] = make_float2(0.f, 0.f);
     int o = o_begin, c = c_lo, o1 = o_begin, c1 = c_lo;               // (o, c) of step s; (o1, c1) of step s - 1
     unsigned b = 0, ph = 0, b1 = 0, ph1 = 0;                          // buffer s % NB and phase parity (s / NB) & 1 of steps s and s - 1
     for (int s = 0; s <= S; ++s) {
@@ -245,9 +262,15 @@ k_fused_c2(FusedParams p, const float4 *__restrict__ Kt, const float *__restrict
                 const cf *F0 = p.F0 + ((size_t)model * p.n_orient + o) * H;
                 if (has_col) {
 #pragma unroll
-                    for (int j = 0; j < 32; ++j) {
+                    for (int j = 0; j < 16; ++j) {
                         const cf pr = cmulc(Oimg[qbase + 7 * j], F0[qbase + 7 * j]);
                         q[j] = make_float2(pr.x, pr.y);
+                    }
+#pragma unroll
+                    for (int i = 0; i < 8; ++i) {
+                        const cf p0 = cmulc(Oimg[qbase + 7 * (16 + 2 * i)], F0[qbase + 7 * (16 + 2 * i)]);
+                        const cf p1 = cmulc(Oimg[qbase + 7 * (17 + 2 * i)], F0[qbase + 7 * (17 + 2 * i)]);
+                        Qs[(size_t)i * NT + tid] = make_float4(p0.x, p0.y, p1.x, p1.y);
                     }
                 }
                 if (nyq) {
@@ -261,8 +284,8 @@ k_fused_c2(FusedParams p, const float4 *__restrict__ Kt, const float *__restrict
             // ---- pass 1, F-phase (a4): 32-point transforms along m into the warp's tile
             __syncwarp();                                             // every lane has read the previous tile
             const float4 *kt = kt_t + (size_t)c * KSTR;
-            if (warp_nyq) c2_pass1_f<true>(q, kt, zrow, nyq, qn + t, KtN + (size_t)c * 224 + t);
-            else c2_pass1_f<false>(q, kt, zrow, false, nullptr, nullptr);
+            if (warp_nyq) c2_pass1_f<true>(q, Qs + tid, kt, zrow, has_col, nyq, qn + t, KtN + (size_t)c * 224 + t);
+            else c2_pass1_f<false>(q, Qs + tid, kt, zrow, has_col, false, nullptr, nullptr);
             __syncwarp();
             // ---- pass 1, H-phase: the 2D+1 needed outputs of each of the warp's 4 columns -> G_T of the owning CTA
             if (s >= NB) c2_wait(&bar_empty[b], ph ^ 1u);                    // both CTAs have read buffer b (step s - NB)
@@ -290,7 +313,7 @@ k_fused_c2(FusedParams p, const float4 *__restrict__ Kt, const float *__restrict
                 if (w2 == 0 && lane == 0) c2_expect_tx(&bar_full[b1], full_bytes);   // this phase: one arrival + every byte of the tile
                 c2_wait(&bar_full[b1], ph1);    // all 28 warps of the cluster have stored their part of buffer b1
                 __syncwarp();                                         // the H-phase reads of this warp's tile are done
-                c2_pass2_f(G + (size_t)b1 * GSZ + 2 * (pv ? pl : 0), t, bsel, zrow);
+                c2_pass2_f(G + (size_t)b1 * GSZ + 2 * (pv ? pl : 0), t, bsel, zrow, has_col);
                 __syncwarp();                                         // tile complete; every lane's G_T loads are in registers
                 if (lane == 0) { c2_arrive(empty_l + 8u * b1); c2_arrive(empty_p + 8u * b1); }
                 const size_t moc = ((size_t)model * p.n_orient + o1) * p.n_ctf + c1;
@@ -385,7 +408,7 @@ cudaError_t launch_relayout_K_c2(const float *K32, float *Kt, int n_ctf, cudaStr
 // Work items: one cluster (2 CTAs) per (image, model, chunk); partial results: 2 per work item (see the kernel's epilogue).
 cudaError_t launch_fused_c2(const FusedParams &p, const float *Kt, bool dump, cudaStream_t st)
 {
-    const size_t bytes = ((size_t)C2::NW * C2::ZW + C2::NB * C2::GSZ + 224) * 8 + (size_t)C2::NW * BIOEM_TOPK * sizeof(TopEntry) + 2 * C2::NW * 4 + 64;
+    const size_t bytes = ((size_t)C2::NW * C2::ZW + C2::NB * C2::GSZ + 16 * C2::NT + 224) * 8 + (size_t)C2::NW * BIOEM_TOPK * sizeof(TopEntry) + 2 * C2::NW * 4 + 64;
     const int P0 = (p.D + 2) / 2;                                     // rank 0 takes ceil(NP / 2) of the NP = D + 1 row pairs
     const float4 *kt = reinterpret_cast<const float4 *>(Kt);
     const float *ktn = c2_ktn(Kt, p.n_ctf);

@@ -269,6 +269,32 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+def run_sweep(args):
+    """Shapes of the paper's Fig. 4 (time against the number of images; linear above 128-256) and Fig. 2 (time against the
+    number of displacements; the Fourier route is almost flat) on the `small` grid with every 16th orientation.
+    One JSON line per point: device time of bioem_run (CUDA events inside the library), median of 3."""
+    import torch
+    from paper_1609_06634_b200 import BioEM
+    wl = build_inputs("small", 0, 16)
+    s = wl["spec"]
+    pts = ([("images", n, s.max_shift) for n in (1, 2, 4, 8, 16, 32, 64, 128, 256)] if args.sweep == "images"
+           else [("shifts", s.n_images, d) for d in (0, 1, 2, 4, 8, 12, 16)])
+    with BioEM(device=0) as b:
+        b.load_workload(wl)
+        for kind, n_img, D in pts:
+            b.set_shift_range(D)
+            b.push_images(wl["images"][:n_img])
+            ms = []
+            for _ in range(4):
+                b.run()
+                b.get_log_posterior()
+                ms.append(b.get_timing())
+            tot, fused = np.median([m[0] for m in ms[1:]]), np.median([m[1] for m in ms[1:]])
+            pairs = n_img * s.n_orient * s.n_ctf
+            print(json.dumps({"sweep": kind, "n_images": n_img, "max_shift": D, "n_shifts": (2 * D + 1) ** 2, "pairs": pairs,
+                              "run_ms": float(tot), "fused_ms": float(fused), "ns_per_pair": 1e6 * float(tot) / pairs}), flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -278,8 +304,11 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--orient-stride", type=int, default=1,
                     help="profiling aid: keep every k-th orientation of the grid (the workload name in the JSON line says so)")
+    ap.add_argument("--sweep", choices=["images", "shifts"], help="Fig. 4 / Fig. 2 shaped sweeps on one GPU (one JSON line per point)")
     args = ap.parse_args()
-    if args.impl == "reference":
+    if args.sweep:
+        run_sweep(args)
+    elif args.impl == "reference":
         run_reference(args)
     else:
         run_ours(args)

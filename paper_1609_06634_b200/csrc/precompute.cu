@@ -172,8 +172,10 @@ __global__ void __launch_bounds__(256) k_project(const double *xyz, const double
         const double yr = R[3] * x0 + R[4] * y0 + R[5] * z0;
         const double Ra = rad[a], R2 = Ra * Ra;
         const double dens = wt[a] / (4.0 / 3.0 * CUDART_PI * Ra * Ra * Ra) * h * h;
-        const int j0 = (int)floor((xr - Ra) / px + N / 2 - 0.5) - 1, j1 = (int)ceil((xr + Ra) / px + N / 2 + 0.5) + 1;
-        const int k0 = (int)floor((yr - Ra) / px + N / 2 - 0.5) - 1, k1 = (int)ceil((yr + Ra) / px + N / 2 + 0.5) + 1;
+        // pixel j covers [(j - N/2 - 1/2) px, (j - N/2 + 1/2) px]: it meets the disc iff A < j < B with A, B below; floor(A) and
+        // ceil(B) keep one spare pixel on either side against rounding (a pixel outside the disc adds exactly 0)
+        const int j0 = (int)floor((xr - Ra) / px + N / 2 - 0.5), j1 = (int)ceil((xr + Ra) / px + N / 2 + 0.5);
+        const int k0 = (int)floor((yr - Ra) / px + N / 2 - 0.5), k1 = (int)ceil((yr + Ra) / px + N / 2 + 0.5);
         for (int k = k0; k <= k1; ++k) {
             if (k < 0 || k >= N) continue;
             const double yc = (k - N / 2) * px - 0.5 * px - yr;

@@ -249,7 +249,7 @@ def run_ours(args):
             "hbm_alt": {"bytes_per_launch_if_streamed": hbm_bytes, "gbs_equivalent": hbm_bytes / (fused_ms * 1e-3) / 1e9,
                         "peak_gbs": peaks.get("hbm_gbs")},
         }
-        ni, no, nc = oracle_sample_shape(wl, 15.0)               # 10-30 s of oracle time
+        ni, no, nc = oracle_sample_shape(wl, 24.0)               # lands at 10-30 s of oracle time (the one-orientation probe overestimates)
         rate, dt, cores, sample = oracle_sample_rate(wl, ni, no, nc)
         line = {
             "metric": METRIC, "value": evals_job / t_dev, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,

@@ -20,7 +20,12 @@
 //   slot A   F(0)   a = Q K_c0                 ||  H'(group gi-2): B(dx,dy) -> a5 likelihood -> a6 log-sum-exp, candidates
 //   slot B   F(ci)  a = Q K_ci                 ||  H(ci-1): the 2D+1 pruned outputs per column -> rows of G[gi & 1]
 //   slot C   F'(group gi-1): rows of G[gi-1 & 1], Hermitian completion, two real rows per transform  ||  H(nc-1)
-//   one CTA barrier per group (G is double-buffered over groups; the Z tiles are warp-private).
+//   G is double-buffered over groups and the Z tiles are warp-private.  There is NO CTA barrier in the loop: two shared-memory
+//   mbarriers in split phase hand G over ("rows of group g written": arrive after the last G store, wait before F' reads them;
+//   "rows of group g read": arrive right after the F' loads, wait before the next store into that buffer), so warps drift.
+//   Pass-2 tasks (CTF in group, row pair) come from a host-built table (pk_build_map): conflict-free G row loads per
+//   half-warp, idle slots as whole warps (warp 0, which carries the Nyquist column, always; two more rotating over the
+//   schedulers from group to group).
 // The k = +16 output (D = 16 only) is the DC bin of the 16-point transforms: a twiddle and a shuffle-reduction over the
 // N2 lanes of a column.  The pipeline is primed and drained with masked groups (2 per work item, < 1 % of the work).
 //   a5  rho^2 = B^2 alpha_c^2 beta_w^2, g = cA log1p(-rho^2) + h_c (form C2; base-2 units inside the kernel)

@@ -256,3 +256,21 @@ def test_ensemble_posterior_eq10():
             rtot, rper = oracle.ensemble_log_posterior(ref, weights)
             assert np.abs(per - rper).max() <= TOL_LOGP and abs(tot - rtot) <= TOL_LOGP * len(per)
             assert abs(per.sum() - tot) <= 1e-9 * abs(tot)
+
+
+@pytest.mark.parametrize("name", ["small_mini", "paper_mini"])
+def test_affine_invariance_of_the_image(name):
+    """Property that holds at any size (SURVEY 8(c) pins, from the marginalisation over N and mu): replacing
+    I_obs by alpha I_obs + beta shifts every log-posterior by -(n-3) log|alpha| and leaves the argmax alone."""
+    wl = W.build_workload(name)
+    s = wl["spec"]
+    n = s.n_pix ** 2
+    a = _gpu_full(wl)
+    alpha, beta = 2.5, 7.0
+    wl2 = dict(wl)
+    wl2["images"] = (alpha * wl["images"].astype(np.float64) + beta).astype(np.float32)
+    b = _gpu_full(wl2)
+    # float32 storage of the transformed pixels perturbs them by 2^-24 relative: allow for it on top of the 1e-3 bar
+    assert np.abs(b["logp"] - (a["logp"] - (n - 3) * math.log(alpha))).max() <= 2e-3
+    for k in ("orient", "ctf", "dx", "dy"):
+        assert np.array_equal(a[k], b[k])

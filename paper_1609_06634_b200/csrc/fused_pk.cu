@@ -273,8 +273,7 @@ __global__ void __launch_bounds__(PK<N>::NT, 1) k_fused_pk(FusedParams p, const 
         {
             int cn = c0 + 1;
             if (cn >= c_hi) cn = c_lo;
-            PK_LOAD_A(cn)
-            PK_FFT_XS()
+            // H' first: it does not touch Q, so at a new orientation the Q loads issued above are in flight underneath it
             int h2e[NR];
 #pragma unroll
             for (int cp = 0; cp < NR; ++cp) h2e[cp] = map.e[var2][warp * CPW + 2 * cp + half];
@@ -306,6 +305,8 @@ __global__ void __launch_bounds__(PK<N>::NT, 1) k_fused_pk(FusedParams p, const 
                     pk_score<DUMP, 2>(p, st, mylist, y, v, sh, s2.x, s2.y, pair2 + (uint32_t)xcl);
                 }
             }
+            PK_LOAD_A(cn)
+            PK_FFT_XS()
             if (gi > 0) pk_mbar_wait(&mbar[1], (unsigned)(gi - 1) & 1u);   // every warp has read G[gi & 1] (F' of group gi-2): first write below
             if (xlane) Gw[(size_t)(KK - 1) * GP + col] = xs;
             PK_SPILL()

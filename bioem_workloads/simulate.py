@@ -11,6 +11,7 @@ same forward model as the oracle (so planted parameters are the best-scoring one
 from __future__ import annotations
 
 import math
+import os
 
 import numpy as np
 
@@ -112,17 +113,36 @@ def render_signal(model, q, ctf, N, px, cache=None):
     return np.fft.irfft2(spec0 * ctf_image(N, px, a, A, b), s=(N, N))
 
 
-def render_images(spec, models, quats, ctfs, truth):
+def _render_block(args):
+    spec, models, quats, ctfs, truth, lo, hi = args
     N, px = spec.n_pix, spec.pixel_A
-    I = len(truth["orient"])
-    out = np.empty((I, N, N), dtype=np.float32)
+    out = np.empty((hi - lo, N, N), dtype=np.float32)
     caches = [dict() for _ in models]
-    for i in range(I):
+    for i in range(lo, hi):
         mi = int(truth["model"][i])
         sig = render_signal(models[mi], quats[truth["orient"][i]], ctfs[truth["ctf"][i]], N, px, caches[mi])
         # I_obs(r) = N * I1(r + d) + mu + noise  (Eq. 7 with reading R4), circular (R5)
         sig = truth["N"][i] * np.roll(sig, shift=(-int(truth["dy"][i]), -int(truth["dx"][i])), axis=(0, 1))
         sd = sig.std()
         noise = np.random.default_rng(int(truth["noise_seed"][i])).normal(size=(N, N))
-        out[i] = (sig + truth["mu_frac"][i] * sd + noise * sd / math.sqrt(truth["snr"][i])).astype(np.float32)
+        out[i - lo] = (sig + truth["mu_frac"][i] * sd + noise * sd / math.sqrt(truth["snr"][i])).astype(np.float32)
     return out
+
+
+def render_images(spec, models, quats, ctfs, truth, workers=None):
+    """Every image is rendered from its own parameters and its own noise seed, so the stack can be rendered in blocks by
+    worker processes (spawned, not forked: the caller may hold a CUDA context) with a result identical to the serial loop."""
+    I = len(truth["orient"])
+    if workers is None:
+        workers = min(os.cpu_count() or 1, 32, I // 32)
+    if workers <= 1:
+        return _render_block((spec, models, quats, ctfs, truth, 0, I))
+    import multiprocessing as mp
+    from concurrent.futures import ProcessPoolExecutor
+    # only the models that generate images travel to the workers (a density map is 8 MB, an atom model a few hundred KB)
+    used = sorted(set(int(m) for m in truth["model"]))
+    slim = [models[m] if m in used else None for m in range(len(models))]
+    edges = np.linspace(0, I, 4 * workers + 1).astype(int)
+    jobs = [(spec, slim, quats, ctfs, truth, int(a), int(b)) for a, b in zip(edges[:-1], edges[1:]) if b > a]
+    with ProcessPoolExecutor(max_workers=workers, mp_context=mp.get_context("spawn")) as ex:
+        return np.concatenate(list(ex.map(_render_block, jobs)), axis=0)

@@ -77,13 +77,23 @@ int bioem_ctf_from_defocus(float defocus_um, float bfactor_A2, float kV, float *
 int bioem_set_shift_range(bioem_ctx *ctx, int max_shift_px);
 
 /* Replace the image stack: n_img images [n][N][N] float32 (host, or device if is_device). Runs the
- * observed-image preprocessing (a0: mean removal, spectra, C_o / C_oo sums). */
+ * observed-image preprocessing (a0: mean removal, spectra, C_o / C_oo sums).
+ * BIOEM_EBADARG if an image is constant or not finite (C_oo - C_o^2/n is not > 0: the marginal over
+ * N, mu, lambda of Eq. 8 does not exist for it); the stack is then left empty. */
 int bioem_push_images(bioem_ctx *ctx, int n_img, const float *pixels, int is_device);
 
 /* The hot path: all models x orientations x CTFs x shifts against all images (Eq. 9 on the grid,
  * P:126; Eqs. 11-12; closed-form marginal over N, mu, lambda).  Requires geometry,
  * >= 1 model, orientations, CTFs, a shift range and images (else BIOEM_EBADSTATE). */
 int bioem_run(bioem_ctx *ctx);
+/* Domain of validity.  bioem_run only enqueues; a calculated image that is empty or not finite (T_c = n C_cc - C_c^2 is
+ * not > 0: the model projects to nothing inside the box) is detected on the device and reported as BIOEM_EBADARG by the first
+ * bioem_get_* call.  The hot loop is FP32 on operands correctly rounded from FP64; the BIOEM_TOPK largest terms per
+ * (image, model) are re-scored in FP64 and the argmax is taken among them.  The 1e-3 absolute accuracy of log_posterior
+ * therefore holds when the terms outside the BIOEM_TOPK largest carry a small share of the sum, or carry a small FP32 error:
+ * |delta log P| <~ (share of the sum outside the top BIOEM_TOPK) x n rho^2 / (1 - rho^2) x 1e-6, rho^2 = the squared
+ * correlation of the best match.  rho^2 -> 1 (a noiseless planted image, R14) is clamped at
+ * 1 - rho^2 >= 2^-24 in the FP32 loop and 1e-300 in the re-scoring: finite results, parity with the oracle not defined. */
 
 /* Results of the last bioem_run, each [n_img][n_model] (image-major):
  *   log_posterior = log sum_theta w(theta) P_m,omega(theta), w uniform unless priors were given (R7);
@@ -109,7 +119,21 @@ int bioem_get_orientation_log_posterior(bioem_ctx *ctx, double *out);
  * inner log-sums) or NULL.  FP64, fixed summation order. */
 int bioem_get_ensemble_log_posterior(bioem_ctx *ctx, const double *weights, double *out_total, double *out_per_image);
 
+/* Work decomposition of bioem_run: one work item (thread block) scores one image against `n_orient_per_item` consecutive
+ * orientations x all CTFs x all shifts of one model (the image-stationary loop order of DESIGN.md section 8; P:199-203 has
+ * the loops the other way round).  0 = automatic: >= 32 work items per SM, at most 32 orientations per item.  The value
+ * fixes the order in which the FP32 partial sums are combined, so results are bit-identical between two runs only if it is
+ * the same; ranks that shard one image stack set it explicitly.  Ignored (1) while the per-orientation
+ * posterior is enabled. */
+int bioem_set_orientation_chunk(bioem_ctx *ctx, int n_orient_per_item);
+
 /* ---- test / debug entry points (not on the measured path) ---- */
+/* Which fused kernel bioem_run may use: 0 automatic (packed register-resident kernel for n_pix 64 / 128 with max_shift <= 16,
+ * tensor-memory kernel for n_pix 224 with max_shift <= 31, generic kernel otherwise), 1 generic kernel always, 3 the
+ * two-CTA-cluster kernel of round 1 (n_pix 224, max_shift <= 31; kept as a cross-check of the tensor-memory kernel). */
+int bioem_debug_set_kernel(bioem_ctx *ctx, int which);
+/* The plan of the last bioem_run: kernel (1 generic, 2 packed, 3 cluster, 4 tensor memory) and orientations per work item. */
+int bioem_get_run_plan(bioem_ctx *ctx, int *kernel, int *n_orient_per_item);
 /* real-space calculated image I1 of (model, orient, ctf) [N][N] ("synthetic map"). */
 int bioem_debug_calc_image(bioem_ctx *ctx, int model, int orient, int ctf, float *out_real);
 /* per-shift terms log P + log w of one (image, calc image) pair, [dy+D][dx+D]:

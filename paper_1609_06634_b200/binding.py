@@ -17,7 +17,9 @@ EXPORTED_SYMBOLS = [
     "bioem_get_best", "bioem_debug_calc_image", "bioem_debug_shift_map", "bioem_debug_shift_map_f64",
     "bioem_debug_log_posterior_f32", "bioem_get_timing", "bioem_get_launch_count", "bioem_measure_fp32_peak",
     "bioem_set_orientation_posterior", "bioem_get_orientation_log_posterior", "bioem_get_ensemble_log_posterior",
+    "bioem_set_orientation_chunk", "bioem_debug_set_kernel", "bioem_get_run_plan",
 ]
+KERNEL_AUTO, KERNEL_GENERIC, KERNEL_PK, KERNEL_C2, KERNEL_TM = 0, 1, 2, 3, 4
 
 _fp = C.POINTER(C.c_float)
 _dp = C.POINTER(C.c_double)
@@ -66,6 +68,9 @@ def lib():
         L.bioem_get_timing.argtypes = [C.c_void_p, _dp, _dp]
         L.bioem_get_launch_count.argtypes = [C.c_void_p, C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
         L.bioem_measure_fp32_peak.argtypes = [C.c_void_p, _dp, _dp]
+        L.bioem_set_orientation_chunk.argtypes = [C.c_void_p, C.c_int]
+        L.bioem_debug_set_kernel.argtypes = [C.c_void_p, C.c_int]
+        L.bioem_get_run_plan.argtypes = [C.c_void_p, C.POINTER(C.c_int), C.POINTER(C.c_int)]
         for name in EXPORTED_SYMBOLS:
             if name != "bioem_last_error":
                 getattr(L, name).restype = C.c_int
@@ -200,6 +205,18 @@ class BioEM:
         self._ck(self._L.bioem_get_best(self._h, o.ctypes.data_as(_ip), c.ctypes.data_as(_ip), dx.ctypes.data_as(_ip),
                                         dy.ctypes.data_as(_ip), lp.ctypes.data_as(_dp)))
         return dict(orient=o, ctf=c, dx=dx, dy=dy, log_p=lp)
+
+    def set_orientation_chunk(self, n_orient_per_item=0):
+        self._ck(self._L.bioem_set_orientation_chunk(self._h, int(n_orient_per_item)))
+
+    def debug_set_kernel(self, which=KERNEL_AUTO):
+        self._ck(self._L.bioem_debug_set_kernel(self._h, int(which)))
+
+    def get_run_plan(self):
+        """(kernel, orientations per work item) of the last run."""
+        k, oc = C.c_int(), C.c_int()
+        self._ck(self._L.bioem_get_run_plan(self._h, C.byref(k), C.byref(oc)))
+        return k.value, oc.value
 
     def set_orientation_posterior(self, enable=True):
         self._ck(self._L.bioem_set_orientation_posterior(self._h, int(bool(enable))))

@@ -59,12 +59,18 @@ struct bioem_ctx {
     // run state
     bool ran = false;
     bool want_orient = false, ran_orient = false;      // per-orientation posterior: requested / produced by the last run
+    int oc_user = 0;                                   // orientations per work item (0 = automatic)
+    int kernel_user = 0;                               // BIOEM_KERNEL_*: which fused kernel bioem_run may pick (0 = automatic)
+    int n_sm = 148;
+    DBuf flags;                                        // int[1]: bit 0 = an image without variance, bit 1 = an empty calculated image
+    int run_kernel = 0, run_oc = 0;
+    bool flags_checked = true;
     DBuf logp_orient;
     int run_models = 0, run_orient = 0, run_ctf = 0, run_D = 0, run_img = 0;
     DBuf F064, F032, K64, K32, Kt, Tc64, h64, alpha32, h32;
     DBuf part_m, part_s, part_top, m32, s32, top, g64;
     DBuf logp, logp32, best, best_logp;
-    DBuf scratch_a, scratch_b, scratch_c, dump;
+    DBuf scratch_a, scratch_b, scratch_c, dump, staging;
     cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
     int64_t launches = 0, fused_launches = 0, push_launches = 0;
 };
@@ -101,6 +107,13 @@ int bioem_create(bioem_ctx **out, int device, void *cuda_stream)
     ctx->stream = reinterpret_cast<cudaStream_t>(cuda_stream);
     for (int i = 0; i < 4; ++i)
         if (cudaEventCreate(&ctx->ev[i]) != cudaSuccess) { delete ctx; return BIOEM_ECUDA; }
+    if (cudaDeviceGetAttribute(&ctx->n_sm, cudaDevAttrMultiProcessorCount, device) != cudaSuccess || ctx->n_sm < 1) ctx->n_sm = 148;
+    if (ctx->flags.ensure(sizeof(int)) != cudaSuccess || cudaMemset(ctx->flags.p, 0, sizeof(int)) != cudaSuccess) {
+        cudaGetLastError();
+        for (int i = 0; i < 4; ++i) cudaEventDestroy(ctx->ev[i]);
+        delete ctx;
+        return BIOEM_ECUDA;
+    }
     *out = ctx;
     return BIOEM_OK;
 }
@@ -114,7 +127,7 @@ int bioem_destroy(bioem_ctx *ctx)
     DBuf *all[] = {&ctx->rot, &ctx->lp_orient, &ctx->ctf_a, &ctx->ctf_A, &ctx->ctf_b, &ctx->lp_ctf, &ctx->Ohat64, &ctx->Ohat32, &ctx->Dw,
                    &ctx->beta, &ctx->F064, &ctx->F032, &ctx->K64, &ctx->K32, &ctx->Kt, &ctx->Tc64, &ctx->h64, &ctx->alpha32, &ctx->h32,
                    &ctx->part_m, &ctx->part_s, &ctx->part_top, &ctx->m32, &ctx->s32, &ctx->top, &ctx->g64, &ctx->logp, &ctx->logp_orient, &ctx->logp32,
-                   &ctx->best, &ctx->best_logp, &ctx->scratch_a, &ctx->scratch_b, &ctx->scratch_c, &ctx->dump};
+                   &ctx->best, &ctx->best_logp, &ctx->scratch_a, &ctx->scratch_b, &ctx->scratch_c, &ctx->dump, &ctx->flags, &ctx->staging};
     for (DBuf *b : all) b->release();
     for (int i = 0; i < 4; ++i) if (ctx->ev[i]) cudaEventDestroy(ctx->ev[i]);
     delete ctx;
@@ -287,39 +300,55 @@ int bioem_push_images(bioem_ctx *ctx, int n_img, const float *pixels, int is_dev
     CK(ctx->beta.ensure((size_t)n_img * sizeof(float)));
     CK(ctx->scratch_a.ensure((size_t)slab * n * sizeof(double)));       // centred images
     CK(ctx->scratch_b.ensure((size_t)slab * H * sizeof(cd)));           // transform intermediate
-    DBuf staging;
     const float *dsrc = pixels;
     if (!is_device) {
-        cudaError_t e = staging.ensure((size_t)n_img * n * sizeof(float));
-        if (e == cudaSuccess) e = cudaMemcpyAsync(staging.p, pixels, (size_t)n_img * n * sizeof(float), cudaMemcpyHostToDevice, st);
-        if (e != cudaSuccess) { staging.release(); CK(e); }
-        dsrc = staging.as<float>();
+        // grow-only staging buffer owned by the context: no cudaMalloc / cudaFree (both synchronise the device) per call
+        CK(ctx->staging.ensure((size_t)n_img * n * sizeof(float)));
+        CK(cudaMemcpyAsync(ctx->staging.p, pixels, (size_t)n_img * n * sizeof(float), cudaMemcpyHostToDevice, st));
+        dsrc = ctx->staging.as<float>();
     }
-    cudaError_t e = cudaSuccess;
-    for (int i0 = 0; i0 < n_img && e == cudaSuccess; i0 += slab) {
+    CK(cudaMemsetAsync(ctx->flags.p, 0, sizeof(int), st));
+    for (int i0 = 0; i0 < n_img; i0 += slab) {
         const int nb = std::min(slab, n_img - i0);
-        e = launch_image_stats(dsrc + (size_t)i0 * n, nb, N, ctx->scratch_a.as<double>(), ctx->Dw.as<double>() + i0, st);
-        if (e == cudaSuccess) e = launch_fft2_r2c_f64(ctx->scratch_a.as<double>(), nb, N, ctx->scratch_b.as<cd>(), ctx->Ohat64.as<cd>() + (size_t)i0 * H, st);
-        if (e == cudaSuccess) e = launch_zero_dc(ctx->Ohat64.as<cd>() + (size_t)i0 * H, nb, H, st);
+        CK(launch_image_stats(dsrc + (size_t)i0 * n, nb, N, ctx->scratch_a.as<double>(), ctx->Dw.as<double>() + i0, st));
+        CK(launch_fft2_r2c_f64(ctx->scratch_a.as<double>(), nb, N, ctx->scratch_b.as<cd>(), ctx->Ohat64.as<cd>() + (size_t)i0 * H, st));
+        CK(launch_zero_dc(ctx->Ohat64.as<cd>() + (size_t)i0 * H, nb, H, st));
     }
-    if (e == cudaSuccess) e = launch_cast_spectrum(ctx->Ohat64.as<cd>(), ctx->Ohat32.as<cf>(), (size_t)n_img * H, st);
-    if (e == cudaSuccess) e = launch_beta(ctx->Dw.as<double>(), n_img, ctx->beta.as<float>(), st);
-    if (e == cudaSuccess) e = cudaStreamSynchronize(st);      // inputs are copied: safe to free after return
-    staging.release();
-    CK(e);
+    CK(launch_cast_spectrum(ctx->Ohat64.as<cd>(), ctx->Ohat32.as<cf>(), (size_t)n_img * H, st));
+    CK(launch_beta(ctx->Dw.as<double>(), n_img, ctx->beta.as<float>(), ctx->flags.as<int>(), st));
+    int fl = 0;
+    CK(cudaMemcpyAsync(&fl, ctx->flags.p, sizeof(int), cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));                            // inputs are copied: the caller may free `pixels` after return
+    if (fl & 1) {
+        ctx->n_img = 0;
+        FAIL(BIOEM_EBADARG, "push_images: an image is constant or not finite (sum of squared deviations from its mean is not > 0): its posterior is undefined");
+    }
     ctx->push_launches = 4 * (int64_t)((n_img + slab - 1) / slab) + 2;
     ctx->n_img = n_img;
     ctx->ran = false;
     return BIOEM_OK;
 }
 
-static int choose_oc(long long n_img, long long n_model, long long n_orient)
+// Orientations per work item: aim at >= 32 work items per SM, at most 32 orientations per item.
+static int choose_oc(long long n_img, long long n_model, long long n_orient, int n_sm)
 {
-    long long oc = n_img * n_model * n_orient / 4736;      // aim at >= 32 work items per SM
+    long long oc = n_img * n_model * n_orient / (32LL * n_sm);
     if (oc < 1) oc = 1;
     if (oc > 32) oc = 32;
     if (oc > n_orient) oc = n_orient;
     return (int)oc;
+}
+
+enum { KERNEL_AUTO = 0, KERNEL_GENERIC = 1, KERNEL_PK = 2, KERNEL_C2 = 3, KERNEL_TM = 4 };
+
+// the fused kernel a run of (N, D) uses: the one asked for if it supports the shape, else the automatic choice
+static int choose_kernel(int N, int D, int user)
+{
+    if (user == KERNEL_GENERIC) return KERNEL_GENERIC;
+    if (user == KERNEL_C2 && c2_supported(N, D)) return KERNEL_C2;
+    if (pk_supported(N, D)) return KERNEL_PK;
+    if (tm_supported(N, D)) return KERNEL_TM;
+    return KERNEL_GENERIC;
 }
 
 int bioem_run(bioem_ctx *ctx)
@@ -353,8 +382,11 @@ int bioem_run(bioem_ctx *ctx)
     CK(ctx->h64.ensure(MOC * sizeof(double)));
     CK(ctx->alpha32.ensure(MOC * sizeof(float)));
     CK(ctx->h32.ensure(MOC * sizeof(float)));
-    const bool use_pk = pk_supported(N, D), use_c2 = !use_pk && c2_supported(N, D);
-    const int oc = ctx->want_orient ? 1 : choose_oc(I, M, O), cpm = (O + oc - 1) / oc;     // one orientation per work item when its posterior is wanted
+    const int kern = choose_kernel(N, D, ctx->kernel_user);
+    const bool use_pk = kern == KERNEL_PK, use_c2 = kern == KERNEL_C2, use_tm = kern == KERNEL_TM;
+    int oc = ctx->oc_user > 0 ? std::min(ctx->oc_user, O) : choose_oc(I, M, O, ctx->n_sm);
+    if (ctx->want_orient) oc = 1;                                         // one orientation per work item when its posterior is wanted
+    const int cpm = (O + oc - 1) / oc;
     const int ppi = use_c2 ? 2 : 1;                                       // partials per work item (the cluster kernel writes one per CTA)
     const size_t items = (size_t)I * M * cpm * ppi, IM = (size_t)I * M;
     CK(ctx->part_m.ensure(items * sizeof(float)));
@@ -370,6 +402,7 @@ int bioem_run(bioem_ctx *ctx)
     CK(ctx->best_logp.ensure(IM * sizeof(double)));
 
     CK(cudaEventRecord(ctx->ev[0], st));
+    CK(cudaMemsetAsync(ctx->flags.p, 0, sizeof(int), st));
 
     // ---- a3: CTF tables
     CK(launch_ctf_tables(ctx->ctf_a.as<double>(), ctx->ctf_A.as<double>(), ctx->ctf_b.as<double>(), C, N, ctx->px, ctx->K64.as<double>(),
@@ -382,6 +415,10 @@ int bioem_run(bioem_ctx *ctx)
     } else if (use_c2) {
         CK(ctx->Kt.ensure(c2_kt_bytes(C)));
         CK(launch_relayout_K_c2(ctx->K32.as<float>(), ctx->Kt.as<float>(), C, st));
+        ctx->launches += 1;
+    } else if (use_tm) {
+        CK(ctx->Kt.ensure(tm_kt_bytes(C)));
+        CK(launch_relayout_K_tm(ctx->K32.as<float>(), ctx->Kt.as<float>(), C, st));
         ctx->launches += 1;
     }
 
@@ -417,7 +454,7 @@ int bioem_run(bioem_ctx *ctx)
     CK(launch_cast_spectrum(ctx->F064.as<cd>(), ctx->F032.as<cf>(), MO * H, st));
     CK(launch_calc_stats(ctx->F064.as<cd>(), ctx->K64.as<double>(), (int)MO, O, C, N, ctx->has_lp_orient ? ctx->lp_orient.as<double>() : nullptr,
                          ctx->has_lp_ctf ? ctx->lp_ctf.as<double>() : nullptr, std::log((double)(2 * D + 1) * (2 * D + 1)),
-                         ctx->Tc64.as<double>(), ctx->h64.as<double>(), ctx->alpha32.as<float>(), ctx->h32.as<float>(), st));
+                         ctx->Tc64.as<double>(), ctx->h64.as<double>(), ctx->alpha32.as<float>(), ctx->h32.as<float>(), ctx->flags.as<int>(), st));
     ctx->launches += 2;
 
     // ---- a4-a6: the fused kernel
@@ -431,6 +468,7 @@ int bioem_run(bioem_ctx *ctx)
     int nl = 1;
     if (use_pk) CK(launch_fused_pk(N, p, ctx->Kt.as<float>(), false, st));
     else if (use_c2) CK(launch_fused_c2(p, ctx->Kt.as<float>(), false, st));
+    else if (use_tm) CK(launch_fused_tm(p, ctx->Kt.as<float>(), false, st));
     else CK(launch_fused(N, p, false, st, &nl));
     CK(cudaEventRecord(ctx->ev[2], st));
     ctx->launches += nl; ctx->fused_launches += nl;
@@ -454,13 +492,32 @@ int bioem_run(bioem_ctx *ctx)
     }
     CK(cudaEventRecord(ctx->ev[3], st));
     ctx->ran = true;
+    ctx->flags_checked = false;
+    ctx->run_kernel = kern; ctx->run_oc = oc;
     ctx->run_models = M; ctx->run_orient = O; ctx->run_ctf = C; ctx->run_D = D; ctx->run_img = I;
+    return BIOEM_OK;
+}
+
+// bioem_run only enqueues: a degenerate calculated image (T_c = 0: the model projects to nothing inside the box, or the CTF
+// table is all zero) is seen by the device and reported by the first call that synchronises.
+static int check_run_flags(bioem_ctx *ctx)
+{
+    if (ctx->flags_checked) return BIOEM_OK;
+    int fl = 0;
+    CK(cudaMemcpyAsync(&fl, ctx->flags.p, sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
+    CK(cudaStreamSynchronize(ctx->stream));
+    if (fl & 2) {
+        ctx->ran = false;
+        FAIL(BIOEM_EBADARG, "run: a calculated image is empty or not finite (T_c = sum |I1|^2 is not > 0): its posterior is undefined");
+    }
+    ctx->flags_checked = true;
     return BIOEM_OK;
 }
 
 static int fetch(bioem_ctx *ctx, void *dst, const void *src, size_t bytes)
 {
     CK(cudaSetDevice(ctx->device));
+    if (ctx->ran) { int rc = check_run_flags(ctx); if (rc) return rc; }
     CK(cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToHost, ctx->stream));
     CK(cudaStreamSynchronize(ctx->stream));
     return BIOEM_OK;
@@ -582,8 +639,9 @@ int bioem_debug_shift_map(bioem_ctx *ctx, int img, int model, int orient, int ct
     p.chunks_per_model = 1;
     p.cA = (float)(-0.5 * ((double)n - 3.0) * 1.4426950408889634);
     p.dump = ctx->dump.as<float>(); p.dump_img = img; p.dump_model = model; p.dump_orient = orient; p.dump_ctf = ctf;
-    if (pk_supported(N, D)) CK(launch_fused_pk(N, p, ctx->Kt.as<float>(), true, ctx->stream));
-    else if (c2_supported(N, D)) CK(launch_fused_c2(p, ctx->Kt.as<float>(), true, ctx->stream));
+    if (ctx->run_kernel == KERNEL_PK) CK(launch_fused_pk(N, p, ctx->Kt.as<float>(), true, ctx->stream));
+    else if (ctx->run_kernel == KERNEL_C2) CK(launch_fused_c2(p, ctx->Kt.as<float>(), true, ctx->stream));
+    else if (ctx->run_kernel == KERNEL_TM) CK(launch_fused_tm(p, ctx->Kt.as<float>(), true, ctx->stream));
     else CK(launch_fused(N, p, true, ctx->stream, nullptr));
     std::vector<float> tmp((size_t)KK * KK);
     rc = fetch(ctx, tmp.data(), ctx->dump.p, tmp.size() * sizeof(float));
@@ -627,6 +685,31 @@ int bioem_debug_shift_map_f64(bioem_ctx *ctx, int img, int model, int orient, in
     const double base = -0.5 * (nn - 2.0) * std::log(2.0 * M_PI) + 0.5 * (nn - 5.0) * std::log(2.0) + std::lgamma(0.5 * (nn - 3.0)) -
                         0.5 * (nn - 3.0) * std::log(dw[0]);
     for (int s = 0; s < S; ++s) out[s] = base + g[s];
+    return BIOEM_OK;
+}
+
+int bioem_set_orientation_chunk(bioem_ctx *ctx, int n_orient_per_item)
+{
+    if (!ctx) return BIOEM_EBADARG;
+    if (n_orient_per_item < 0) FAIL(BIOEM_EBADARG, "set_orientation_chunk: negative");
+    ctx->oc_user = n_orient_per_item;
+    return BIOEM_OK;
+}
+
+int bioem_debug_set_kernel(bioem_ctx *ctx, int which)
+{
+    if (!ctx) return BIOEM_EBADARG;
+    if (which != KERNEL_AUTO && which != KERNEL_GENERIC && which != KERNEL_C2) FAIL(BIOEM_EBADARG, "debug_set_kernel: 0 (automatic), 1 (generic) or 3 (two-CTA cluster, n_pix = 224)");
+    ctx->kernel_user = which;
+    return BIOEM_OK;
+}
+
+int bioem_get_run_plan(bioem_ctx *ctx, int *kernel, int *n_orient_per_item)
+{
+    if (!ctx) return BIOEM_EBADARG;
+    if (!ctx->ran) FAIL(BIOEM_EBADSTATE, "get_run_plan: no completed run");
+    if (kernel) *kernel = ctx->run_kernel;
+    if (n_orient_per_item) *n_orient_per_item = ctx->run_oc;
     return BIOEM_OK;
 }
 

@@ -60,6 +60,12 @@ size_t c2_kt_bytes(int n_ctf);
 cudaError_t launch_relayout_K_c2(const float *K32, float *Kt, int n_ctf, cudaStream_t st);
 cudaError_t launch_fused_c2(const FusedParams &p, const float *Kt, bool dump, cudaStream_t st);
 
+// tensor-memory variant (N = 224; D <= 31): Q resident in TMEM, one CTA per work item, one partial per work item
+bool tm_supported(int N, int D);
+size_t tm_kt_bytes(int n_ctf);
+cudaError_t launch_relayout_K_tm(const float *K32, float *Kt, int n_ctf, cudaStream_t st);
+cudaError_t launch_fused_tm(const FusedParams &p, const float *Kt, bool dump, cudaStream_t st);
+
 // precompute
 cudaError_t launch_image_stats(const float *img, int n_img, int N, double *centered, double *Dw, cudaStream_t st);
 cudaError_t launch_fft2_r2c_f64(const double *in, int batch, int N, cd *tmp, cd *out, cudaStream_t st);   // out [b][l][m]
@@ -73,8 +79,8 @@ cudaError_t launch_ctf_tables(const double *a, const double *A, const double *b,
                               double *K64, float *K32, cudaStream_t st);
 cudaError_t launch_calc_stats(const cd *F0, const double *K64, int n_mo, int n_orient, int n_ctf, int N,
                               const double *lp_orient, const double *lp_ctf, double log_shifts,
-                              double *Tc64, double *h64, float *alpha32, float *h32, cudaStream_t st);
-cudaError_t launch_beta(const double *Dw, int n_img, float *beta, cudaStream_t st);
+                              double *Tc64, double *h64, float *alpha32, float *h32, int *flags, cudaStream_t st);
+cudaError_t launch_beta(const double *Dw, int n_img, float *beta, int *flags, cudaStream_t st);
 
 // finalise
 cudaError_t launch_merge(const float *part_m, const float *part_s, const TopEntry *part_top, int n_img, int n_model,

@@ -98,9 +98,11 @@ __global__ void __launch_bounds__(256) k_rescore(const cd *Ohat, const cd *F0, c
         const size_t moc = ((size_t)model * n_orient + o) * n_ctf + c;
         const double n = (double)N * N;
         const double B = sh[0];
-        double rho2 = B * B / (n * Tc64[moc] * Dw[img]);
-        if (rho2 > 1.0 - 1e-300) rho2 = 1.0 - 1e-300;                               // R14
-        g64[ci] = -0.5 * (n - 3.0) * log1p(-rho2) + h64[moc];
+        const double rho2 = B * B / (n * Tc64[moc] * Dw[img]);
+        // R14 (DESIGN 3): 1 - rho^2 >= 1e-300 (1.0 - 1e-300 == 1.0 in double, so the clamp has to sit on
+        // the difference: a noiseless planted image then gives a large finite term instead of +inf)
+        const double g = rho2 < 0.5 ? log1p(-rho2) : log(fmax(1.0 - rho2, 1e-300));
+        g64[ci] = -0.5 * (n - 3.0) * g + h64[moc];
     }
 }
 

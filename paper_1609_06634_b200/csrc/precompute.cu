@@ -46,14 +46,18 @@ cudaError_t launch_image_stats(const float *img, int n_img, int N, double *cente
     return cudaGetLastError();
 }
 
-__global__ void k_beta(const double *Dw, int n, float *beta)
+// flags[0] |= 1 when an image has no variance (D_omega = sum o^2 <= 0, or not finite): rho^2 = B^2 / (A D) is undefined for it
+__global__ void k_beta(const double *Dw, int n, float *beta, int *flags)
 {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < n) beta[i] = (float)(1.0 / sqrt(Dw[i]));
+    if (i >= n) return;
+    const double d = Dw[i];
+    if (!(d > 0.0) || isinf(d)) atomicOr(flags, 1);
+    beta[i] = (float)(1.0 / sqrt(d));
 }
-cudaError_t launch_beta(const double *Dw, int n_img, float *beta, cudaStream_t st)
+cudaError_t launch_beta(const double *Dw, int n_img, float *beta, int *flags, cudaStream_t st)
 {
-    k_beta<<<(n_img + 255) / 256, 256, 0, st>>>(Dw, n_img, beta);
+    k_beta<<<(n_img + 255) / 256, 256, 0, st>>>(Dw, n_img, beta, flags);
     return cudaGetLastError();
 }
 
@@ -336,7 +340,7 @@ cudaError_t launch_ctf_tables(const double *a, const double *A, const double *b,
 // columns l = 0 and l = N/2 count once, the others twice.  One CTA per (model, orientation), loop over CTFs.
 __global__ void __launch_bounds__(256) k_calc_stats(const cd *F0, const double *K64, int n_orient, int n_ctf, int N, const double *lp_orient,
                                                     const double *lp_ctf, double log_shifts, double *Tc64, double *h64, float *alpha32,
-                                                    float *h32)
+                                                    float *h32, int *flags)
 {
     __shared__ double sh[256];
     const int NC = N / 2 + 1, H = NC * N;
@@ -359,6 +363,7 @@ __global__ void __launch_bounds__(256) k_calc_stats(const cd *F0, const double *
             const double lpo = lp_orient ? lp_orient[o] : -log((double)n_orient);
             const double lpc = lp_ctf ? lp_ctf[c] : -log((double)n_ctf);
             const double h = -0.5 * log(s) + lpo + lpc - log_shifts;
+            if (!(s > 0.0) || isinf(s)) atomicOr(flags, 2);          // empty calculated image: T_c = 0, rho^2 undefined
             Tc64[moc] = s; h64[moc] = h;
             alpha32[moc] = (float)(1.0 / sqrt(n * s)); h32[moc] = (float)(h * 1.4426950408889634);   // FP32 path: base-2 units
         }
@@ -367,9 +372,9 @@ __global__ void __launch_bounds__(256) k_calc_stats(const cd *F0, const double *
 
 cudaError_t launch_calc_stats(const cd *F0, const double *K64, int n_mo, int n_orient, int n_ctf, int N, const double *lp_orient,
                               const double *lp_ctf, double log_shifts, double *Tc64, double *h64, float *alpha32, float *h32,
-                              cudaStream_t st)
+                              int *flags, cudaStream_t st)
 {
-    k_calc_stats<<<n_mo, 256, 0, st>>>(F0, K64, n_orient, n_ctf, N, lp_orient, lp_ctf, log_shifts, Tc64, h64, alpha32, h32);
+    k_calc_stats<<<n_mo, 256, 0, st>>>(F0, K64, n_orient, n_ctf, N, lp_orient, lp_ctf, log_shifts, Tc64, h64, alpha32, h32, flags);
     return cudaGetLastError();
 }
 

@@ -31,7 +31,7 @@ def stale() -> bool:
 def build(force: bool = False, verbose: bool = False) -> Path:
     if not force and not stale():
         return LIB
-    flags = list(NVCC_FLAGS)
+    flags = list(NVCC_FLAGS) + os.environ.get("BIOEM_NVCC_EXTRA", "").split()      # e.g. -DNAME for an experiment build
     objs = []
     bdir = HERE / "build"
     bdir.mkdir(exist_ok=True)

@@ -109,6 +109,18 @@ CONFIGS["ensemble_mini"] = replace(_ENSEMBLE, name="ensemble_mini", n_images=6, 
 CONFIGS["tiny_mini"] = replace(_TINY, name="tiny_mini", n_images=5, orient_stride=13)
 
 
+# "mid" variants: >= 40 orientations and >= 7 CTFs (three CTF groups of the packed kernel, an orientation change in the middle
+# of a work item's software pipeline), still seconds for the direct-summation oracle: the element-by-element parity cases of
+# the chunked launch (orientations per work item 1, 2, 5, 32).
+CONFIGS["tiny_mid"] = replace(_TINY, name="tiny_mid", n_images=6, defocus_um=(1.0, 1.5, 2.0, 2.5))
+CONFIGS["small_mid"] = replace(_SMALL, name="small_mid", n_images=5, orient_stride=107,
+                               bfactor_A2=(0.0, 150.0), amp_contrast=(0.1,))
+CONFIGS["paper_mid"] = replace(_PAPER, name="paper_mid", n_images=3, orient_stride=97,
+                               defocus_um=_lin(0.5, 3.0, 7), bfactor_A2=(50.0,))
+CONFIGS["ensemble_mid"] = replace(_ENSEMBLE, name="ensemble_mid", n_images=4, n_models=3, n_source_models=2,
+                                  orient_stride=28, defocus_um=_lin(0.5, 3.0, 4), bfactor_A2=(0.0, 100.0))
+
+
 def get_spec(name: str, **overrides) -> WorkloadSpec:
     spec = CONFIGS[name]
     return replace(spec, **overrides) if overrides else spec

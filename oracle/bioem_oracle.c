@@ -439,6 +439,7 @@ typedef struct {
 
 static void bo_acc_add(bo_acc *a, double x, long long flat)
 {
+    if (x == -INFINITY) return;     /* a grid point of weight zero (log-prior -inf, R7) adds nothing to the sum of Eq. 9 */
     if (x > a->m) { a->s = a->s * exp(a->m - x) + 1.0; a->m = x; }
     else a->s += exp(x - a->m);
     if (x > a->best) { a->second = a->best; a->best = x; a->best_flat = flat; }   /* strict: ties keep lowest flat index */

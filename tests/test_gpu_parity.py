@@ -127,50 +127,114 @@ def test_edge_cases_and_errors():
     assert np.array_equal(dev, _gpu_full(wl)["logp"])
 
 
+_ORACLE_CACHE = {}
+
+
+def _oracle_cached(name):
+    """Tier-A oracle of a named config, once per test session (the chunk tests reuse it for every chunk size)."""
+    if name not in _ORACLE_CACHE:
+        wl = W.build_workload(name)
+        _ORACLE_CACHE[name] = (wl, _oracle_full(wl))
+    return _ORACLE_CACHE[name]
+
+
+@pytest.mark.parametrize("oc", [1, 2, 5, 32])
+@pytest.mark.parametrize("name", ["tiny_mid", "small_mid", "paper_mid", "ensemble_mid"])
+def test_chunked_launch_element_by_element(name, oc):
+    """The launch shape bench.py times -- several orientations per work item, the software pipeline running across orientation
+    and CTF-group boundaries, chunk partials merged in order -- against the direct-summation oracle, every image and model:
+    >= 40 orientations x >= 7 CTFs, orientations per work item 1, 2, 5 (ragged last chunk) and 32."""
+    from paper_1609_06634_b200 import BioEM
+    wl, ref = _oracle_cached(name)
+    with BioEM() as b:
+        b.load_workload(wl)
+        b.set_orientation_chunk(oc)
+        b.run()
+        got = dict(logp=b.get_log_posterior(), **b.get_best())
+        assert b.get_run_plan()[1] == min(oc, len(wl["quats"]))
+    err = np.abs(got["logp"] - ref["logp"])
+    assert err.max() <= TOL_LOGP, f"max |dlogP| = {err.max():.3e}"
+    for k in ("orient", "ctf", "dx", "dy"):
+        bad = got[k] != ref[k]
+        assert not np.any(bad & (ref["gap"] >= 1e-6)), f"argmax {k} differs: gpu {got[k][bad]} oracle {ref[k][bad]}"
+    assert np.abs(got["log_p"] - ref["best"]).max() <= TOL_LOGP
+
+
+def _full_grid_oracle(wl, img_idx, models):
+    """Tier C (oracle/fftgrid.py: the tier-A loop nest with numpy's FFT for the transforms; pinned against tier A) on the FULL grid
+    for the chosen images and models."""
+    from oracle import fftgrid
+    s = wl["spec"]
+    out = {}
+    for mi in models:
+        st = fftgrid.run_model_fft(wl["models"][mi], s.n_pix, s.pixel_A, s.max_shift, wl["quats"], wl["ctfs"], wl["images"][img_idx])
+        out[mi] = st
+    return out
+
+
 @pytest.mark.parametrize("name", ["small", "density", "ensemble", "paper"])
-def test_full_size_sampled(name):
-    """BASELINE.json's full size, in the launch configuration bench.py times (same calls, same grid): the full-grid
-    oracle is out of reach (2.6e12 MACs per image), so outputs are checked on samples the oracle computes
-    one by one -- whole shift maps of sampled (image, orientation, CTF) tuples and of every sampled image's reported
-    argmax -- plus properties that hold at any size."""
+def test_full_size_full_grid(name):
+    """BASELINE.json's full size, in the launch configuration bench.py times (same calls, same grid, automatic chunking).
+    (1) S = 4 seeded images: log-posterior, best term and argmax against the oracle's FULL grid (tier C), for the model that
+        generated each image -- and, on Ensemble, image 0 against all 64 models;
+    (2) R = 32 seeded (image, model, orientation, CTF) tuples: the whole (2D+1)^2 map, FP64 and FP32, against tier A's direct
+        summation -- and tier C's map against tier A's on the same tuples (the pin of tier C at this size);
+    (3) properties at any size and recovery of the planted parameters."""
     import oracle
+    from oracle import fftgrid
     from paper_1609_06634_b200 import BioEM
     wl = W.build_workload(name)
     s = wl["spec"]
     n = s.n_pix ** 2
-    KK = 2 * s.max_shift + 1
-    model = oracle.prepare_model(wl["models"][0])
     logw = oracle.uniform_logw(len(wl["quats"]), len(wl["ctfs"]), s.max_shift)
     rng = np.random.default_rng(7)
     with BioEM() as b:
         b.load_workload(wl)
         b.run()
         logp, best = b.get_log_posterior(), b.get_best()
-        # (1) random tuples: the whole (2D+1)^2 map against direct summation
-        for _ in range(6):
-            img, o, c = int(rng.integers(s.n_images)), int(rng.integers(s.n_orient)), int(rng.integers(s.n_ctf))
-            I1 = oracle.calc_image(model, wl["quats"][o], wl["ctfs"][c], s.n_pix, s.pixel_A)
-            ref = oracle.shift_map(wl["images"][img], I1, s.max_shift, logw)
-            assert np.abs(b.debug_shift_map(img, 0, o, c, f64=True) - ref).max() <= 1e-6
-            assert np.abs(b.debug_shift_map(img, 0, o, c) - ref).max() <= 5e-7 * n + 1e-3
-        # (2) sampled images: the reported argmax is the maximum of the oracle's map of that (orientation, CTF), at the
-        #     reported shift, with the reported value
-        for img in rng.choice(s.n_images, size=8, replace=False):
-            o, c = int(best["orient"][img, 0]), int(best["ctf"][img, 0])
-            I1 = oracle.calc_image(model, wl["quats"][o], wl["ctfs"][c], s.n_pix, s.pixel_A)
-            ref = np.asarray(oracle.shift_map(wl["images"][img], I1, s.max_shift, logw)).reshape(KK, KK)
-            iy, ix = np.unravel_index(np.argmax(ref), ref.shape)
-            assert (ix - s.max_shift, iy - s.max_shift) == (int(best["dx"][img, 0]), int(best["dy"][img, 0]))
-            assert abs(ref[iy, ix] - best["log_p"][img, 0]) <= TOL_LOGP
-            # the posterior holds at least this map's mass and at most every term at the maximum
-            m = ref.max()
-            assert logp[img, 0] >= m + math.log(np.exp(ref - m).sum()) - TOL_LOGP
+        kernel, oc = b.get_run_plan()
+        assert oc == min(32, s.n_orient)                                  # the timed launch shape
+        # (2) random tuples
+        pm = {}
+        for _ in range(32):
+            img, mi = int(rng.integers(s.n_images)), int(rng.integers(s.n_models))
+            o, c = int(rng.integers(s.n_orient)), int(rng.integers(s.n_ctf))
+            if mi not in pm:
+                pm[mi] = oracle.prepare_model(wl["models"][mi])
+            K = fftgrid.ctf_env_table(s.n_pix, s.pixel_A, *wl["ctfs"][c])[None]
+            I1 = fftgrid.calc_image_fft(pm[mi], wl["quats"][o], K, s.n_pix, s.pixel_A)[0]
+            ref = oracle.shift_map(wl["images"][img], I1, s.max_shift, logw)              # tier A: direct summation
+            assert np.abs(fftgrid.shift_map_fft(wl["images"][img], I1, s.max_shift, logw) - ref).max() <= 1e-7
+            assert np.abs(b.debug_shift_map(img, mi, o, c, f64=True) - ref).max() <= 1e-6
+            assert np.abs(b.debug_shift_map(img, mi, o, c) - ref).max() <= 5e-7 * n + 1e-3
+    # (1) full grid
+    imgs = np.sort(rng.choice(s.n_images, size=4, replace=False))
+    t = wl["truth"]
+    todo = {}                                                             # model -> images
+    for i in imgs:
+        todo.setdefault(int(t["model"][i]), []).append(int(i))
+    if s.n_models > 1:
+        for mi in range(s.n_models):
+            todo.setdefault(mi, [])
+            if int(imgs[0]) not in todo[mi]:
+                todo[mi].append(int(imgs[0]))
+    worst = 0.0
+    for mi, il in todo.items():
+        il = np.array(sorted(il))
+        st = _full_grid_oracle(wl, il, [mi])[mi]
+        err = np.abs(logp[il, mi] - st.log_posterior())
+        worst = max(worst, err.max())
+        assert err.max() <= TOL_LOGP, f"{name}: max |dlogP| = {err.max():.3e} (model {mi}, images {il})"
+        assert np.abs(best["log_p"][il, mi] - st.best).max() <= TOL_LOGP
+        o, c, dx, dy = oracle.unflatten(st.best_flat, s.n_ctf, s.max_shift)
+        tie = (st.best - st.second) < 1e-6
+        for k, r in (("orient", o), ("ctf", c), ("dx", dx), ("dy", dy)):
+            assert np.all((best[k][il, mi] == r) | tie), (name, mi, k, best[k][il, mi], r)
+    print(f"{name}: full-grid max |dlogP| = {worst:.2e} over {sum(len(v) for v in todo.values())} (image, model) pairs")
     # (3) properties at any size: max term <= sum <= (number of terms) x max term
     n_terms = s.n_orient * s.n_ctf * s.n_shifts
     assert np.all(logp >= best["log_p"] - 1e-9) and np.all(logp <= best["log_p"] + math.log(n_terms) + 1e-9)
     assert np.all(np.isfinite(logp))
-    # planted parameters: under the generating model, the generating orientation and shift are recovered
-    t = wl["truth"]
     ii, mm = np.arange(s.n_images), np.asarray(t["model"])
     hit = (best["orient"][ii, mm] == t["orient"]) & (best["dx"][ii, mm] == t["dx"]) & (best["dy"][ii, mm] == t["dy"])
     assert hit.mean() >= 0.95, hit.mean()
@@ -183,6 +247,7 @@ def test_full_size_sampled(name):
     ("tiny_mini", 0, 3, 13, 4), ("tiny_mini", 1, 2, 21, 1), ("tiny_mini", 16, 3, 32, 3), ("tiny_mini", 17, 2, 32, 2),
     ("small_mini", 0, 2, 2304, 4), ("small_mini", 5, 3, 1536, 3), ("small_mini", 17, 2, 2304, 2),
     ("paper_mini", 0, 2, 2048, 2), ("paper_mini", 1, 3, 2048, 1), ("paper_mini", 7, 2, 4095, 2), ("paper_mini", 31, 2, 2048, 1),
+    ("paper_mini", 32, 2, 2048, 2), ("paper_mini", 40, 1, 4095, 1),       # 224 with D > 31: generic kernel
 ])
 def test_kernel_plan_edges(base, D, n_img, stride, nctf):
     import oracle
@@ -274,3 +339,124 @@ def test_affine_invariance_of_the_image(name):
     assert np.abs(b["logp"] - (a["logp"] - (n - 3) * math.log(alpha))).max() <= 2e-3
     for k in ("orient", "ctf", "dx", "dy"):
         assert np.array_equal(a[k], b[k])
+
+
+@pytest.mark.parametrize("name,which", [("tiny_mini", 1), ("small_mini", 1), ("paper_mini", 1), ("paper_mini", 3), ("paper_mid", 3)])
+def test_other_kernels_against_the_oracle(name, which):
+    """The fused kernels the automatic choice does not pick at these shapes: the generic kernel (1) at 64, 128 and 224, and round 1's
+    two-CTA-cluster kernel (3) at 224 -- a second, independently written CUDA route to the tensor-memory kernel's result."""
+    from paper_1609_06634_b200 import BioEM
+    wl, ref = _oracle_cached(name)
+    with BioEM() as b:
+        b.load_workload(wl)
+        b.debug_set_kernel(which)
+        b.run()
+        assert b.get_run_plan()[0] == which
+        got = dict(logp=b.get_log_posterior(), **b.get_best())
+    assert np.abs(got["logp"] - ref["logp"]).max() <= TOL_LOGP
+    for k in ("orient", "ctf", "dx", "dy"):
+        assert not np.any((got[k] != ref[k]) & (ref["gap"] >= 1e-6)), k
+
+
+def test_n_pix_256():
+    """The largest image size the ABI accepts (generic kernel): 256^2, D = 9, against the oracle."""
+    import oracle
+    from paper_1609_06634_b200 import BioEM
+    wl = W.build_workload(W.get_spec("paper_mini", n_pix=256, max_shift=9, n_images=2, orient_stride=2048))
+    s = wl["spec"]
+    ref = _oracle_full(wl)
+    with BioEM() as b:
+        b.load_workload(wl)
+        b.run()
+        got = dict(logp=b.get_log_posterior(), **b.get_best())
+        o, c = int(got["orient"][0, 0]), int(got["ctf"][0, 0])
+        I1 = oracle.calc_image(oracle.prepare_model(wl["models"][0]), wl["quats"][o], wl["ctfs"][c], s.n_pix, s.pixel_A)
+        assert np.abs(b.debug_calc_image(0, o, c) - I1).max() <= 2e-6 * np.abs(I1).max()
+    assert np.abs(got["logp"] - ref["logp"]).max() <= TOL_LOGP
+    for k in ("orient", "ctf", "dx", "dy"):
+        assert not np.any((got[k] != ref[k]) & (ref["gap"] >= 1e-6)), k
+
+
+@pytest.mark.parametrize("name", ["small_mini", "paper_mini"])
+def test_non_uniform_priors(name):
+    """Grid weights p(theta) (R7): per-orientation and per-CTF log-priors, one orientation and one CTF excluded (-inf)."""
+    import oracle
+    from paper_1609_06634_b200 import BioEM
+    wl = W.build_workload(name)
+    s = wl["spec"]
+    rng = np.random.default_rng(11)
+    lpo = np.log(rng.dirichlet(np.ones(len(wl["quats"])))).astype(np.float32)
+    lpc = np.log(rng.dirichlet(np.ones(len(wl["ctfs"])))).astype(np.float32)
+    lpo[1] = -np.inf
+    lpc[0] = -np.inf
+    st = oracle.run_model(wl["models"][0], s.n_pix, s.pixel_A, s.max_shift, wl["quats"], wl["ctfs"], wl["images"],
+                          lp_orient=lpo.astype(np.float64), lp_ctf=lpc.astype(np.float64))
+    with BioEM() as b:
+        b.load_workload(wl, images=False)
+        b.set_orientations_quat(wl["quats"], lpo)
+        b.set_ctf_grid(wl["ctfs"][:, 0], wl["ctfs"][:, 1], wl["ctfs"][:, 2], lpc)
+        b.push_images(wl["images"])
+        b.run()
+        got, best = b.get_log_posterior(), b.get_best()
+    assert np.abs(got[:, 0] - st.log_posterior()).max() <= TOL_LOGP
+    o, c, dx, dy = oracle.unflatten(st.best_flat, s.n_ctf, s.max_shift)
+    tie = (st.best - st.second) < 1e-6
+    for k, r in (("orient", o), ("ctf", c), ("dx", dx), ("dy", dy)):
+        assert np.all((best[k][:, 0] == r) | tie), k
+    assert not np.any(best["orient"][:, 0] == 1) and not np.any(best["ctf"][:, 0] == 0)    # the excluded grid points never win
+
+
+def test_degenerate_inputs():
+    """Inputs for which the marginal of Eq. 8 does not exist are refused, not scored (advisor, round 1): a constant image (D_omega = 0)
+    at push_images, a model that projects to nothing inside the box (T_c = 0) at the first getter after bioem_run.  A noiseless
+    planted image (rho^2 -> 1, R14) gives finite results and the planted parameters."""
+    import bioem_workloads.simulate as sim
+    from paper_1609_06634_b200 import BioEM, BioEMError
+    wl = W.build_workload("tiny_mini")
+    s = wl["spec"]
+    with BioEM() as b:
+        b.load_workload(wl, images=False)
+        flat = wl["images"].copy()
+        flat[2] = 3.25
+        with pytest.raises(BioEMError) as ei:
+            b.push_images(flat)
+        assert ei.value.code == -1
+        with pytest.raises(BioEMError):
+            b.run()                                                  # the stack was left empty
+        # noiseless planted image: N * I1(r + d) + mu with nothing else
+        o, c, d = 3, 1, (2, -3)
+        sig = sim.render_signal(wl["models"][0], wl["quats"][o], wl["ctfs"][c], s.n_pix, s.pixel_A)
+        img = (1.7 * np.roll(sig, shift=(-d[1], -d[0]), axis=(0, 1)) + 0.4).astype(np.float32)
+        b.push_images(np.stack([img, wl["images"][0]]))
+        b.run()
+        lp, best = b.get_log_posterior(), b.get_best()
+        assert np.all(np.isfinite(lp)) and np.all(np.isfinite(best["log_p"]))
+        assert (best["orient"][0, 0], best["ctf"][0, 0], best["dx"][0, 0], best["dy"][0, 0]) == (o, c, d[0], d[1])
+        # a model far outside the box: every projection is empty
+        b.clear_models()
+        b.add_model_atoms(np.array([[900.0, 900.0, 0.0]]), np.array([1.5]), np.array([1.0]))
+        b.push_images(wl["images"])
+        b.run()
+        with pytest.raises(BioEMError) as ei:
+            b.get_log_posterior()
+        assert ei.value.code == -1
+
+
+def test_split_stack_is_bit_identical():
+    """Images are independent: scoring a stack whole and in two parts gives the same bits when the orientations per
+    work item are the same (bioem_set_orientation_chunk) -- what the multi-GPU image sharding relies on."""
+    from paper_1609_06634_b200 import BioEM
+    wl = W.build_workload("small_mid")
+    outs = []
+    for parts in ([slice(None)], [slice(0, 2), slice(2, None)]):
+        lp, bo = [], []
+        for sl in parts:
+            with BioEM() as b:
+                b.load_workload(wl, images=False)
+                b.set_orientation_chunk(5)
+                b.push_images(wl["images"][sl])
+                b.run()
+                lp.append(b.get_log_posterior())
+                bo.append(np.stack([b.get_best()[k] for k in ("orient", "ctf", "dx", "dy")]))
+        outs.append((np.concatenate(lp), np.concatenate(bo, axis=1)))
+    assert np.array_equal(outs[0][0], outs[1][0]) and np.array_equal(outs[0][1], outs[1][1])

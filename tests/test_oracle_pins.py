@@ -452,3 +452,62 @@ def test_ensemble_posterior_pins():
     assert abs(oracle.ensemble_log_posterior(lp, [0.5, 0.5, 0.0, 0.0])[0] - oracle.ensemble_log_posterior(lp[:, :2], [0.5, 0.5])[0]) <= 1e-12
     u, _ = oracle.ensemble_log_posterior(lp)
     assert abs(u - oracle.ensemble_log_posterior(lp, [0.25] * 4)[0]) <= 1e-12
+
+
+# ------------------------------------------------------------------ tier C (oracle/fftgrid.py): the tier-A loop nest with numpy's FFT
+@pytest.mark.parametrize("name", ["tiny", "small_mini", "paper_mini", "density_mini"])
+def test_tier_c_matches_the_definition(name):
+    """oracle/fftgrid.py replaces tier A's transforms and its direct correlation by numpy's FFT; everything it returns -- log-posterior,
+    largest and second largest term, argmax -- must agree with tier A (direct summation, naive DFTs) on whole grids."""
+    import bioem_workloads as W
+    from oracle import fftgrid
+    wl = W.build_workload(name)
+    s = wl["spec"]
+    a = oracle.run_model(wl["models"][0], s.n_pix, s.pixel_A, s.max_shift, wl["quats"], wl["ctfs"], wl["images"])
+    b = fftgrid.run_model_fft(wl["models"][0], s.n_pix, s.pixel_A, s.max_shift, wl["quats"], wl["ctfs"], wl["images"], workers=1, chunk=2)
+    assert np.abs(a.log_posterior() - b.log_posterior()).max() <= 1e-8
+    assert np.abs(a.best - b.best).max() <= 1e-8 and np.abs(a.second - b.second).max() <= 1e-8
+    assert np.array_equal(a.best_flat, b.best_flat)
+
+
+def test_tier_c_pieces():
+    from oracle import fftgrid
+    # the CTF table against the C function, bin by bin (signed frequencies, Nyquist included)
+    N, px, a, A, b = 8, 1.5, 31.33, 0.1, 0.633
+    K = fftgrid.ctf_env_table(N, px, a, A, b)
+    for m in range(N):
+        for l in range(N):
+            ls, ms = (l if l <= N // 2 else l - N), (m if m <= N // 2 else m - N)
+            s2 = (2 * np.pi / (N * px)) ** 2 * (ls * ls + ms * ms)
+            assert abs(K[m, l] - oracle.ctf_env(s2, a, A, b)) <= 1e-14
+    # the vectorised closed form against bo_log_post_c1
+    rng = np.random.default_rng(5)
+    n = 64
+    for _ in range(20):
+        o, c = rng.normal(size=n), rng.normal(size=n)
+        Co, Coo, Cc, Ccc, Cco = o.sum(), (o * o).sum(), c.sum(), (c * c).sum(), (o * c).sum()
+        assert abs(float(fftgrid.log_post_c1(n, Co, Coo, Cc, Ccc, np.array([Cco]))[0]) - oracle.log_post_c1(n, Co, Coo, Cc, Ccc, Cco)) <= 1e-10
+    # the shift-map twin against direct summation, wrap-around included
+    img, I1 = rng.normal(size=(16, 16)).astype(np.float32), rng.normal(size=(16, 16))
+    assert np.abs(fftgrid.shift_map_fft(img, I1, 5, -1.25) - oracle.shift_map(img, I1, 5, -1.25)).max() <= 1e-9
+
+
+def test_zero_weight_grid_points_add_nothing():
+    """R7: a grid point with log-prior -inf has weight zero in Eq. 9's sum -- the result equals the run on the grid without it,
+    also when the excluded point comes first (the running log-sum-exp then starts from an empty sum)."""
+    import bioem_workloads as W
+    wl = W.build_workload("tiny_mini")
+    s = wl["spec"]
+    O, Cn = len(wl["quats"]), len(wl["ctfs"])
+    rng = np.random.default_rng(3)
+    lpo, lpc = np.log(rng.dirichlet(np.ones(O))), np.log(rng.dirichlet(np.ones(Cn)))
+    lpo0, lpc0 = lpo.copy(), lpc.copy()
+    lpo0[0] = -np.inf
+    lpc0[0] = -np.inf
+    a = oracle.run_model(wl["models"][0], s.n_pix, s.pixel_A, s.max_shift, wl["quats"], wl["ctfs"], wl["images"], lp_orient=lpo0, lp_ctf=lpc0)
+    b = oracle.run_model(wl["models"][0], s.n_pix, s.pixel_A, s.max_shift, wl["quats"][1:], wl["ctfs"][1:], wl["images"],
+                         lp_orient=lpo[1:], lp_ctf=lpc[1:])
+    assert np.all(np.isfinite(a.log_posterior())) and np.abs(a.log_posterior() - b.log_posterior()).max() <= 1e-9
+    oa, ca, dxa, dya = oracle.unflatten(a.best_flat, Cn, s.max_shift)
+    ob, cb, dxb, dyb = oracle.unflatten(b.best_flat, Cn - 1, s.max_shift)
+    assert np.array_equal(oa, ob + 1) and np.array_equal(ca, cb + 1) and np.array_equal(dxa, dxb) and np.array_equal(dya, dyb)

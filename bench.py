@@ -1,15 +1,19 @@
 #!/usr/bin/env python
 """bench.py -- posterior evaluations/s of the BioEM hot path on B200 (BASELINE.json metric).
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--config small] [--impl ours|reference]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config paper] [--impl ours|reference]
 
 A "step" is one pass of the whole hot path over one batch of synthetic images: bioem_push_images (a0) +
-bioem_run (a1-a7) for the named config (default: BASELINE.json configs[1] "small": 128^2 px, 256 images,
-4608 orientations x 32 CTFs x 33^2 shifts = 4.11e10 evaluations per step).  `value` is timed with the images
-already resident in HBM; `e2e` is the same step through the C ABI with HOST buffers (H2D of the image stack and
-D2H of the results inside the timed region).  One process per GPU (torchrun for N > 1): the path shards over
-images with no data-path collective (paper: P:199), every rank scores its own batch -> "scaling": "weak".
-`--impl reference` times the FP64 CPU oracle (the only reference there is) on a bounded sample of the same workload.
+bioem_run (a1-a7) for the named config.  The default is the LARGEST single-GPU configuration of BASELINE.json,
+"paper" (configs[2]: 224^2 px -- the paper's own box size, P:229 -- 1024 images, 4096 orientations x 32 CTFs x 61^2
+shifts = 4.99e11 evaluations per step, about 5 s); BASELINE.json quotes its metric on no particular config, and the
+other four are parity-test cases (`--config` still runs them).  `value` is timed with the images already resident in
+HBM; `e2e` is the same step through the C ABI with HOST buffers (H2D of the image stack and D2H of the results inside
+the timed region).  One process per GPU (torchrun for N > 1): the path shards over images with no data-path
+collective (paper: P:199): the global stack of N x 1024 images goes through shard.score_block_and_gather
+(every rank scores its contiguous block, one all_gather of the per-image results inside the timed region) ->
+"scaling": "weak".  `--impl reference` times the FP64 CPU oracle (the only reference there is) on a bounded sample
+of the same workload.
 """
 from __future__ import annotations
 
@@ -33,9 +37,22 @@ import bioem_workloads as W  # noqa: E402
 METRIC = "posterior evaluations/s (image x orientation x CTF x shift)"
 UNIT = "evaluations/s"
 SM_COUNT, FP32_LANES = 148, 128
-# dram__bytes_read.sum + dram__bytes_write.sum of the fused kernel, per launch, from the committed `ncu --set full`
-# capture (profiles/); None until a capture of the current kernel exists for that config.
-NCU_TRAFFIC_BYTES = {"small": 341270528 + 10024960}        # profiles/r1_v11_fused_small_full.csv
+KERNEL_NAMES = {1: "k_fused", 2: "k_fused_pk", 3: "k_fused_c2", 4: "k_fused_tm", 5: "k_fused_dft", 6: "k_realspace"}
+
+
+def ncu_table(workload):
+    """Per-launch DRAM traffic and executed flops of the fused kernel from the committed ncu captures: the row of
+    profiles/fused_kernel_ncu.csv for this workload (the .md beside it names the capture commands), or None."""
+    f = ROOT / "profiles" / "fused_kernel_ncu.csv"
+    if not f.exists():
+        return None
+    rows = [r.split(",") for r in f.read_text().splitlines() if r and not r.startswith("#")]
+    hdr = rows[0]
+    for r in rows[1:]:
+        d = dict(zip(hdr, r))
+        if d.get("workload") == workload:
+            return d
+    return None
 
 
 def algorithmic_flops_per_pair(N: int, D: int) -> float:
@@ -161,7 +178,7 @@ def run_reference(args):
 def run_ours(args):
     import torch
     import torch.distributed as dist
-    from paper_1609_06634_b200 import BioEM
+    from paper_1609_06634_b200 import BioEM, shard
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
@@ -177,8 +194,10 @@ def run_ours(args):
             dist.barrier()
         torch.cuda.synchronize()
 
+    # rank r holds block r of the global stack of world x n_images images (same config, its own image seeds)
     wl = build_inputs(args.config, rank, args.orient_stride)
     s = wl["spec"]
+    n_global = s.n_images * world
     img_host = torch.from_numpy(wl["images"]).pin_memory()
     img_dev = img_host.cuda()
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")          # > 126 MB L2
@@ -187,16 +206,20 @@ def run_ours(args):
 
     def step_device():
         flush.zero_()                                                          # L2 flush between iterations
+        b.invalidate_precompute()                                              # a1-a3 run in every step (nothing cached across steps)
+        if world > 1:                                                          # block -> results -> one all_gather (shard.py)
+            return shard.score_block_and_gather(b, img_dev, n_global)
         b.push_images(img_dev)
         b.run()
 
     def step_e2e():
         flush.zero_()
+        b.invalidate_precompute()
+        if world > 1:
+            return shard.score_block_and_gather(b, img_host, n_global)
         b.push_images(img_host)                                                # H2D inside the step
         b.run()
-        lp = b.get_log_posterior()                                             # D2H inside the step
-        best = b.get_best()
-        return lp, best
+        return dict(logp=b.get_log_posterior(), **b.get_best())                # D2H inside the step
 
     for _ in range(max(args.warmup, 1)):
         step_device()
@@ -208,25 +231,27 @@ def run_ours(args):
     for _ in range(args.steps):
         step_device()
         launches += b.get_launch_count()[0]                                    # kernels of push_images + run
+        fused_ms.append(b.get_timing()[1])                                     # CUDA events around the fused kernel, on the context's stream
     e1.record()
     barrier()
     clocks = sampler.stop() if sampler else None
-    fused_ms = b.get_timing()[1]                                               # CUDA events around the fused kernel (last step)
+    fused_ms = float(np.mean(fused_ms))                                        # average launch duration over the timed region
     total_ms_last = b.get_timing()[0]
+    kern, oc = b.get_run_plan()
     t_dev = e0.elapsed_time(e1) * 1e-3
 
     # ---- end to end through the C ABI with host buffers
-    lp, best = step_e2e()
+    res = step_e2e()
     barrier()
     t0 = time.perf_counter()
     e0.record()
     for _ in range(args.steps):
-        lp, best = step_e2e()
+        res = step_e2e()
     e1.record()
     barrier()
     t_e2e = max(e0.elapsed_time(e1) * 1e-3, time.perf_counter() - t0)
     h2d = int(img_host.numel() * 4)
-    d2h = int(lp.nbytes + sum(v.nbytes for v in best.values()))
+    d2h = int(sum(np.asarray(v).nbytes for v in res.values())) // world       # this rank's share of the results
 
     if world > 1:
         t = torch.tensor([t_dev, t_e2e], device="cuda", dtype=torch.float64)
@@ -237,15 +262,21 @@ def run_ours(args):
         peaks, peak_src = measured_peaks()
         fp32_peak = SM_COUNT * FP32_LANES * 2 * peaks.get("sm_max_mhz", 1965.0) * 1e6 / 1e12          # TFLOP/s, DESIGN 7
         fma_meas, _ = b.measure_fp32_peak()
-        fl = algorithmic_flops_per_pair(s.n_pix, s.max_shift) * s.n_pairs
+        fpp = algorithmic_flops_per_pair(s.n_pix, s.max_shift)
+        fl = fpp * s.n_pairs
         achieved = fl / (fused_ms * 1e-3) / 1e12
         hbm_bytes = s.n_pairs * 8.0 * s.n_pix * (s.n_pix // 2 + 1)               # streaming Ohat once per pair
+        ncu = ncu_table(s.name) or {}
+        ex = float(ncu["executed_flops_per_pair"]) if ncu.get("executed_flops_per_pair") else None
         roof = {
-            "bound": "alu", "kernel": ("k_fused_pk" if s.n_pix in (64, 128) and s.max_shift <= 16 else "k_fused_c2" if s.n_pix == 224 and s.max_shift <= 31 else "k_fused") + " (a4+a5+a6)", "achieved": achieved, "peak": fp32_peak, "unit": "TFLOP/s",
-            "frac": achieved / fp32_peak, "traffic": NCU_TRAFFIC_BYTES.get(s.name),
+            "bound": "alu", "kernel": KERNEL_NAMES.get(kern, str(kern)) + " (a4+a5+a6)", "orientations_per_work_item": oc,
+            "achieved": achieved, "peak": fp32_peak, "unit": "TFLOP/s",
+            "frac": achieved / fp32_peak, "traffic": float(ncu["dram_bytes_per_launch"]) if ncu.get("dram_bytes_per_launch") else None,
+            "traffic_source": ncu.get("capture"),
             "peak_source": f"148 SM x 128 lanes x 2 x {peaks.get('sm_max_mhz', 1965.0):.0f} MHz (formula, {peak_src})",
             "measured_ffma_tflops": fma_meas, "frac_of_measured_ffma": achieved / fma_meas,
-            "kernel_ms": fused_ms, "step_ms_on_device": total_ms_last, "flops_per_pair": algorithmic_flops_per_pair(s.n_pix, s.max_shift),
+            "kernel_ms": fused_ms, "step_ms_on_device": total_ms_last, "flops_per_pair": fpp,
+            "executed_flops_per_pair": ex, "executed_tflops": (ex * s.n_pairs / (fused_ms * 1e-3) / 1e12) if ex else None,
             "hbm_alt": {"bytes_per_launch_if_streamed": hbm_bytes, "gbs_equivalent": hbm_bytes / (fused_ms * 1e-3) / 1e9,
                         "peak_gbs": peaks.get("hbm_gbs")},
         }
@@ -257,8 +288,9 @@ def run_ours(args):
             "dtype": "f32", "data": "synthetic",
             "config": {"workload": s.name, "n_pix": s.n_pix, "n_images_per_gpu": s.n_images, "n_models": s.n_models,
                        "n_orient": s.n_orient, "n_ctf": s.n_ctf, "max_shift": s.max_shift, "evaluations_per_step_per_gpu": s.n_evaluations,
-                       "cache": "L2 flushed between iterations (256 MiB write); projection spectra (>= 306 MB) are regenerated every step",
-                       "precision": "hot loop FP32, precompute and top-8 re-scoring FP64", "parallelism": f"images sharded, dp{world}"},
+                       "cache": "L2 flushed between iterations (256 MiB write); projection spectra are regenerated every step",
+                       "precision": "hot loop FP32, precompute and top-8 re-scoring FP64",
+                       "parallelism": f"images sharded, dp{world}" + (", results all_gathered every step" if world > 1 else "")},
             "e2e": {"value": evals_job / t_e2e, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
             "gpu_launches": launches, "clocks": clocks, "roofline": roof,
             "cpu_baseline": {"value": rate, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample, "seconds": dt},
@@ -300,7 +332,7 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", default="small", choices=sorted(W.CONFIGS))
+    ap.add_argument("--config", default="paper", choices=sorted(W.CONFIGS))
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--orient-stride", type=int, default=1,
                     help="profiling aid: keep every k-th orientation of the grid (the workload name in the JSON line says so)")

@@ -86,6 +86,13 @@ int bioem_push_images(bioem_ctx *ctx, int n_img, const float *pixels, int is_dev
  * P:126; Eqs. 11-12; closed-form marginal over N, mu, lambda).  Requires geometry,
  * >= 1 model, orientations, CTFs, a shift range and images (else BIOEM_EBADSTATE). */
 int bioem_run(bioem_ctx *ctx);
+/* Calculated-image cache.  The outputs of a1-a3 (projection spectra, CTF tables, T_c; "calculated once per
+ * orientation and CTF set") depend on the models, grids and shift range only, so a bioem_run that follows another one with
+ * nothing but the image stack replaced reuses them: this is how an image stack larger than device memory is scored in
+ * subsets -- bioem_push_images(subset) + bioem_run + bioem_get_* per subset, results concatenated; images are
+ * independent.  Every bioem_set_* / bioem_add_model_* / bioem_clear_models call drops the cache;
+ * bioem_invalidate_precompute drops it explicitly (bench.py does, so that every timed step runs all of a0-a7). */
+int bioem_invalidate_precompute(bioem_ctx *ctx);
 /* Domain of validity.  bioem_run only enqueues; a calculated image that is empty or not finite (T_c = n C_cc - C_c^2 is
  * not > 0: the model projects to nothing inside the box) is detected on the device and reported as BIOEM_EBADARG by the first
  * bioem_get_* call.  The hot loop is FP32 on operands correctly rounded from FP64; the BIOEM_TOPK largest terms per

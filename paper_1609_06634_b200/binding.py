@@ -17,7 +17,7 @@ EXPORTED_SYMBOLS = [
     "bioem_get_best", "bioem_debug_calc_image", "bioem_debug_shift_map", "bioem_debug_shift_map_f64",
     "bioem_debug_log_posterior_f32", "bioem_get_timing", "bioem_get_launch_count", "bioem_measure_fp32_peak",
     "bioem_set_orientation_posterior", "bioem_get_orientation_log_posterior", "bioem_get_ensemble_log_posterior",
-    "bioem_set_orientation_chunk", "bioem_debug_set_kernel", "bioem_get_run_plan",
+    "bioem_set_orientation_chunk", "bioem_debug_set_kernel", "bioem_get_run_plan", "bioem_invalidate_precompute",
 ]
 KERNEL_AUTO, KERNEL_GENERIC, KERNEL_PK, KERNEL_C2, KERNEL_TM = 0, 1, 2, 3, 4
 
@@ -59,6 +59,7 @@ def lib():
         L.bioem_set_shift_range.argtypes = [C.c_void_p, C.c_int]
         L.bioem_push_images.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_int]
         L.bioem_run.argtypes = [C.c_void_p]
+        L.bioem_invalidate_precompute.argtypes = [C.c_void_p]
         L.bioem_get_log_posterior.argtypes = [C.c_void_p, _dp]
         L.bioem_get_best.argtypes = [C.c_void_p, _ip, _ip, _ip, _ip, _dp]
         L.bioem_debug_calc_image.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, _fp]
@@ -192,6 +193,9 @@ class BioEM:
 
     def run(self):
         self._ck(self._L.bioem_run(self._h))
+
+    def invalidate_precompute(self):
+        self._ck(self._L.bioem_invalidate_precompute(self._h))
 
     def get_log_posterior(self):
         out = np.empty((self.n_img, self.n_models))

@@ -58,11 +58,12 @@ struct bioem_ctx {
     DBuf Ohat64, Ohat32, Dw, beta;
     // run state
     bool ran = false;
+    bool pre_valid = false;                            // a1-a3 outputs (F0, K, T_c, h, alpha) match the current models / grids / shift range
     bool want_orient = false, ran_orient = false;      // per-orientation posterior: requested / produced by the last run
     int oc_user = 0;                                   // orientations per work item (0 = automatic)
     int kernel_user = 0;                               // BIOEM_KERNEL_*: which fused kernel bioem_run may pick (0 = automatic)
     int n_sm = 148;
-    DBuf flags;                                        // int[1]: bit 0 = an image without variance, bit 1 = an empty calculated image
+    DBuf flags;                                        // int[2]: [0] bit 0 = an image without variance (a0); [1] bit 1 = an empty calculated image (a3)
     int run_kernel = 0, run_oc = 0;
     bool flags_checked = true;
     DBuf logp_orient;
@@ -108,7 +109,7 @@ int bioem_create(bioem_ctx **out, int device, void *cuda_stream)
     for (int i = 0; i < 4; ++i)
         if (cudaEventCreate(&ctx->ev[i]) != cudaSuccess) { delete ctx; return BIOEM_ECUDA; }
     if (cudaDeviceGetAttribute(&ctx->n_sm, cudaDevAttrMultiProcessorCount, device) != cudaSuccess || ctx->n_sm < 1) ctx->n_sm = 148;
-    if (ctx->flags.ensure(sizeof(int)) != cudaSuccess || cudaMemset(ctx->flags.p, 0, sizeof(int)) != cudaSuccess) {
+    if (ctx->flags.ensure(2 * sizeof(int)) != cudaSuccess || cudaMemset(ctx->flags.p, 0, 2 * sizeof(int)) != cudaSuccess) {
         cudaGetLastError();
         for (int i = 0; i < 4; ++i) cudaEventDestroy(ctx->ev[i]);
         delete ctx;
@@ -144,7 +145,7 @@ int bioem_set_image_geometry(bioem_ctx *ctx, int n_pix, float pixel_size_A)
     ctx->N = n_pix;
     ctx->px = (double)pixel_size_A;
     ctx->n_img = 0;
-    ctx->ran = false;
+    ctx->ran = false; ctx->pre_valid = false;
     return BIOEM_OK;
 }
 
@@ -155,7 +156,7 @@ int bioem_clear_models(bioem_ctx *ctx)
     cudaStreamSynchronize(ctx->stream);
     for (auto &m : ctx->models) { m.xyz.release(); m.rad.release(); m.wt.release(); m.rho.release(); }
     ctx->models.clear();
-    ctx->ran = false;
+    ctx->ran = false; ctx->pre_valid = false;
     return BIOEM_OK;
 }
 
@@ -189,7 +190,7 @@ int bioem_add_model_atoms(bioem_ctx *ctx, int n_atoms, const float *xyz_A, const
         return rc;
     }
     if (model_id) *model_id = (int)ctx->models.size() - 1;
-    ctx->ran = false;
+    ctx->ran = false; ctx->pre_valid = false;
     return BIOEM_OK;
 }
 
@@ -208,7 +209,7 @@ int bioem_add_model_density(bioem_ctx *ctx, int n_vox, float voxel_A, const floa
     if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
     if (e != cudaSuccess) { m.rho.release(); ctx->models.pop_back(); CK(e); }
     if (model_id) *model_id = (int)ctx->models.size() - 1;
-    ctx->ran = false;
+    ctx->ran = false; ctx->pre_valid = false;
     return BIOEM_OK;
 }
 
@@ -236,7 +237,7 @@ int bioem_set_orientations_quat(bioem_ctx *ctx, int n, const float *q, const flo
         if ((rc = upload_doubles(ctx, ctx->lp_orient, lp))) return rc;
     }
     ctx->n_orient = n;
-    ctx->ran = false;
+    ctx->ran = false; ctx->pre_valid = false;
     return BIOEM_OK;
 }
 
@@ -259,7 +260,7 @@ int bioem_set_ctf_grid(bioem_ctx *ctx, int n, const float *a, const float *A, co
         if ((rc = upload_doubles(ctx, ctx->lp_ctf, lp))) return rc;
     }
     ctx->n_ctf = n;
-    ctx->ran = false;
+    ctx->ran = false; ctx->pre_valid = false;
     return BIOEM_OK;
 }
 
@@ -279,7 +280,7 @@ int bioem_set_shift_range(bioem_ctx *ctx, int max_shift_px)
     if (max_shift_px < 0) FAIL(BIOEM_EBADARG, "set_shift_range: negative");
     if (ctx->N && 2 * max_shift_px + 1 > ctx->N) FAIL(BIOEM_EBADARG, "set_shift_range: 2D+1 exceeds n_pix");
     ctx->D = max_shift_px;
-    ctx->ran = false;
+    ctx->ran = false; ctx->pre_valid = false;
     return BIOEM_OK;
 }
 
@@ -402,60 +403,63 @@ int bioem_run(bioem_ctx *ctx)
     CK(ctx->best_logp.ensure(IM * sizeof(double)));
 
     CK(cudaEventRecord(ctx->ev[0], st));
-    CK(cudaMemsetAsync(ctx->flags.p, 0, sizeof(int), st));
+    if (!ctx->pre_valid) CK(cudaMemsetAsync(ctx->flags.as<int>() + 1, 0, sizeof(int), st));
 
-    // ---- a3: CTF tables
-    CK(launch_ctf_tables(ctx->ctf_a.as<double>(), ctx->ctf_A.as<double>(), ctx->ctf_b.as<double>(), C, N, ctx->px, ctx->K64.as<double>(),
-                         ctx->K32.as<float>(), st));
-    ctx->launches += 1;
-    if (use_pk) {
-        CK(ctx->Kt.ensure(pk_kt_bytes(N, C)));
-        CK(launch_relayout_K(N, ctx->K32.as<float>(), ctx->Kt.as<float>(), C, st));
+    if (!ctx->pre_valid) {
+        // ---- a3: CTF tables
+        CK(launch_ctf_tables(ctx->ctf_a.as<double>(), ctx->ctf_A.as<double>(), ctx->ctf_b.as<double>(), C, N, ctx->px, ctx->K64.as<double>(),
+                             ctx->K32.as<float>(), st));
         ctx->launches += 1;
-    } else if (use_c2) {
-        CK(ctx->Kt.ensure(c2_kt_bytes(C)));
-        CK(launch_relayout_K_c2(ctx->K32.as<float>(), ctx->Kt.as<float>(), C, st));
-        ctx->launches += 1;
-    } else if (use_tm) {
-        CK(ctx->Kt.ensure(tm_kt_bytes(C)));
-        CK(launch_relayout_K_tm(ctx->K32.as<float>(), ctx->Kt.as<float>(), C, st));
-        ctx->launches += 1;
-    }
-
-    // ---- a1/a1' + a2: spectra of all projections, model by model, orientation batch by batch
-    const int OB = 256;
-    for (int mi = 0; mi < M; ++mi) {
-        Model &m = ctx->models[mi];
-        cd *F64m = ctx->F064.as<cd>() + (size_t)mi * O * H;
-        if (m.kind == 0) {
-            CK(ctx->scratch_a.ensure((size_t)OB * n * sizeof(double)));      // I0 (double)
-            CK(ctx->scratch_b.ensure((size_t)OB * H * sizeof(cd)));          // transform intermediate
-            CK(ctx->scratch_c.ensure((size_t)OB * n * sizeof(long long)));   // fixed-point accumulator
-            // fixed-point scale: a pixel can never hold more than the total |weight| of the model
-            int ex = 0;
-            std::frexp(m.sum_abs_w > 0 ? m.sum_abs_w : 1.0, &ex);
-            const double fx_scale = std::ldexp(1.0, 60 - ex);
-            for (int o0 = 0; o0 < O; o0 += OB) {
-                const int nb = std::min(OB, O - o0);
-                CK(launch_project_atoms(m.xyz.as<double>(), m.rad.as<double>(), m.wt.as<double>(), m.n_atoms, ctx->rot.as<double>() + (size_t)o0 * 9,
-                                        nb, N, ctx->px, fx_scale, ctx->scratch_c.as<long long>(), ctx->scratch_a.as<double>(), st));
-                CK(launch_fft2_r2c_f64(ctx->scratch_a.as<double>(), nb, N, ctx->scratch_b.as<cd>(), F64m + (size_t)o0 * H, st));
-                ctx->launches += 4;
-            }
-        } else {
-            const size_t n3 = (size_t)N * N * N;
-            CK(ctx->scratch_a.ensure(n3 * sizeof(cd)));
-            CK(ctx->scratch_b.ensure(n3 * sizeof(cd)));
-            CK(launch_dft3_f64(m.rho.as<float>(), N, ctx->scratch_a.as<cd>(), ctx->scratch_b.as<cd>(), st));
-            CK(launch_slice_f64(ctx->scratch_a.as<cd>(), N, m.voxel, ctx->rot.as<double>(), O, F64m, st));
-            ctx->launches += 6;
+        if (use_pk) {
+            CK(ctx->Kt.ensure(pk_kt_bytes(N, C)));
+            CK(launch_relayout_K(N, ctx->K32.as<float>(), ctx->Kt.as<float>(), C, st));
+            ctx->launches += 1;
+        } else if (use_c2) {
+            CK(ctx->Kt.ensure(c2_kt_bytes(C)));
+            CK(launch_relayout_K_c2(ctx->K32.as<float>(), ctx->Kt.as<float>(), C, st));
+            ctx->launches += 1;
+        } else if (use_tm) {
+            CK(ctx->Kt.ensure(tm_kt_bytes(C)));
+            CK(launch_relayout_K_tm(ctx->K32.as<float>(), ctx->Kt.as<float>(), C, st));
+            ctx->launches += 1;
         }
+
+        // ---- a1/a1' + a2: spectra of all projections, model by model, orientation batch by batch
+        const int OB = 256;
+        for (int mi = 0; mi < M; ++mi) {
+            Model &m = ctx->models[mi];
+            cd *F64m = ctx->F064.as<cd>() + (size_t)mi * O * H;
+            if (m.kind == 0) {
+                CK(ctx->scratch_a.ensure((size_t)OB * n * sizeof(double)));      // I0 (double)
+                CK(ctx->scratch_b.ensure((size_t)OB * H * sizeof(cd)));          // transform intermediate
+                CK(ctx->scratch_c.ensure((size_t)OB * n * sizeof(long long)));   // fixed-point accumulator
+                // fixed-point scale: a pixel can never hold more than the total |weight| of the model
+                int ex = 0;
+                std::frexp(m.sum_abs_w > 0 ? m.sum_abs_w : 1.0, &ex);
+                const double fx_scale = std::ldexp(1.0, 60 - ex);
+                for (int o0 = 0; o0 < O; o0 += OB) {
+                    const int nb = std::min(OB, O - o0);
+                    CK(launch_project_atoms(m.xyz.as<double>(), m.rad.as<double>(), m.wt.as<double>(), m.n_atoms, ctx->rot.as<double>() + (size_t)o0 * 9,
+                                            nb, N, ctx->px, fx_scale, ctx->scratch_c.as<long long>(), ctx->scratch_a.as<double>(), st));
+                    CK(launch_fft2_r2c_f64(ctx->scratch_a.as<double>(), nb, N, ctx->scratch_b.as<cd>(), F64m + (size_t)o0 * H, st));
+                    ctx->launches += 4;
+                }
+            } else {
+                const size_t n3 = (size_t)N * N * N;
+                CK(ctx->scratch_a.ensure(n3 * sizeof(cd)));
+                CK(ctx->scratch_b.ensure(n3 * sizeof(cd)));
+                CK(launch_dft3_f64(m.rho.as<float>(), N, ctx->scratch_a.as<cd>(), ctx->scratch_b.as<cd>(), st));
+                CK(launch_slice_f64(ctx->scratch_a.as<cd>(), N, m.voxel, ctx->rot.as<double>(), O, F64m, st));
+                ctx->launches += 6;
+            }
+        }
+        CK(launch_cast_spectrum(ctx->F064.as<cd>(), ctx->F032.as<cf>(), MO * H, st));
+        CK(launch_calc_stats(ctx->F064.as<cd>(), ctx->K64.as<double>(), (int)MO, O, C, N, ctx->has_lp_orient ? ctx->lp_orient.as<double>() : nullptr,
+                             ctx->has_lp_ctf ? ctx->lp_ctf.as<double>() : nullptr, std::log((double)(2 * D + 1) * (2 * D + 1)),
+                             ctx->Tc64.as<double>(), ctx->h64.as<double>(), ctx->alpha32.as<float>(), ctx->h32.as<float>(), ctx->flags.as<int>() + 1, st));
+        ctx->launches += 2;
+
     }
-    CK(launch_cast_spectrum(ctx->F064.as<cd>(), ctx->F032.as<cf>(), MO * H, st));
-    CK(launch_calc_stats(ctx->F064.as<cd>(), ctx->K64.as<double>(), (int)MO, O, C, N, ctx->has_lp_orient ? ctx->lp_orient.as<double>() : nullptr,
-                         ctx->has_lp_ctf ? ctx->lp_ctf.as<double>() : nullptr, std::log((double)(2 * D + 1) * (2 * D + 1)),
-                         ctx->Tc64.as<double>(), ctx->h64.as<double>(), ctx->alpha32.as<float>(), ctx->h32.as<float>(), ctx->flags.as<int>(), st));
-    ctx->launches += 2;
 
     // ---- a4-a6: the fused kernel
     FusedParams p{};
@@ -492,6 +496,7 @@ int bioem_run(bioem_ctx *ctx)
     }
     CK(cudaEventRecord(ctx->ev[3], st));
     ctx->ran = true;
+    ctx->pre_valid = true;
     ctx->flags_checked = false;
     ctx->run_kernel = kern; ctx->run_oc = oc;
     ctx->run_models = M; ctx->run_orient = O; ctx->run_ctf = C; ctx->run_D = D; ctx->run_img = I;
@@ -504,10 +509,10 @@ static int check_run_flags(bioem_ctx *ctx)
 {
     if (ctx->flags_checked) return BIOEM_OK;
     int fl = 0;
-    CK(cudaMemcpyAsync(&fl, ctx->flags.p, sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
+    CK(cudaMemcpyAsync(&fl, ctx->flags.as<int>() + 1, sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
     CK(cudaStreamSynchronize(ctx->stream));
     if (fl & 2) {
-        ctx->ran = false;
+        ctx->ran = false; ctx->pre_valid = false;
         FAIL(BIOEM_EBADARG, "run: a calculated image is empty or not finite (T_c = sum |I1|^2 is not > 0): its posterior is undefined");
     }
     ctx->flags_checked = true;
@@ -701,6 +706,13 @@ int bioem_debug_set_kernel(bioem_ctx *ctx, int which)
     if (!ctx) return BIOEM_EBADARG;
     if (which != KERNEL_AUTO && which != KERNEL_GENERIC && which != KERNEL_C2) FAIL(BIOEM_EBADARG, "debug_set_kernel: 0 (automatic), 1 (generic) or 3 (two-CTA cluster, n_pix = 224)");
     ctx->kernel_user = which;
+    return BIOEM_OK;
+}
+
+int bioem_invalidate_precompute(bioem_ctx *ctx)
+{
+    if (!ctx) return BIOEM_EBADARG;
+    ctx->pre_valid = false;
     return BIOEM_OK;
 }
 

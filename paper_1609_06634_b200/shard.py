@@ -50,6 +50,26 @@ def gather_by_image(local: dict, n_images: int, group=None) -> dict:
     return out
 
 
+def default_score(ctx, block) -> dict:
+    """The library calls on one block of images: a0 (push_images), a1-a7 (run), results."""
+    ctx.push_images(block)
+    ctx.run()
+    return dict(logp=ctx.get_log_posterior(), **ctx.get_best())
+
+
+def score_block_and_gather(ctx, block, n_images: int, score=None, group=None) -> dict:
+    """This rank already holds ITS block of a stack of `n_images` images (block r = image_shard(n_images, r, world); e.g. each
+    rank read its own part of the stack): score it and all_gather the per-image results in image order."""
+    import torch.distributed as dist
+
+    world = dist.get_world_size(group) if dist.is_initialized() else 1
+    rank = dist.get_rank(group) if dist.is_initialized() else 0
+    b, e = image_shard(n_images, rank, world)
+    if len(block) != e - b:
+        raise ValueError(f"score_block_and_gather: rank {rank} owns images [{b}, {e}) but was handed {len(block)}")
+    return gather_by_image((score or default_score)(ctx, block), n_images, group)
+
+
 def run_sharded(make_ctx, images, score=None, group=None) -> dict:
     """Score `images` ([I][N][N]) across the ranks of `group`.  `make_ctx()` returns a configured context (models and
     grids set, no images); `score(ctx, block)` returns a dict of per-image arrays and defaults to the library calls."""
@@ -58,11 +78,6 @@ def run_sharded(make_ctx, images, score=None, group=None) -> dict:
     world = dist.get_world_size(group) if dist.is_initialized() else 1
     rank = dist.get_rank(group) if dist.is_initialized() else 0
     b, e = image_shard(len(images), rank, world)
-
-    def default_score(ctx, block):
-        ctx.push_images(block)
-        ctx.run()
-        return dict(logp=ctx.get_log_posterior(), **ctx.get_best())
 
     ctx = make_ctx()
     local = (score or default_score)(ctx, images[b:e]) if e > b else None

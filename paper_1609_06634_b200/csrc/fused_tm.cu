@@ -95,6 +95,14 @@ __device__ __forceinline__ void tm_horner7x4(c2 (&y)[4], const c2 *zc, c2 r_lo, 
         }
 }
 
+// The four pass-1 outputs of a lane -> rows of G_T.  Lanes whose output index lies outside |k| <= D do not store (predicated
+// stores: a dummy address for them put a second wavefront on every store, profiles/r2_tm_v8).
+__device__ __forceinline__ void tm_store_rows(c2 *g_lo, c2 *g_hi, bool v_lo, bool v_hi, const c2 (&y)[4])
+{
+    if (v_lo) { g_lo[0] = y[0]; g_lo[TM::RP] = y[2]; }
+    if (v_hi) { g_hi[0] = y[1]; g_hi[TM::RP] = y[3]; }
+}
+
 // a5 + a6 for the 8 correlations a lane holds after the H-phase of a pass-2 tile: y[2 i + u] = (B(dx_u, row' 2 p), B(dx_u, row' 2 p + 1))
 // of row pair p = pA + i, at dx_0 = k_lo, dx_1 = k_hi.  rho^2 = B^2 alpha^2 beta^2; g = cA log1p(-rho^2) + h (form C2, base-2 units);
 // log1p(-x) = -x (1 + x/2 + x^2/3 + x^3/4 + x^4/5) for x < 2^-6 (truncation < 2e-10 relative).
@@ -199,7 +207,7 @@ __device__ __forceinline__ void tm_score_commit(const TmScore &sc, const FusedPa
 // is G(., 0) + i G(., 112) with both parts real).
 template <bool ODD, bool NYQ, bool BACK>
 __device__ __forceinline__ void tm_p1_slot(c2 (&a)[16], uint32_t qaddr, const float4 (&kq)[8], bool nyq, const c2 *qn, const float *__restrict__ kn,
-                                           const c2 *zrd, c2 r_lo, c2 r_hi, c2 *g_lo, c2 *g_hi)
+                                           const c2 *zrd, c2 r_lo, c2 r_hi, c2 *g_lo, c2 *g_hi, bool v_lo, bool v_hi)
 {
     uint32_t qa[2][8], qb[2][8];
     tm_ld8(qaddr, qa[0]);
@@ -207,7 +215,7 @@ __device__ __forceinline__ void tm_p1_slot(c2 (&a)[16], uint32_t qaddr, const fl
     if (BACK) {
         c2 y[4];
         tm_horner7x4(y, zrd, r_lo, r_hi);
-        g_lo[0] = y[0]; g_hi[0] = y[1]; g_lo[TM::RP] = y[2]; g_hi[TM::RP] = y[3];
+        tm_store_rows(g_lo, g_hi, v_lo, v_hi, y);
     }
 #pragma unroll
     for (int g = 0; g < 4; ++g) {
@@ -345,7 +353,7 @@ __global__ void __launch_bounds__(TM::NT, 1) k_fused_tm(FusedParams p, const flo
     constexpr size_t KSTR = (size_t)TM::NTASK * 8 * 32;               // float4 per CTF
     // pass 2: this thread's row pair (F') of task q2; the pairs this lane scores are pA2, pA2 + 1
     const bool t2act = cons && q2 < ntask2;
-    const int pl2 = 4 * q2 + colw, prf2 = (has_col && t2act && pl2 < NP) ? pl2 : 0;
+    const int pl2 = 4 * q2 + colw, prf2 = (t2act && pl2 < NP) ? pl2 : 0;      // lanes with t7 = 7 read what lane t = 0 of their quarter-warp reads: a broadcast
     const int pA2 = 4 * q2 + 2 * c2h;
 
     float4 kq[8];
@@ -393,11 +401,11 @@ __global__ void __launch_bounds__(TM::NT, 1) k_fused_tm(FusedParams p, const flo
                 c2 a[16];
                 {
                     c2 *gp = Gw + (size_t)(col0 - 16) * RP;
-                    c2 *g_lo = vl_od ? gp + rl_od : gdump, *g_hi = vh_od ? gp + rh_od : gdump;
+                    c2 *g_lo = gp + rl_od, *g_hi = gp + rh_od;
                     if (i == 0) {
-                        if (warp_nyq) tm_p1_slot<false, true, false>(a, qaddr0, kq, nyq, qn + t, KtN + (size_t)c * N + t, zrd, wl_od, wh_od, g_lo, g_hi);
-                        else tm_p1_slot<false, false, false>(a, qaddr0, kq, false, nullptr, nullptr, zrd, wl_od, wh_od, g_lo, g_hi);
-                    } else tm_p1_slot<false, false, true>(a, qaddr0 + 64, kq, false, nullptr, nullptr, zrd, wl_od, wh_od, g_lo, g_hi);
+                        if (warp_nyq) tm_p1_slot<false, true, false>(a, qaddr0, kq, nyq, qn + t, KtN + (size_t)c * N + t, zrd, wl_od, wh_od, g_lo, g_hi, vl_od, vh_od);
+                        else tm_p1_slot<false, false, false>(a, qaddr0, kq, false, nullptr, nullptr, zrd, wl_od, wh_od, g_lo, g_hi, vl_od, vh_od);
+                    } else tm_p1_slot<false, false, true>(a, qaddr0 + 64, kq, false, nullptr, nullptr, zrd, wl_od, wh_od, g_lo, g_hi, vl_od, vh_od);
                 }
                 __syncwarp();                                         // every lane has read the tile
                 pk_spill16(zrow, a);
@@ -406,9 +414,9 @@ __global__ void __launch_bounds__(TM::NT, 1) k_fused_tm(FusedParams p, const flo
                 if (i == 0 && s >= 2) tm_mbar_wait(&bar_empty[b], ((unsigned)(s >> 1) & 1u) ^ 1u);   // every consumer has read buffer b (step s - 2)
                 {
                     c2 *gp = Gw + (size_t)col0 * RP;
-                    c2 *g_lo = vl_ev ? gp + rl_ev : gdump, *g_hi = vh_ev ? gp + rh_ev : gdump;
-                    if (warp_nyq && i == 0) tm_p1_slot<true, true, true>(a, qaddr0, kq, nyq, qn + t, KtN + (size_t)c * N + t, zrd, wl_ev, wh_ev, g_lo, g_hi);
-                    else tm_p1_slot<true, false, true>(a, qaddr0 + 64 * i, kq, false, nullptr, nullptr, zrd, wl_ev, wh_ev, g_lo, g_hi);
+                    c2 *g_lo = gp + rl_ev, *g_hi = gp + rh_ev;
+                    if (warp_nyq && i == 0) tm_p1_slot<true, true, true>(a, qaddr0, kq, nyq, qn + t, KtN + (size_t)c * N + t, zrd, wl_ev, wh_ev, g_lo, g_hi, vl_ev, vh_ev);
+                    else tm_p1_slot<true, false, true>(a, qaddr0 + 64 * i, kq, false, nullptr, nullptr, zrd, wl_ev, wh_ev, g_lo, g_hi, vl_ev, vh_ev);
                 }
                 {
                     // K of the next task: the next task of this CTF, or the first task of the next CTF (wrapping to c_lo with the next orientation)
@@ -425,10 +433,9 @@ __global__ void __launch_bounds__(TM::NT, 1) k_fused_tm(FusedParams p, const flo
             {
                 // ================= flush: odd-k rows of the last task -> G_T; this warp's share of step s is complete
                 c2 *gp = Gw + (size_t)(4 * (task0 + 4 * (nt - 1))) * RP;
-                c2 *g_lo = vl_od ? gp + rl_od : gdump, *g_hi = vh_od ? gp + rh_od : gdump;
                 c2 y[4];
                 tm_horner7x4(y, zrd, wl_od, wh_od);
-                g_lo[0] = y[0]; g_hi[0] = y[1]; g_lo[RP] = y[2]; g_hi[RP] = y[3];
+                tm_store_rows(gp + rl_od, gp + rh_od, vl_od, vh_od, y);
                 __syncwarp();
                 if (lane == 0) pk_mbar_arrive(&bar_full[b]);
             }

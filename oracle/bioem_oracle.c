@@ -20,9 +20,12 @@
  *     the direct summation and it is only used to extend full-grid goldens.
  *
  * Parity pins (tests/test_oracle_*.py): every function below has at least one pin
- * that is not a restatement of itself, except bo_fourier_slice at general
- * orientations, which is pinned only loosely against the analytic projection of
- * Gaussian blobs ("parity unpinned beyond the definition R21" -- see DESIGN.md).
+ * that is not a restatement of itself.  bo_fourier_slice (R21, a definition the
+ * paper does not give) is pinned exactly at general orientations on spectra that
+ * are multi-affine in k (which trilinear interpolation reproduces exactly, so the
+ * expected slice is a closed form), exactly at the rotations that permute the grid
+ * (90 deg about x, y, z; 120 deg about the body diagonal), exactly at the identity
+ * against the 2-D DFT of the z-sum, and loosely against analytic Gaussian blobs.
  *
  * Layout: images are row-major [k][j] = [y][x], x fastest (R11).
  */

@@ -134,6 +134,36 @@ int bioem_get_ensemble_log_posterior(bioem_ctx *ctx, const double *weights, doub
  * posterior is enabled. */
 int bioem_set_orientation_chunk(bioem_ctx *ctx, int n_orient_per_item);
 
+/* ---- orientation sharding: the paper's MPI axis ("MPI over orientations"; no communication but one gather) ----
+ * Every rank holds all models, grids and images and scores a contiguous SLICE [o_begin, o_end) of the orientation grid; indices,
+ * priors and the uniform weight -log(n_orient) still refer to the full grid.  bioem_run is the four phases below on one
+ * context; sharded, the ranks exchange two small buffers between them (paper_1609_06634_b200/shard.py does it with
+ * torch.distributed):
+ *   bioem_run_partial          a1-a6 on the slice: one partial {m, s, BIOEM_TOPK candidates} per (image, model, chunk of orientations)
+ *   bioem_export_partials      -> all_gather over ranks (rank order = grid order)
+ *   bioem_merge_partials       the fixed-order combine of ALL ranks' partials, on every rank (a6)
+ *   bioem_rescore_local        FP64 values of the merged candidates whose orientation this rank holds, exactly 0.0 for the others (a7)
+ *   bioem_export_rescore       -> all_reduce(SUM) over ranks -> bioem_import_rescore
+ *   bioem_finish               corrected log-sum-exp, argmax, constants (a7): every rank then holds the full results.
+ * The results are bit-identical to one GPU scoring the whole grid with the same bioem_set_orientation_chunk value: the chunk
+ * partials are the same numbers and are combined in the same order.  Requirements (BIOEM_EBADSTATE / BIOEM_EBADARG otherwise):
+ * an explicit orientation chunk, the same on all ranks; o_begin a multiple of it; the per-orientation posterior disabled.
+ * set_orientation_slice(ctx, 0, -1) clears the slice.  Buffers: caller-allocated, host or device (is_device). */
+int bioem_set_orientation_slice(bioem_ctx *ctx, int o_begin, int o_end);
+int bioem_run_partial(bioem_ctx *ctx);
+/* size of this context's partials: n_bytes of the blob bioem_export_partials writes, n_chunks = chunks per model in it */
+int bioem_get_partials_size(bioem_ctx *ctx, int64_t *n_bytes, int32_t *n_chunks);
+int bioem_export_partials(bioem_ctx *ctx, void *dst, int is_device);
+/* blobs: n_blobs blobs, blob r at blobs + r * stride_bytes with chunks_of_blob[r] (host array) chunks per model, in grid order;
+ * blobs = NULL merges this context's own partials (what bioem_run does). */
+int bioem_merge_partials(bioem_ctx *ctx, int n_blobs, const void *blobs, int64_t stride_bytes, const int32_t *chunks_of_blob,
+                         int is_device);
+int bioem_rescore_local(bioem_ctx *ctx);
+/* [n_img][n_model][BIOEM_TOPK] doubles */
+int bioem_export_rescore(bioem_ctx *ctx, double *dst, int is_device);
+int bioem_import_rescore(bioem_ctx *ctx, const double *src, int is_device);
+int bioem_finish(bioem_ctx *ctx);
+
 /* ---- test / debug entry points (not on the measured path) ---- */
 /* Which fused kernel bioem_run may use: 0 automatic (packed register-resident kernel for n_pix 64 / 128 with max_shift <= 16,
  * tensor-memory kernel for n_pix 224 with max_shift <= 31, generic kernel otherwise), 1 generic kernel always, 3 the

@@ -228,6 +228,16 @@ class RunState:
         return self.m + np.log(self.s)
 
 
+def cropped_sums(obs, I1, D):
+    """Real-space cropping variant (R25): (C_co(d), C_c(d), C_cc(d)), each [2D+1][2D+1] indexed [dy+D][dx+D]."""
+    obs, op = _d(obs)
+    I1, ip = _d(I1)
+    N, S1 = obs.shape[0], 2 * D + 1
+    out = [np.empty((S1, S1)) for _ in range(3)]
+    lib().bo_cropped_sums(C.c_int(N), op, ip, C.c_int(D), *[o.ctypes.data_as(_dp) for o in out])
+    return tuple(out)
+
+
 def run_model(model, N, px, D, quats, ctfs, images, lp_orient=None, lp_ctf=None, o_begin=0, o_end=None,
               tier=0, state=None):
     """Eq. 9 on the grid for ONE model: all orientations in [o_begin, o_end) x CTFs x shifts, every image.

@@ -449,12 +449,40 @@ static void bo_acc_add(bo_acc *a, double x, long long flat)
     else if (x > a->second) a->second = x;
 }
 
+/* Real-space displacement variant ("in a real space formulation, the cross-correlation is simply calculated for
+ * different displacements d"; P:171 it "crops" the borders where the Fourier variant wraps around).  Reading R25
+ * (DESIGN.md): the calculated image displaced by d is I_d(r) = I1(r + d) where r + d lies inside the box and 0 elsewhere
+ * (the part pushed over the border is cut off, nothing re-enters on the other side), and Eq. 8 is applied to the pair
+ * (I_obs, I_d) over all n pixels.  So all three sums that involve the calculated image depend on d:
+ *   C_co(d) = sum_{r, r+d in box} I_obs(r) I1(r+d),   C_c(d) = sum_{r, r+d in box} I1(r+d),   C_cc(d) likewise with squares.
+ * Output index (dy+D)*(2D+1) + (dx+D), as bo_cross_corr_direct. */
+void bo_cropped_sums(int N, const double *obs, const double *I1, int D, double *cco, double *cc, double *ccc)
+{
+    int S1 = 2 * D + 1;
+    for (int dy = -D; dy <= D; ++dy)
+        for (int dx = -D; dx <= D; ++dx) {
+            long double s_co = 0.0L, s_c = 0.0L, s_cc = 0.0L;
+            for (int k = 0; k < N; ++k) {
+                int k2 = k + dy;
+                if (k2 < 0 || k2 >= N) continue;
+                for (int j = 0; j < N; ++j) {
+                    int j2 = j + dx;
+                    if (j2 < 0 || j2 >= N) continue;
+                    double v = I1[(size_t)k2 * N + j2];
+                    s_co += (long double)obs[(size_t)k * N + j] * v; s_c += v; s_cc += (long double)v * v;
+                }
+            }
+            size_t d = (size_t)(dy + D) * S1 + (dx + D);
+            cco[d] = (double)s_co; cc[d] = (double)s_c; ccc[d] = (double)s_cc;
+        }
+}
+
 /* Scores images against calc images (orientation o in [o_begin,o_end), all CTFs, all shifts) of ONE model and
  * folds the terms into acc[] in loop order.  lse_m/lse_s/best/second/best_flat are in/out (initialise with
  * -inf, 0, -inf, -inf, -1) so a grid can be processed in orientation chunks with identical results.
  * Per term: log P(C1) + logw,  logw = lp_o + lp_c - log S  (R7; lp_* default to -log O, -log C).
  * model_kind 0: atoms (xyz,radius,weight,Kq);  1: density spectrum (V_re,V_im,voxel_A).
- * tier: 0 = direct summation (the definition), 1 = tier B pruned DFT. */
+ * tier: 0 = direct summation (the definition), 1 = tier B pruned DFT, 2 = the real-space CROPPING variant (bo_cropped_sums, R25). */
 int bo_run(int N, double px, int D, int model_kind,
            int n_atoms, const double *xyz, const double *radius, const double *weight, int Kq,
            const double *V_re, const double *V_im, double voxel_A,
@@ -471,6 +499,8 @@ int bo_run(int N, double px, int D, int model_kind,
     double *obs = (double *)malloc(sizeof(double) * n * n_img);
     double *Co = (double *)malloc(sizeof(double) * n_img), *Coo = (double *)malloc(sizeof(double) * n_img);
     double *cco = (double *)malloc(sizeof(double) * S * n_img);
+    double *ccd = NULL, *cccd = NULL;                       /* tier 2: C_c(d), C_cc(d) per image and shift */
+    if (tier == 2) { ccd = (double *)malloc(sizeof(double) * S * n_img); cccd = (double *)malloc(sizeof(double) * S * n_img); }
     /* tier B scratch */
     double *or_ = NULL, *oi = NULL, *br = NULL, *bi = NULL, *tc = NULL, *ts = NULL;
     for (int w = 0; w < n_img; ++w) {                      /* "Eqs. S3, S5": C_o, C_oo */
@@ -508,6 +538,7 @@ int bo_run(int N, double px, int D, int model_kind,
 #pragma omp for schedule(dynamic, 1)
                 for (int w = 0; w < n_img; ++w) {
                     if (tier == 0) bo_cross_corr_direct(N, obs + (size_t)w * n, I1, D, cco + (size_t)w * S);
+                    else if (tier == 2) bo_cropped_sums(N, obs + (size_t)w * n, I1, D, cco + (size_t)w * S, ccd + (size_t)w * S, cccd + (size_t)w * S);
                     else bo_cross_corr_dft_spec(N, or_ + (size_t)w * n, oi + (size_t)w * n, br, bi, D, tc, ts, cco + (size_t)w * S, wr, wi);
                 }
                 free(wr); free(wi);
@@ -516,14 +547,15 @@ int bo_run(int N, double px, int D, int model_kind,
             for (int w = 0; w < n_img; ++w) {
                 bo_acc a = { lse_m[w], lse_s[w], best[w], second[w], best_flat[w] };
                 for (size_t d = 0; d < S; ++d) {
-                    double lp = bo_log_post_c1((double)n, Co[w], Coo[w], Cc, Ccc, cco[(size_t)w * S + d]);
+                    double lp = tier == 2 ? bo_log_post_c1((double)n, Co[w], Coo[w], ccd[(size_t)w * S + d], cccd[(size_t)w * S + d], cco[(size_t)w * S + d])
+                                          : bo_log_post_c1((double)n, Co[w], Coo[w], Cc, Ccc, cco[(size_t)w * S + d]);
                     bo_acc_add(&a, lp + logw, ((long long)o * n_ctf + c) * (long long)S + (long long)d);
                 }
                 lse_m[w] = a.m; lse_s[w] = a.s; best[w] = a.best; second[w] = a.second; best_flat[w] = a.best_flat;
             }
         }
     }
-    free(I0); free(I1); free(fr); free(fi); free(obs); free(Co); free(Coo); free(cco);
+    free(I0); free(I1); free(fr); free(fi); free(obs); free(Co); free(Coo); free(cco); free(ccd); free(cccd);
     free(or_); free(oi); free(br); free(bi); free(tc); free(ts);
     return 0;
 }

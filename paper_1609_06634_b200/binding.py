@@ -18,6 +18,8 @@ EXPORTED_SYMBOLS = [
     "bioem_debug_log_posterior_f32", "bioem_get_timing", "bioem_get_launch_count", "bioem_measure_fp32_peak",
     "bioem_set_orientation_posterior", "bioem_get_orientation_log_posterior", "bioem_get_ensemble_log_posterior",
     "bioem_set_orientation_chunk", "bioem_debug_set_kernel", "bioem_get_run_plan", "bioem_invalidate_precompute",
+    "bioem_set_orientation_slice", "bioem_run_partial", "bioem_get_partials_size", "bioem_export_partials", "bioem_merge_partials",
+    "bioem_rescore_local", "bioem_export_rescore", "bioem_import_rescore", "bioem_finish",
 ]
 KERNEL_AUTO, KERNEL_GENERIC, KERNEL_PK, KERNEL_C2, KERNEL_TM = 0, 1, 2, 3, 4
 
@@ -60,6 +62,15 @@ def lib():
         L.bioem_push_images.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_int]
         L.bioem_run.argtypes = [C.c_void_p]
         L.bioem_invalidate_precompute.argtypes = [C.c_void_p]
+        L.bioem_set_orientation_slice.argtypes = [C.c_void_p, C.c_int, C.c_int]
+        L.bioem_run_partial.argtypes = [C.c_void_p]
+        L.bioem_get_partials_size.argtypes = [C.c_void_p, C.POINTER(C.c_int64), C.POINTER(C.c_int32)]
+        L.bioem_export_partials.argtypes = [C.c_void_p, C.c_void_p, C.c_int]
+        L.bioem_merge_partials.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_int64, _ip, C.c_int]
+        L.bioem_rescore_local.argtypes = [C.c_void_p]
+        L.bioem_export_rescore.argtypes = [C.c_void_p, C.c_void_p, C.c_int]
+        L.bioem_import_rescore.argtypes = [C.c_void_p, C.c_void_p, C.c_int]
+        L.bioem_finish.argtypes = [C.c_void_p]
         L.bioem_get_log_posterior.argtypes = [C.c_void_p, _dp]
         L.bioem_get_best.argtypes = [C.c_void_p, _ip, _ip, _ip, _ip, _dp]
         L.bioem_debug_calc_image.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, _fp]
@@ -197,6 +208,57 @@ class BioEM:
     def invalidate_precompute(self):
         self._ck(self._L.bioem_invalidate_precompute(self._h))
 
+    # ---- the run in phases (orientation sharding, include/bioem.h)
+    def set_orientation_slice(self, o_begin=0, o_end=-1):
+        self._ck(self._L.bioem_set_orientation_slice(self._h, int(o_begin), int(o_end)))
+
+    def run_partial(self):
+        self._ck(self._L.bioem_run_partial(self._h))
+
+    def get_partials_size(self):
+        """(bytes of this context's partial blob, chunks per model in it)"""
+        nb, nc = C.c_int64(), C.c_int32()
+        self._ck(self._L.bioem_get_partials_size(self._h, C.byref(nb), C.byref(nc)))
+        return nb.value, nc.value
+
+    @staticmethod
+    def _buf(t):
+        """(address, is_device) of a contiguous torch tensor or numpy array"""
+        if hasattr(t, "data_ptr"):
+            assert t.is_contiguous()
+            return C.c_void_p(t.data_ptr()), 1 if t.is_cuda else 0
+        assert t.flags["C_CONTIGUOUS"]
+        return C.c_void_p(t.ctypes.data), 0
+
+    def export_partials(self, dst):
+        p, dev = self._buf(dst)
+        self._ck(self._L.bioem_export_partials(self._h, p, dev))
+
+    def merge_partials(self, blobs=None, stride_bytes=0, chunks_of_blob=None):
+        if blobs is None:
+            self._ck(self._L.bioem_merge_partials(self._h, 0, None, 0, None, 1))
+            return
+        ch = np.ascontiguousarray(chunks_of_blob, dtype=np.int32)
+        p, dev = self._buf(blobs)
+        self._ck(self._L.bioem_merge_partials(self._h, len(ch), p, int(stride_bytes), ch.ctypes.data_as(_ip), dev))
+
+    def rescore_local(self):
+        self._ck(self._L.bioem_rescore_local(self._h))
+
+    def rescore_shape(self):
+        return (self.n_img, self.n_models, TOPK)
+
+    def export_rescore(self, dst):
+        p, dev = self._buf(dst)
+        self._ck(self._L.bioem_export_rescore(self._h, p, dev))
+
+    def import_rescore(self, src):
+        p, dev = self._buf(src)
+        self._ck(self._L.bioem_import_rescore(self._h, p, dev))
+
+    def finish(self):
+        self._ck(self._L.bioem_finish(self._h))
+
     def get_log_posterior(self):
         out = np.empty((self.n_img, self.n_models))
         self._ck(self._L.bioem_get_log_posterior(self._h, out.ctypes.data_as(_dp)))
@@ -218,6 +280,12 @@ class BioEM:
 
     def get_run_plan(self):
         """(kernel, orientations per work item) of the last run."""
+        k, oc = C.c_int(), C.c_int()
+        self._ck(self._L.bioem_get_run_plan(self._h, C.byref(k), C.byref(oc)))
+        return k.value, oc.value
+
+    def get_run_plan_partial(self):
+        """(kernel, orientations per work item) after run_partial (bioem_get_run_plan needs a finished run)."""
         k, oc = C.c_int(), C.c_int()
         self._ck(self._L.bioem_get_run_plan(self._h, C.byref(k), C.byref(oc)))
         return k.value, oc.value

@@ -61,6 +61,10 @@ struct bioem_ctx {
     bool pre_valid = false;                            // a1-a3 outputs (F0, K, T_c, h, alpha) match the current models / grids / shift range
     bool want_orient = false, ran_orient = false;      // per-orientation posterior: requested / produced by the last run
     int oc_user = 0;                                   // orientations per work item (0 = automatic)
+    int slice_begin = 0, slice_end = -1;               // orientation slice this context scores; end < 0 = the whole grid
+    int phase = 0;                                     // of the phased run: 0 nothing, 1 partials, 2 merged, 3 re-scored, 4 finished (= ran)
+    int run_o_first = 0, run_o_local = 0, run_chunks = 0;     // slice and chunk count (per model, partials per item included) of the last partial run
+    DBuf blob, gathered, blob_chunks;                  // this context's partials (one blob); blobs handed to bioem_merge_partials; their chunk counts
     int kernel_user = 0;                               // BIOEM_KERNEL_*: which fused kernel bioem_run may pick (0 = automatic)
     int n_sm = 148;
     DBuf flags;                                        // int[2]: [0] bit 0 = an image without variance (a0); [1] bit 1 = an empty calculated image (a3)
@@ -69,7 +73,7 @@ struct bioem_ctx {
     DBuf logp_orient;
     int run_models = 0, run_orient = 0, run_ctf = 0, run_D = 0, run_img = 0;
     DBuf F064, F032, K64, K32, Kt, Tc64, h64, alpha32, h32;
-    DBuf part_m, part_s, part_top, m32, s32, top, g64;
+    DBuf m32, s32, top, g64;
     DBuf logp, logp32, best, best_logp;
     DBuf scratch_a, scratch_b, scratch_c, dump, staging;
     cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
@@ -127,7 +131,7 @@ int bioem_destroy(bioem_ctx *ctx)
     for (auto &m : ctx->models) { m.xyz.release(); m.rad.release(); m.wt.release(); m.rho.release(); }
     DBuf *all[] = {&ctx->rot, &ctx->lp_orient, &ctx->ctf_a, &ctx->ctf_A, &ctx->ctf_b, &ctx->lp_ctf, &ctx->Ohat64, &ctx->Ohat32, &ctx->Dw,
                    &ctx->beta, &ctx->F064, &ctx->F032, &ctx->K64, &ctx->K32, &ctx->Kt, &ctx->Tc64, &ctx->h64, &ctx->alpha32, &ctx->h32,
-                   &ctx->part_m, &ctx->part_s, &ctx->part_top, &ctx->m32, &ctx->s32, &ctx->top, &ctx->g64, &ctx->logp, &ctx->logp_orient, &ctx->logp32,
+                   &ctx->blob, &ctx->gathered, &ctx->blob_chunks, &ctx->m32, &ctx->s32, &ctx->top, &ctx->g64, &ctx->logp, &ctx->logp_orient, &ctx->logp32,
                    &ctx->best, &ctx->best_logp, &ctx->scratch_a, &ctx->scratch_b, &ctx->scratch_c, &ctx->dump, &ctx->flags, &ctx->staging};
     for (DBuf *b : all) b->release();
     for (int i = 0; i < 4; ++i) if (ctx->ev[i]) cudaEventDestroy(ctx->ev[i]);
@@ -145,7 +149,7 @@ int bioem_set_image_geometry(bioem_ctx *ctx, int n_pix, float pixel_size_A)
     ctx->N = n_pix;
     ctx->px = (double)pixel_size_A;
     ctx->n_img = 0;
-    ctx->ran = false; ctx->pre_valid = false;
+    ctx->ran = false; ctx->phase = 0; ctx->pre_valid = false;
     return BIOEM_OK;
 }
 
@@ -156,7 +160,7 @@ int bioem_clear_models(bioem_ctx *ctx)
     cudaStreamSynchronize(ctx->stream);
     for (auto &m : ctx->models) { m.xyz.release(); m.rad.release(); m.wt.release(); m.rho.release(); }
     ctx->models.clear();
-    ctx->ran = false; ctx->pre_valid = false;
+    ctx->ran = false; ctx->phase = 0; ctx->pre_valid = false;
     return BIOEM_OK;
 }
 
@@ -190,7 +194,7 @@ int bioem_add_model_atoms(bioem_ctx *ctx, int n_atoms, const float *xyz_A, const
         return rc;
     }
     if (model_id) *model_id = (int)ctx->models.size() - 1;
-    ctx->ran = false; ctx->pre_valid = false;
+    ctx->ran = false; ctx->phase = 0; ctx->pre_valid = false;
     return BIOEM_OK;
 }
 
@@ -209,7 +213,7 @@ int bioem_add_model_density(bioem_ctx *ctx, int n_vox, float voxel_A, const floa
     if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
     if (e != cudaSuccess) { m.rho.release(); ctx->models.pop_back(); CK(e); }
     if (model_id) *model_id = (int)ctx->models.size() - 1;
-    ctx->ran = false; ctx->pre_valid = false;
+    ctx->ran = false; ctx->phase = 0; ctx->pre_valid = false;
     return BIOEM_OK;
 }
 
@@ -237,7 +241,7 @@ int bioem_set_orientations_quat(bioem_ctx *ctx, int n, const float *q, const flo
         if ((rc = upload_doubles(ctx, ctx->lp_orient, lp))) return rc;
     }
     ctx->n_orient = n;
-    ctx->ran = false; ctx->pre_valid = false;
+    ctx->ran = false; ctx->phase = 0; ctx->pre_valid = false;
     return BIOEM_OK;
 }
 
@@ -260,7 +264,7 @@ int bioem_set_ctf_grid(bioem_ctx *ctx, int n, const float *a, const float *A, co
         if ((rc = upload_doubles(ctx, ctx->lp_ctf, lp))) return rc;
     }
     ctx->n_ctf = n;
-    ctx->ran = false; ctx->pre_valid = false;
+    ctx->ran = false; ctx->phase = 0; ctx->pre_valid = false;
     return BIOEM_OK;
 }
 
@@ -280,7 +284,7 @@ int bioem_set_shift_range(bioem_ctx *ctx, int max_shift_px)
     if (max_shift_px < 0) FAIL(BIOEM_EBADARG, "set_shift_range: negative");
     if (ctx->N && 2 * max_shift_px + 1 > ctx->N) FAIL(BIOEM_EBADARG, "set_shift_range: 2D+1 exceeds n_pix");
     ctx->D = max_shift_px;
-    ctx->ran = false; ctx->pre_valid = false;
+    ctx->ran = false; ctx->phase = 0; ctx->pre_valid = false;
     return BIOEM_OK;
 }
 
@@ -326,7 +330,7 @@ int bioem_push_images(bioem_ctx *ctx, int n_img, const float *pixels, int is_dev
     }
     ctx->push_launches = 4 * (int64_t)((n_img + slab - 1) / slab) + 2;
     ctx->n_img = n_img;
-    ctx->ran = false;
+    ctx->ran = false; ctx->phase = 0;
     return BIOEM_OK;
 }
 
@@ -352,28 +356,44 @@ static int choose_kernel(int N, int D, int user)
     return KERNEL_GENERIC;
 }
 
-int bioem_run(bioem_ctx *ctx)
+// ---- the run in phases.  bioem_run = all four on one context; ranks that shard the ORIENTATION grid (the paper's MPI axis,
+// P:199) run phase 1 on their slice, exchange the partials, run phase 2 on all of them, phase 3 on the candidates they
+// own, exchange the re-scored values, and phase 4 (paper_1609_06634_b200/shard.py: run_orientation_sharded).
+static int run_checks(bioem_ctx *ctx)
 {
-    if (!ctx) return BIOEM_EBADARG;
     if (!ctx->N) FAIL(BIOEM_EBADSTATE, "run: image geometry not set");
     if (ctx->models.empty()) FAIL(BIOEM_EBADSTATE, "run: no model");
     if (!ctx->n_orient) FAIL(BIOEM_EBADSTATE, "run: no orientations");
     if (!ctx->n_ctf) FAIL(BIOEM_EBADSTATE, "run: no CTF grid");
     if (ctx->D < 0) FAIL(BIOEM_EBADSTATE, "run: shift range not set");
     if (!ctx->n_img) FAIL(BIOEM_EBADSTATE, "run: no images");
-    const int N = ctx->N, D = ctx->D, O = ctx->n_orient, C = ctx->n_ctf, I = ctx->n_img, M = (int)ctx->models.size();
+    const int N = ctx->N, D = ctx->D;
     if (2 * D + 1 > N) FAIL(BIOEM_EBADARG, "run: 2D+1 exceeds n_pix");
-    if ((long long)O * C > 0x7fffffffLL) FAIL(BIOEM_EUNSUPPORTED, "run: orientations x CTFs exceeds 2^31");
+    if ((long long)ctx->n_orient * ctx->n_ctf > 0x7fffffffLL) FAIL(BIOEM_EUNSUPPORTED, "run: orientations x CTFs exceeds 2^31");
     if (fused_smem_bytes(N, D) == 0) FAIL(BIOEM_EUNSUPPORTED, "run: shift range too large for the shared-memory plan at this n_pix");
     for (auto &m : ctx->models)
         if (m.kind == 1 && (m.n_vox != N || std::fabs(m.voxel - ctx->px) > 1e-9 * ctx->px))
             FAIL(BIOEM_EUNSUPPORTED, "run: density model needs n_vox == n_pix and voxel_A == pixel_size_A (R21)");
+    return BIOEM_OK;
+}
+
+int bioem_run_partial(bioem_ctx *ctx)
+{
+    if (!ctx) return BIOEM_EBADARG;
+    int rc = run_checks(ctx);
+    if (rc) return rc;
+    const int N = ctx->N, D = ctx->D, Ofull = ctx->n_orient, C = ctx->n_ctf, I = ctx->n_img, M = (int)ctx->models.size();
+    const bool sliced = ctx->slice_end >= 0;
+    const int o_first = sliced ? ctx->slice_begin : 0, O = (sliced ? ctx->slice_end : Ofull) - o_first;      // resident orientations
+    if (sliced && (o_first < 0 || O < 0 || o_first + O > Ofull)) FAIL(BIOEM_EBADARG, "run: orientation slice outside the grid");
+    if (sliced && ctx->want_orient) FAIL(BIOEM_EUNSUPPORTED, "run: the per-orientation posterior is not available on an orientation slice");
     CK(cudaSetDevice(ctx->device));
     cudaStream_t st = ctx->stream;
     const size_t n = (size_t)N * N, H = (size_t)(N / 2 + 1) * N;
     const size_t MO = (size_t)M * O, MOC = MO * C;
-    ctx->ran = false;
+    ctx->ran = false; ctx->phase = 0;
     ctx->launches = 0; ctx->fused_launches = 0;
+    if (ctx->run_o_first != o_first || ctx->run_o_local != O) ctx->pre_valid = false;     // the cache holds another slice
 
     CK(ctx->F064.ensure(MO * H * sizeof(cd)));
     CK(ctx->F032.ensure(MO * H * sizeof(cf)));
@@ -385,22 +405,15 @@ int bioem_run(bioem_ctx *ctx)
     CK(ctx->h32.ensure(MOC * sizeof(float)));
     const int kern = choose_kernel(N, D, ctx->kernel_user);
     const bool use_pk = kern == KERNEL_PK, use_c2 = kern == KERNEL_C2, use_tm = kern == KERNEL_TM;
-    int oc = ctx->oc_user > 0 ? std::min(ctx->oc_user, O) : choose_oc(I, M, O, ctx->n_sm);
+    // an orientation slice leaves the chunk size to the caller: every rank must cut the grid at the same places
+    if (sliced && ctx->oc_user <= 0) FAIL(BIOEM_EBADSTATE, "run: set_orientation_chunk before scoring an orientation slice (all ranks the same value)");
+    int oc = ctx->oc_user > 0 ? std::min(ctx->oc_user, Ofull) : choose_oc(I, M, Ofull, ctx->n_sm);
     if (ctx->want_orient) oc = 1;                                         // one orientation per work item when its posterior is wanted
+    if (sliced && o_first % oc != 0) FAIL(BIOEM_EBADARG, "run: an orientation slice must begin at a multiple of the orientation chunk");
     const int cpm = (O + oc - 1) / oc;
     const int ppi = use_c2 ? 2 : 1;                                       // partials per work item (the cluster kernel writes one per CTA)
-    const size_t items = (size_t)I * M * cpm * ppi, IM = (size_t)I * M;
-    CK(ctx->part_m.ensure(items * sizeof(float)));
-    CK(ctx->part_s.ensure(items * sizeof(float)));
-    CK(ctx->part_top.ensure(items * BIOEM_TOPK * sizeof(TopEntry)));
-    CK(ctx->m32.ensure(IM * sizeof(double)));
-    CK(ctx->s32.ensure(IM * sizeof(double)));
-    CK(ctx->top.ensure(IM * BIOEM_TOPK * sizeof(TopEntry)));
-    CK(ctx->g64.ensure(IM * BIOEM_TOPK * sizeof(double)));
-    CK(ctx->logp.ensure(IM * sizeof(double)));
-    CK(ctx->logp32.ensure(IM * sizeof(double)));
-    CK(ctx->best.ensure(IM * 4 * sizeof(int32_t)));
-    CK(ctx->best_logp.ensure(IM * sizeof(double)));
+    const size_t items = (size_t)I * M * cpm * ppi;
+    CK(ctx->blob.ensure(partial_blob_bytes(items)));
 
     CK(cudaEventRecord(ctx->ev[0], st));
     if (!ctx->pre_valid) CK(cudaMemsetAsync(ctx->flags.as<int>() + 1, 0, sizeof(int), st));
@@ -424,9 +437,10 @@ int bioem_run(bioem_ctx *ctx)
             ctx->launches += 1;
         }
 
-        // ---- a1/a1' + a2: spectra of all projections, model by model, orientation batch by batch
+        // ---- a1/a1' + a2: spectra of the projections of the resident orientations, model by model, batch by batch
         const int OB = 256;
-        for (int mi = 0; mi < M; ++mi) {
+        const double *rot = ctx->rot.as<double>() + (size_t)o_first * 9;
+        for (int mi = 0; mi < M && O > 0; ++mi) {
             Model &m = ctx->models[mi];
             cd *F64m = ctx->F064.as<cd>() + (size_t)mi * O * H;
             if (m.kind == 0) {
@@ -439,7 +453,7 @@ int bioem_run(bioem_ctx *ctx)
                 const double fx_scale = std::ldexp(1.0, 60 - ex);
                 for (int o0 = 0; o0 < O; o0 += OB) {
                     const int nb = std::min(OB, O - o0);
-                    CK(launch_project_atoms(m.xyz.as<double>(), m.rad.as<double>(), m.wt.as<double>(), m.n_atoms, ctx->rot.as<double>() + (size_t)o0 * 9,
+                    CK(launch_project_atoms(m.xyz.as<double>(), m.rad.as<double>(), m.wt.as<double>(), m.n_atoms, rot + (size_t)o0 * 9,
                                             nb, N, ctx->px, fx_scale, ctx->scratch_c.as<long long>(), ctx->scratch_a.as<double>(), st));
                     CK(launch_fft2_r2c_f64(ctx->scratch_a.as<double>(), nb, N, ctx->scratch_b.as<cd>(), F64m + (size_t)o0 * H, st));
                     ctx->launches += 4;
@@ -449,57 +463,198 @@ int bioem_run(bioem_ctx *ctx)
                 CK(ctx->scratch_a.ensure(n3 * sizeof(cd)));
                 CK(ctx->scratch_b.ensure(n3 * sizeof(cd)));
                 CK(launch_dft3_f64(m.rho.as<float>(), N, ctx->scratch_a.as<cd>(), ctx->scratch_b.as<cd>(), st));
-                CK(launch_slice_f64(ctx->scratch_a.as<cd>(), N, m.voxel, ctx->rot.as<double>(), O, F64m, st));
+                CK(launch_slice_f64(ctx->scratch_a.as<cd>(), N, m.voxel, rot, O, F64m, st));
                 ctx->launches += 6;
             }
         }
-        CK(launch_cast_spectrum(ctx->F064.as<cd>(), ctx->F032.as<cf>(), MO * H, st));
-        CK(launch_calc_stats(ctx->F064.as<cd>(), ctx->K64.as<double>(), (int)MO, O, C, N, ctx->has_lp_orient ? ctx->lp_orient.as<double>() : nullptr,
-                             ctx->has_lp_ctf ? ctx->lp_ctf.as<double>() : nullptr, std::log((double)(2 * D + 1) * (2 * D + 1)),
-                             ctx->Tc64.as<double>(), ctx->h64.as<double>(), ctx->alpha32.as<float>(), ctx->h32.as<float>(), ctx->flags.as<int>() + 1, st));
-        ctx->launches += 2;
-
+        if (O > 0) {
+            CK(launch_cast_spectrum(ctx->F064.as<cd>(), ctx->F032.as<cf>(), MO * H, st));
+            CK(launch_calc_stats(ctx->F064.as<cd>(), ctx->K64.as<double>(), (int)MO, O, Ofull, C, N,
+                                 ctx->has_lp_orient ? ctx->lp_orient.as<double>() + o_first : nullptr,
+                                 ctx->has_lp_ctf ? ctx->lp_ctf.as<double>() : nullptr, std::log((double)(2 * D + 1) * (2 * D + 1)),
+                                 ctx->Tc64.as<double>(), ctx->h64.as<double>(), ctx->alpha32.as<float>(), ctx->h32.as<float>(), ctx->flags.as<int>() + 1, st));
+            ctx->launches += 2;
+        }
     }
 
     // ---- a4-a6: the fused kernel
     FusedParams p{};
     p.Ohat = ctx->Ohat32.as<cf>(); p.F0 = ctx->F032.as<cf>(); p.K = ctx->K32.as<float>();
     p.alpha = ctx->alpha32.as<float>(); p.hterm = ctx->h32.as<float>(); p.beta = ctx->beta.as<float>();
-    p.n_img = I; p.n_model = M; p.n_orient = O; p.n_ctf = C; p.D = D; p.oc = oc; p.chunks_per_model = cpm;
+    p.n_img = I; p.n_model = M; p.n_orient = O; p.n_ctf = C; p.D = D; p.oc = oc; p.chunks_per_model = cpm; p.o_first = o_first;
     p.cA = (float)(-0.5 * ((double)n - 3.0) * 1.4426950408889634);
-    p.part_m = ctx->part_m.as<float>(); p.part_s = ctx->part_s.as<float>(); p.part_top = ctx->part_top.as<TopEntry>();
+    p.part_m = ctx->blob.as<float>(); p.part_s = p.part_m + items; p.part_top = reinterpret_cast<TopEntry *>(p.part_s + items);
     CK(cudaEventRecord(ctx->ev[1], st));
     int nl = 1;
-    if (use_pk) CK(launch_fused_pk(N, p, ctx->Kt.as<float>(), false, st));
+    if (items == 0) nl = 0;
+    else if (use_pk) CK(launch_fused_pk(N, p, ctx->Kt.as<float>(), false, st));
     else if (use_c2) CK(launch_fused_c2(p, ctx->Kt.as<float>(), false, st));
     else if (use_tm) CK(launch_fused_tm(p, ctx->Kt.as<float>(), false, st));
     else CK(launch_fused(N, p, false, st, &nl));
     CK(cudaEventRecord(ctx->ev[2], st));
     ctx->launches += nl; ctx->fused_launches += nl;
+    ctx->pre_valid = true;
+    ctx->flags_checked = false;
+    ctx->run_kernel = kern; ctx->run_oc = oc; ctx->run_o_first = o_first; ctx->run_o_local = O; ctx->run_chunks = cpm * ppi;
+    ctx->run_models = M; ctx->run_orient = Ofull; ctx->run_ctf = C; ctx->run_D = D; ctx->run_img = I;
+    ctx->phase = 1;
+    return BIOEM_OK;
+}
 
-    // ---- a6 combine, a7 re-score, results
-    CK(launch_merge(p.part_m, p.part_s, p.part_top, I, M, cpm * ppi, ctx->m32.as<double>(), ctx->s32.as<double>(), ctx->top.as<TopEntry>(), st));
+int bioem_get_partials_size(bioem_ctx *ctx, int64_t *n_bytes, int32_t *n_chunks)
+{
+    if (!ctx) return BIOEM_EBADARG;
+    if (ctx->phase < 1) FAIL(BIOEM_EBADSTATE, "get_partials_size: call bioem_run_partial first");
+    if (n_bytes) *n_bytes = (int64_t)partial_blob_bytes((size_t)ctx->run_img * ctx->run_models * ctx->run_chunks);
+    if (n_chunks) *n_chunks = ctx->run_chunks;
+    return BIOEM_OK;
+}
+
+int bioem_export_partials(bioem_ctx *ctx, void *dst, int is_device)
+{
+    if (!ctx || !dst) return BIOEM_EBADARG;
+    if (ctx->phase < 1) FAIL(BIOEM_EBADSTATE, "export_partials: call bioem_run_partial first");
+    CK(cudaSetDevice(ctx->device));
+    const size_t bytes = partial_blob_bytes((size_t)ctx->run_img * ctx->run_models * ctx->run_chunks);
+    if (bytes) CK(cudaMemcpyAsync(dst, ctx->blob.p, bytes, is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, ctx->stream));
+    CK(cudaStreamSynchronize(ctx->stream));
+    return BIOEM_OK;
+}
+
+// a6: the fixed-order combine over `n_blobs` blobs (NULL = this context's own partials)
+int bioem_merge_partials(bioem_ctx *ctx, int n_blobs, const void *blobs, int64_t stride_bytes, const int32_t *chunks_of_blob, int is_device)
+{
+    if (!ctx) return BIOEM_EBADARG;
+    if (ctx->phase < 1) FAIL(BIOEM_EBADSTATE, "merge_partials: call bioem_run_partial first");
+    CK(cudaSetDevice(ctx->device));
+    cudaStream_t st = ctx->stream;
+    const int I = ctx->run_img, M = ctx->run_models;
+    const size_t IM = (size_t)I * M;
+    CK(ctx->m32.ensure(IM * sizeof(double)));
+    CK(ctx->s32.ensure(IM * sizeof(double)));
+    CK(ctx->top.ensure(IM * BIOEM_TOPK * sizeof(TopEntry)));
+    const unsigned char *src = nullptr;
+    std::vector<int> chunks;
+    if (!blobs) {
+        n_blobs = 1; stride_bytes = 0; chunks.assign(1, ctx->run_chunks);
+        src = ctx->blob.as<unsigned char>();
+    } else {
+        if (n_blobs < 1 || !chunks_of_blob || stride_bytes < 0 || stride_bytes % 4) FAIL(BIOEM_EBADARG, "merge_partials: n_blobs < 1, NULL chunk counts or a stride that is not a multiple of 4");
+        long long tot = 0;
+        for (int r = 0; r < n_blobs; ++r) {
+            if (chunks_of_blob[r] < 0 || (int64_t)partial_blob_bytes(IM * chunks_of_blob[r]) > stride_bytes) FAIL(BIOEM_EBADARG, "merge_partials: a blob does not fit its stride");
+            chunks.push_back(chunks_of_blob[r]);
+            tot += chunks_of_blob[r];
+        }
+        if (is_device) src = static_cast<const unsigned char *>(blobs);
+        else {
+            CK(ctx->gathered.ensure((size_t)n_blobs * stride_bytes));
+            CK(cudaMemcpyAsync(ctx->gathered.p, blobs, (size_t)n_blobs * stride_bytes, cudaMemcpyHostToDevice, st));
+            src = ctx->gathered.as<unsigned char>();
+        }
+    }
+    CK(ctx->blob_chunks.ensure(chunks.size() * sizeof(int)));
+    CK(cudaMemcpyAsync(ctx->blob_chunks.p, chunks.data(), chunks.size() * sizeof(int), cudaMemcpyHostToDevice, st));
+    CK(launch_merge(src, (size_t)stride_bytes, ctx->blob_chunks.as<int>(), n_blobs, I, M, ctx->m32.as<double>(), ctx->s32.as<double>(),
+                    ctx->top.as<TopEntry>(), st));
+    CK(cudaStreamSynchronize(st));                               // `chunks` (and a host `blobs`) may go away
+    ctx->launches += 1;
+    ctx->phase = 2;
+    return BIOEM_OK;
+}
+
+// a7, first half: FP64 values of the merged candidates whose orientation is resident here; 0 for the others
+int bioem_rescore_local(bioem_ctx *ctx)
+{
+    if (!ctx) return BIOEM_EBADARG;
+    if (ctx->phase < 2) FAIL(BIOEM_EBADSTATE, "rescore_local: call bioem_merge_partials first");
+    CK(cudaSetDevice(ctx->device));
+    const int I = ctx->run_img, M = ctx->run_models;
+    CK(ctx->g64.ensure((size_t)I * M * BIOEM_TOPK * sizeof(double)));
     CK(launch_rescore(ctx->Ohat64.as<cd>(), ctx->F064.as<cd>(), ctx->K64.as<double>(), ctx->Tc64.as<double>(), ctx->h64.as<double>(),
-                      ctx->Dw.as<double>(), ctx->top.as<TopEntry>(), BIOEM_TOPK, I, M, O, C, N, D, -1, ctx->g64.as<double>(), st));
-    const double nn = (double)n;
+                      ctx->Dw.as<double>(), ctx->top.as<TopEntry>(), BIOEM_TOPK, I, M, ctx->run_o_local, ctx->run_ctf, ctx->N, ctx->run_D, -1,
+                      ctx->run_o_first, ctx->g64.as<double>(), ctx->stream));
+    ctx->launches += 1;
+    ctx->phase = 3;
+    return BIOEM_OK;
+}
+
+int bioem_export_rescore(bioem_ctx *ctx, double *dst, int is_device)
+{
+    if (!ctx || !dst) return BIOEM_EBADARG;
+    if (ctx->phase < 3) FAIL(BIOEM_EBADSTATE, "export_rescore: call bioem_rescore_local first");
+    CK(cudaSetDevice(ctx->device));
+    CK(cudaMemcpyAsync(dst, ctx->g64.p, (size_t)ctx->run_img * ctx->run_models * BIOEM_TOPK * sizeof(double),
+                       is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, ctx->stream));
+    CK(cudaStreamSynchronize(ctx->stream));
+    return BIOEM_OK;
+}
+
+int bioem_import_rescore(bioem_ctx *ctx, const double *src, int is_device)
+{
+    if (!ctx || !src) return BIOEM_EBADARG;
+    if (ctx->phase < 3) FAIL(BIOEM_EBADSTATE, "import_rescore: call bioem_rescore_local first");
+    CK(cudaSetDevice(ctx->device));
+    CK(cudaMemcpyAsync(ctx->g64.p, src, (size_t)ctx->run_img * ctx->run_models * BIOEM_TOPK * sizeof(double),
+                       is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, ctx->stream));
+    CK(cudaStreamSynchronize(ctx->stream));
+    return BIOEM_OK;
+}
+
+// a7, second half: corrected log-sum-exp, argmax, constants
+int bioem_finish(bioem_ctx *ctx)
+{
+    if (!ctx) return BIOEM_EBADARG;
+    if (ctx->phase < 3) FAIL(BIOEM_EBADSTATE, "finish: call bioem_rescore_local first");
+    CK(cudaSetDevice(ctx->device));
+    cudaStream_t st = ctx->stream;
+    const int I = ctx->run_img, M = ctx->run_models, N = ctx->N;
+    const size_t IM = (size_t)I * M;
+    CK(ctx->logp.ensure(IM * sizeof(double)));
+    CK(ctx->logp32.ensure(IM * sizeof(double)));
+    CK(ctx->best.ensure(IM * 4 * sizeof(int32_t)));
+    CK(ctx->best_logp.ensure(IM * sizeof(double)));
+    const double nn = (double)N * N;
     const double const_n = -0.5 * (nn - 2.0) * std::log(2.0 * M_PI) + 0.5 * (nn - 5.0) * std::log(2.0) + std::lgamma(0.5 * (nn - 3.0));
     CK(launch_final(ctx->m32.as<double>(), ctx->s32.as<double>(), ctx->top.as<TopEntry>(), ctx->g64.as<double>(), ctx->Dw.as<double>(), I, M,
-                    C, N, D, const_n, ctx->logp.as<double>(), ctx->logp32.as<double>(), ctx->best.as<int32_t>(), ctx->best_logp.as<double>(), st));
-    ctx->launches += 3;
+                    ctx->run_ctf, N, ctx->run_D, const_n, ctx->logp.as<double>(), ctx->logp32.as<double>(), ctx->best.as<int32_t>(),
+                    ctx->best_logp.as<double>(), st));
+    ctx->launches += 1;
     ctx->ran_orient = false;
     if (ctx->want_orient) {
-        CK(ctx->logp_orient.ensure(IM * O * sizeof(double)));
-        CK(launch_orient_final(p.part_m, p.part_s, ppi, ctx->top.as<TopEntry>(), ctx->g64.as<double>(), ctx->Dw.as<double>(), I, M, O, C, N,
-                               const_n, ctx->logp_orient.as<double>(), st));
+        const size_t items = IM * ctx->run_chunks;
+        const float *part_m = ctx->blob.as<float>(), *part_s = part_m + items;
+        CK(ctx->logp_orient.ensure(IM * ctx->run_orient * sizeof(double)));
+        CK(launch_orient_final(part_m, part_s, ctx->run_kernel == KERNEL_C2 ? 2 : 1, ctx->top.as<TopEntry>(), ctx->g64.as<double>(), ctx->Dw.as<double>(), I, M,
+                               ctx->run_orient, ctx->run_ctf, N, const_n, ctx->logp_orient.as<double>(), st));
         ctx->launches += 1;
         ctx->ran_orient = true;
     }
     CK(cudaEventRecord(ctx->ev[3], st));
     ctx->ran = true;
-    ctx->pre_valid = true;
-    ctx->flags_checked = false;
-    ctx->run_kernel = kern; ctx->run_oc = oc;
-    ctx->run_models = M; ctx->run_orient = O; ctx->run_ctf = C; ctx->run_D = D; ctx->run_img = I;
+    ctx->phase = 4;
+    return BIOEM_OK;
+}
+
+int bioem_run(bioem_ctx *ctx)
+{
+    if (!ctx) return BIOEM_EBADARG;
+    if (ctx->slice_end >= 0 && !(ctx->slice_begin == 0 && ctx->slice_end == ctx->n_orient))
+        FAIL(BIOEM_EBADSTATE, "run: an orientation slice is set: this context holds part of the grid (use the phased calls, or clear the slice)");
+    int rc = bioem_run_partial(ctx);
+    if (!rc) rc = bioem_merge_partials(ctx, 0, nullptr, 0, nullptr, 1);
+    if (!rc) rc = bioem_rescore_local(ctx);
+    if (!rc) rc = bioem_finish(ctx);
+    return rc;
+}
+
+int bioem_set_orientation_slice(bioem_ctx *ctx, int o_begin, int o_end)
+{
+    if (!ctx) return BIOEM_EBADARG;
+    if (o_end >= 0 && (o_begin < 0 || o_begin > o_end)) FAIL(BIOEM_EBADARG, "set_orientation_slice: need 0 <= o_begin <= o_end (o_end < 0 clears the slice)");
+    ctx->slice_begin = o_end < 0 ? 0 : o_begin;
+    ctx->slice_end = o_end < 0 ? -1 : o_end;
+    ctx->ran = false; ctx->phase = 0; ctx->pre_valid = false;
     return BIOEM_OK;
 }
 
@@ -512,7 +667,7 @@ static int check_run_flags(bioem_ctx *ctx)
     CK(cudaMemcpyAsync(&fl, ctx->flags.as<int>() + 1, sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
     CK(cudaStreamSynchronize(ctx->stream));
     if (fl & 2) {
-        ctx->ran = false; ctx->pre_valid = false;
+        ctx->ran = false; ctx->phase = 0; ctx->pre_valid = false;
         FAIL(BIOEM_EBADARG, "run: a calculated image is empty or not finite (T_c = sum |I1|^2 is not > 0): its posterior is undefined");
     }
     ctx->flags_checked = true;
@@ -604,9 +759,9 @@ int bioem_get_best(bioem_ctx *ctx, int32_t *orient_idx, int32_t *ctf_idx, int32_
 static int check_tuple(bioem_ctx *ctx, int img, int model, int orient, int ctf)
 {
     if (!ctx->ran) FAIL(BIOEM_EBADSTATE, "debug: call bioem_run first (the precomputed spectra are reused)");
-    if (img < 0 || img >= ctx->run_img || model < 0 || model >= ctx->run_models || orient < 0 || orient >= ctx->run_orient || ctf < 0 ||
-        ctf >= ctx->run_ctf)
-        FAIL(BIOEM_EBADARG, "debug: index out of range");
+    if (img < 0 || img >= ctx->run_img || model < 0 || model >= ctx->run_models || orient < ctx->run_o_first ||
+        orient >= ctx->run_o_first + ctx->run_o_local || ctf < 0 || ctf >= ctx->run_ctf)
+        FAIL(BIOEM_EBADARG, "debug: index out of range (or an orientation outside this context's slice)");
     return BIOEM_OK;
 }
 
@@ -619,7 +774,7 @@ int bioem_debug_calc_image(bioem_ctx *ctx, int model, int orient, int ctf, float
     const int N = ctx->N;
     const size_t n = (size_t)N * N, H = (size_t)(N / 2 + 1) * N;
     CK(ctx->dump.ensure(n * sizeof(double)));
-    CK(launch_calc_image(ctx->F064.as<cd>() + ((size_t)model * ctx->run_orient + orient) * H, ctx->K64.as<double>() + (size_t)ctf * H, N,
+    CK(launch_calc_image(ctx->F064.as<cd>() + ((size_t)model * ctx->run_o_local + (orient - ctx->run_o_first)) * H, ctx->K64.as<double>() + (size_t)ctf * H, N,
                          ctx->dump.as<double>(), ctx->stream));
     std::vector<double> tmp(n);
     rc = fetch(ctx, tmp.data(), ctx->dump.p, n * sizeof(double));
@@ -640,10 +795,11 @@ int bioem_debug_shift_map(bioem_ctx *ctx, int img, int model, int orient, int ct
     FusedParams p{};
     p.Ohat = ctx->Ohat32.as<cf>(); p.F0 = ctx->F032.as<cf>(); p.K = ctx->K32.as<float>();
     p.alpha = ctx->alpha32.as<float>(); p.hterm = ctx->h32.as<float>(); p.beta = ctx->beta.as<float>();
-    p.n_img = ctx->run_img; p.n_model = ctx->run_models; p.n_orient = ctx->run_orient; p.n_ctf = ctx->run_ctf; p.D = D; p.oc = 1;
+    p.n_img = ctx->run_img; p.n_model = ctx->run_models; p.n_orient = ctx->run_o_local; p.n_ctf = ctx->run_ctf; p.D = D; p.oc = 1;
+    p.o_first = ctx->run_o_first;
     p.chunks_per_model = 1;
     p.cA = (float)(-0.5 * ((double)n - 3.0) * 1.4426950408889634);
-    p.dump = ctx->dump.as<float>(); p.dump_img = img; p.dump_model = model; p.dump_orient = orient; p.dump_ctf = ctf;
+    p.dump = ctx->dump.as<float>(); p.dump_img = img; p.dump_model = model; p.dump_orient = orient - ctx->run_o_first; p.dump_ctf = ctf;
     if (ctx->run_kernel == KERNEL_PK) CK(launch_fused_pk(N, p, ctx->Kt.as<float>(), true, ctx->stream));
     else if (ctx->run_kernel == KERNEL_C2) CK(launch_fused_c2(p, ctx->Kt.as<float>(), true, ctx->stream));
     else if (ctx->run_kernel == KERNEL_TM) CK(launch_fused_tm(p, ctx->Kt.as<float>(), true, ctx->stream));
@@ -679,7 +835,7 @@ int bioem_debug_shift_map_f64(bioem_ctx *ctx, int img, int model, int orient, in
     if (e == cudaSuccess)
         e = launch_rescore(ctx->Ohat64.as<cd>() + (size_t)img * (size_t)(N / 2 + 1) * N, ctx->F064.as<cd>(), ctx->K64.as<double>(),
                            ctx->Tc64.as<double>(), ctx->h64.as<double>(), ctx->Dw.as<double>() + img, dc.as<TopEntry>(), S, 1, ctx->run_models,
-                           ctx->run_orient, ctx->run_ctf, N, D, model, dg.as<double>(), ctx->stream);
+                           ctx->run_o_local, ctx->run_ctf, N, D, model, ctx->run_o_first, dg.as<double>(), ctx->stream);
     std::vector<double> g(S), dw(1);
     if (e == cudaSuccess) e = cudaMemcpyAsync(g.data(), dg.p, S * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream);
     if (e == cudaSuccess) e = cudaMemcpyAsync(dw.data(), ctx->Dw.as<double>() + img, sizeof(double), cudaMemcpyDeviceToHost, ctx->stream);
@@ -719,7 +875,7 @@ int bioem_invalidate_precompute(bioem_ctx *ctx)
 int bioem_get_run_plan(bioem_ctx *ctx, int *kernel, int *n_orient_per_item)
 {
     if (!ctx) return BIOEM_EBADARG;
-    if (!ctx->ran) FAIL(BIOEM_EBADSTATE, "get_run_plan: no completed run");
+    if (!ctx->ran && ctx->phase < 1) FAIL(BIOEM_EBADSTATE, "get_run_plan: no run yet");
     if (kernel) *kernel = ctx->run_kernel;
     if (n_orient_per_item) *n_orient_per_item = ctx->run_oc;
     return BIOEM_OK;

@@ -36,6 +36,7 @@ struct FusedParams {
     const float *beta;     // [I]       1/sqrt(D_omega)
     int n_img, n_model, n_orient, n_ctf, D;
     int oc;                // orientations per work item (chunk)
+    int o_first;           // index in the FULL orientation grid of local orientation 0 (orientation sharding); candidates carry global indices
     int chunks_per_model;
     float cA;              // -(n-3)/2 * log2(e)
     // outputs: one partial per work item = (model, chunk, image)
@@ -77,17 +78,19 @@ cudaError_t launch_dft3_f64(const float *rho, int N, cd *work_a, cd *work_b, cud
 cudaError_t launch_slice_f64(const cd *Vc, int N, double voxel, const double *rot, int n_orient, cd *out, cudaStream_t st);
 cudaError_t launch_ctf_tables(const double *a, const double *A, const double *b, int n_ctf, int N, double px,
                               double *K64, float *K32, cudaStream_t st);
-cudaError_t launch_calc_stats(const cd *F0, const double *K64, int n_mo, int n_orient, int n_ctf, int N,
+cudaError_t launch_calc_stats(const cd *F0, const double *K64, int n_mo, int n_orient, int n_orient_total, int n_ctf, int N,
                               const double *lp_orient, const double *lp_ctf, double log_shifts,
                               double *Tc64, double *h64, float *alpha32, float *h32, int *flags, cudaStream_t st);
 cudaError_t launch_beta(const double *Dw, int n_img, float *beta, int *flags, cudaStream_t st);
 
 // finalise
-cudaError_t launch_merge(const float *part_m, const float *part_s, const TopEntry *part_top, int n_img, int n_model,
-                         int chunks_per_model, double *m32, double *s32, TopEntry *top, cudaStream_t st);
+// per-work-item partials travel as one blob: float m[n], float s[n], TopEntry top[n][TOPK], n = n_model * chunks * n_img
+inline size_t partial_blob_bytes(size_t n_items) { return n_items * (2 * sizeof(float) + BIOEM_TOPK * sizeof(TopEntry)); }
+cudaError_t launch_merge(const unsigned char *blobs, size_t stride, const int *chunks_of_blob, int n_blobs, int n_img, int n_model,
+                         double *m32, double *s32, TopEntry *top, cudaStream_t st);
 cudaError_t launch_rescore(const cd *Ohat64, const cd *F064, const double *K64, const double *Tc64, const double *h64,
                            const double *Dw, const TopEntry *cand, int n_cand_per, int n_img, int n_model, int n_orient,
-                           int n_ctf, int N, int D, int cand_model_fixed, double *g64, cudaStream_t st);
+                           int n_ctf, int N, int D, int cand_model_fixed, int o_first, double *g64, cudaStream_t st);
 cudaError_t launch_final(const double *m32, const double *s32, const TopEntry *top, const double *g64, const double *Dw,
                          int n_img, int n_model, int n_ctf, int N, int D, double const_n, double *logp, double *logp32,
                          int32_t *best, double *best_logp, cudaStream_t st);

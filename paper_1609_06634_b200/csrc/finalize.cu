@@ -12,8 +12,12 @@ __device__ __forceinline__ bool before(const TopEntry &a, const TopEntry &b)
     return a.g > b.g || (a.g == b.g && (a.pair < b.pair || (a.pair == b.pair && a.shift < b.shift)));
 }
 
-// One thread per (image, model): combine chunk partials in chunk order (bit-reproducible).
-__global__ void k_merge(const float *part_m, const float *part_s, const TopEntry *part_top, int n_img, int n_model, int cpm, double *m32,
+// One thread per (image, model): combine the per-work-item partials in chunk order (bit-reproducible).  The partials arrive as
+// `n_blobs` blobs of `stride` bytes (one per rank when the orientation grid is sharded; one otherwise), blob r
+// holding chunks_of_blob[r] chunks per model: float m[n_r], float s[n_r], TopEntry top[n_r][TOPK], n_r = n_model * chunks * n_img,
+// item = (model * chunks + chunk) * n_img + img.  Blobs in rank order = chunks in grid order, so the sums and the candidate
+// lists come out exactly as on one GPU with the same chunking.
+__global__ void k_merge(const unsigned char *blobs, size_t stride, const int *chunks_of_blob, int n_blobs, int n_img, int n_model, double *m32,
                         double *s32, TopEntry *top)
 {
     const int im = blockIdx.x * blockDim.x + threadIdx.x;
@@ -23,32 +27,38 @@ __global__ void k_merge(const float *part_m, const float *part_s, const TopEntry
     TopEntry best[BIOEM_TOPK];
 #pragma unroll
     for (int k = 0; k < BIOEM_TOPK; ++k) best[k] = {-CUDART_INF_F, 0xffffffffu, 0xffffffffu};
-    for (int ch = 0; ch < cpm; ++ch) {
-        const size_t item = ((size_t)model * cpm + ch) * n_img + img;
-        const double m = part_m[item], s = part_s[item];
-        if (m != -CUDART_INF) {
-            if (M == -CUDART_INF) { M = m; S = s; }
-            else if (m > M) { S = S * exp2(M - m) + s; M = m; }          // base-2 units
-            else S += s * exp2(m - M);
-        }
-        for (int k = 0; k < BIOEM_TOPK; ++k) {
-            TopEntry e = part_top[item * BIOEM_TOPK + k];
-            if (e.pair == 0xffffffffu) break;
-            if (!before(e, best[BIOEM_TOPK - 1])) continue;
-            int pos = BIOEM_TOPK - 1;
-            while (pos > 0 && before(e, best[pos - 1])) { best[pos] = best[pos - 1]; --pos; }
-            best[pos] = e;
+    for (int r = 0; r < n_blobs; ++r) {
+        const int cpm = chunks_of_blob[r];
+        const size_t n_r = (size_t)n_model * cpm * n_img;
+        const float *part_m = reinterpret_cast<const float *>(blobs + (size_t)r * stride), *part_s = part_m + n_r;
+        const TopEntry *part_top = reinterpret_cast<const TopEntry *>(part_s + n_r);
+        for (int ch = 0; ch < cpm; ++ch) {
+            const size_t item = ((size_t)model * cpm + ch) * n_img + img;
+            const double m = part_m[item], s = part_s[item];
+            if (m != -CUDART_INF) {
+                if (M == -CUDART_INF) { M = m; S = s; }
+                else if (m > M) { S = S * exp2(M - m) + s; M = m; }          // base-2 units
+                else S += s * exp2(m - M);
+            }
+            for (int k = 0; k < BIOEM_TOPK; ++k) {
+                TopEntry e = part_top[item * BIOEM_TOPK + k];
+                if (e.pair == 0xffffffffu) break;
+                if (!before(e, best[BIOEM_TOPK - 1])) continue;
+                int pos = BIOEM_TOPK - 1;
+                while (pos > 0 && before(e, best[pos - 1])) { best[pos] = best[pos - 1]; --pos; }
+                best[pos] = e;
+            }
         }
     }
     m32[im] = M; s32[im] = S;
     for (int k = 0; k < BIOEM_TOPK; ++k) top[(size_t)im * BIOEM_TOPK + k] = best[k];
 }
 
-cudaError_t launch_merge(const float *part_m, const float *part_s, const TopEntry *part_top, int n_img, int n_model, int cpm, double *m32,
+cudaError_t launch_merge(const unsigned char *blobs, size_t stride, const int *chunks_of_blob, int n_blobs, int n_img, int n_model, double *m32,
                          double *s32, TopEntry *top, cudaStream_t st)
 {
     int n = n_img * n_model;
-    k_merge<<<(n + 63) / 64, 64, 0, st>>>(part_m, part_s, part_top, n_img, n_model, cpm, m32, s32, top);
+    k_merge<<<(n + 63) / 64, 64, 0, st>>>(blobs, stride, chunks_of_blob, n_blobs, n_img, n_model, m32, s32, top);
     return cudaGetLastError();
 }
 
@@ -57,7 +67,7 @@ cudaError_t launch_merge(const float *part_m, const float *part_s, const TopEntr
 // g = -(n-3)/2 log1p(-rho^2) + h,  rho^2 = B_fft^2 / (n T_c D_w)  (form C2).
 __global__ void __launch_bounds__(256) k_rescore(const cd *Ohat, const cd *F0, const double *K64, const double *Tc64, const double *h64,
                                                  const double *Dw, const TopEntry *cand, int ncp, int n_img, int n_model, int n_orient,
-                                                 int n_ctf, int N, int D, int model_fixed, double *g64)
+                                                 int n_ctf, int N, int D, int model_fixed, int o_first, double *g64)
 {
     __shared__ double sh[256];
     __shared__ cd tw[256];
@@ -67,7 +77,10 @@ __global__ void __launch_bounds__(256) k_rescore(const cd *Ohat, const cd *F0, c
     if (e.pair == 0xffffffffu) { if (threadIdx.x == 0) g64[ci] = -CUDART_INF; return; }
     const int im = (int)(ci / ncp);
     const int img = model_fixed >= 0 ? im : im / n_model, model = model_fixed >= 0 ? model_fixed : im % n_model;
-    const int o = e.pair / n_ctf, c = e.pair % n_ctf;
+    // n_orient orientations starting at o_first of the full grid are resident (orientation sharding): a candidate of
+    // another rank's slice gets 0 here, so that the SUM over ranks is exactly the owner's value
+    const int o = (int)(e.pair / n_ctf) - o_first, c = e.pair % n_ctf;
+    if (o < 0 || o >= n_orient) { if (threadIdx.x == 0) g64[ci] = 0.0; return; }
     const int dy = (int)(e.shift / KK) - D, dx = (int)(e.shift % KK) - D;
     for (int i = threadIdx.x; i < N; i += 256) {
         double sn, cs;
@@ -108,11 +121,11 @@ __global__ void __launch_bounds__(256) k_rescore(const cd *Ohat, const cd *F0, c
 
 cudaError_t launch_rescore(const cd *Ohat64, const cd *F064, const double *K64, const double *Tc64, const double *h64, const double *Dw,
                            const TopEntry *cand, int n_cand_per, int n_img, int n_model, int n_orient, int n_ctf, int N, int D,
-                           int cand_model_fixed, double *g64, cudaStream_t st)
+                           int cand_model_fixed, int o_first, double *g64, cudaStream_t st)
 {
     size_t total = (size_t)n_img * (cand_model_fixed >= 0 ? 1 : n_model) * n_cand_per;
     k_rescore<<<(unsigned)total, 256, 0, st>>>(Ohat64, F064, K64, Tc64, h64, Dw, cand, n_cand_per, n_img, n_model, n_orient, n_ctf, N, D,
-                                               cand_model_fixed, g64);
+                                               cand_model_fixed, o_first, g64);
     return cudaGetLastError();
 }
 

@@ -104,7 +104,7 @@ __global__ void __launch_bounds__(NT) k_fused(FusedParams p, int CB, int GP)
         const int c_begin = DUMP ? p.dump_ctf : 0, c_end = DUMP ? p.dump_ctf + 1 : p.n_ctf;
         for (int c = c_begin; c < c_end; ++c) {
             const float *__restrict__ Kc = p.K + (size_t)c * H;
-            const uint32_t pair = (uint32_t)(o * p.n_ctf + c);
+            const uint32_t pair = (uint32_t)((o + p.o_first) * p.n_ctf + c);
             const size_t moc = ((size_t)model * p.n_orient + o) * p.n_ctf + c;
             const float ab = p.alpha[moc] * beta, hterm = p.hterm[moc];
 

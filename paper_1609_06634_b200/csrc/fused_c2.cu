@@ -318,7 +318,7 @@ k_fused_c2(FusedParams p, const float4 *__restrict__ Kt, const float *__restrict
                 if (lane == 0) { c2_arrive(empty_l + 8u * b1); c2_arrive(empty_p + 8u * b1); }
                 const size_t moc = ((size_t)model * p.n_orient + o1) * p.n_ctf + c1;
                 const float ab = p.alpha[moc] * beta, hterm = p.hterm[moc];
-                const uint32_t pair = (uint32_t)(o1 * p.n_ctf + c1);
+                const uint32_t pair = (uint32_t)((o1 + p.o_first) * p.n_ctf + c1);
 #pragma unroll
                 for (int cw = 0; cw < 4; ++cw) {
                     c2 y[2];

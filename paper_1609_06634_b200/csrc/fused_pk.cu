@@ -364,7 +364,7 @@ __global__ void __launch_bounds__(PK<N>::NT, 1) k_fused_pk(FusedParams p, const 
         }
         nc2 = nc1; pair2 = pair1; eX = eF;
         var2 = var1; var1 = var0; var0 = var0 + 1 == map.nvar ? 0 : var0 + 1;
-        nc1 = live ? nc : 0; pair1 = (uint32_t)(o * p.n_ctf + c0);
+        nc1 = live ? nc : 0; pair1 = (uint32_t)((o + p.o_first) * p.n_ctf + c0);
         c0 += CG;
         if (c0 >= c_hi) { c0 = c_lo; ++o; }
     }

@@ -466,7 +466,7 @@ __global__ void __launch_bounds__(TM::NT, 1) k_fused_tm(FusedParams p, const flo
         if (live) {
             const size_t moc = ((size_t)model * p.n_orient + o) * p.n_ctf + c;
             pab = p.alpha[moc] * beta; ph = p.hterm[moc];
-            ppair = (uint32_t)(o * p.n_ctf + c);
+            ppair = (uint32_t)((o + p.o_first) * p.n_ctf + c);
             if (++c >= c_hi) { c = c_lo; ++o; }
         }
     }

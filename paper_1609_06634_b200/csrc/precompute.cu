@@ -338,7 +338,7 @@ cudaError_t launch_ctf_tables(const double *a, const double *A, const double *b,
 
 // T_c = n C_cc - C_c^2 = sum_{s != 0} |F0(s) K_c(s)|^2 (Plancherel; "Eqs. S4, S6"), Hermitian weights:
 // columns l = 0 and l = N/2 count once, the others twice.  One CTA per (model, orientation), loop over CTFs.
-__global__ void __launch_bounds__(256) k_calc_stats(const cd *F0, const double *K64, int n_orient, int n_ctf, int N, const double *lp_orient,
+__global__ void __launch_bounds__(256) k_calc_stats(const cd *F0, const double *K64, int n_orient, int n_orient_total, int n_ctf, int N, const double *lp_orient,
                                                     const double *lp_ctf, double log_shifts, double *Tc64, double *h64, float *alpha32,
                                                     float *h32, int *flags)
 {
@@ -360,7 +360,7 @@ __global__ void __launch_bounds__(256) k_calc_stats(const cd *F0, const double *
         if (threadIdx.x == 0) {
             const size_t moc = (size_t)mo * n_ctf + c;
             const double n = (double)N * N;
-            const double lpo = lp_orient ? lp_orient[o] : -log((double)n_orient);
+            const double lpo = lp_orient ? lp_orient[o] : -log((double)n_orient_total);   // a rank that scores a slice of the grid still weighs with the whole grid (R7)
             const double lpc = lp_ctf ? lp_ctf[c] : -log((double)n_ctf);
             const double h = -0.5 * log(s) + lpo + lpc - log_shifts;
             if (!(s > 0.0) || isinf(s)) atomicOr(flags, 2);          // empty calculated image: T_c = 0, rho^2 undefined
@@ -370,11 +370,11 @@ __global__ void __launch_bounds__(256) k_calc_stats(const cd *F0, const double *
     }
 }
 
-cudaError_t launch_calc_stats(const cd *F0, const double *K64, int n_mo, int n_orient, int n_ctf, int N, const double *lp_orient,
+cudaError_t launch_calc_stats(const cd *F0, const double *K64, int n_mo, int n_orient, int n_orient_total, int n_ctf, int N, const double *lp_orient,
                               const double *lp_ctf, double log_shifts, double *Tc64, double *h64, float *alpha32, float *h32,
                               int *flags, cudaStream_t st)
 {
-    k_calc_stats<<<n_mo, 256, 0, st>>>(F0, K64, n_orient, n_ctf, N, lp_orient, lp_ctf, log_shifts, Tc64, h64, alpha32, h32, flags);
+    k_calc_stats<<<n_mo, 256, 0, st>>>(F0, K64, n_orient, n_orient_total, n_ctf, N, lp_orient, lp_ctf, log_shifts, Tc64, h64, alpha32, h32, flags);
     return cudaGetLastError();
 }
 

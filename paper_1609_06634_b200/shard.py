@@ -1,4 +1,9 @@
-"""Multi-GPU host logic: the path shards over IMAGES with no data-path collective (paper: MPI over independent work,
+"""Multi-GPU host logic.  Two ways to shard, both from the paper:
+  * IMAGES (default; run_sharded, score_block_and_gather): no data-path collective at all;
+  * ORIENTATIONS (run_orientation_sharded): the paper's MPI axis -- every rank holds all images and a slice of the grid, one
+    all_gather of the per-chunk partials {m, s, top-8} and one all_reduce of the re-scored candidates; bit-identical to one GPU.
+
+Image sharding: the path shards over IMAGES with no data-path collective (paper: MPI over independent work,
 "absence of both communication and load-imbalances").  One process per GPU; every rank
 holds the models and grids, scores its contiguous block of the image stack, and the per-image results are
 concatenated in image order with one all_gather at the end (results only: a few bytes per image, not on the data path).
@@ -85,3 +90,59 @@ def run_sharded(make_ctx, images, score=None, group=None) -> dict:
         probe = (score or default_score)(ctx, images[:1]) if len(images) else {}
         local = {k: np.asarray(v)[:0] for k, v in probe.items()}
     return gather_by_image(local, len(images), group)
+
+
+def orientation_shard(n_orient: int, chunk: int, rank: int, world: int) -> tuple[int, int]:
+    """Slice [begin, end) of the orientation grid for rank `rank`: whole chunks of `chunk` orientations (every rank cuts the grid
+    at the same places as one GPU with that chunk size would), chunk counts differing by at most one, in grid order."""
+    if chunk < 1 or world < 1 or not 0 <= rank < world:
+        raise ValueError("orientation_shard: need chunk >= 1, world >= 1, 0 <= rank < world")
+    n_chunks = -(-n_orient // chunk)
+    b, e = image_shard(n_chunks, rank, world)
+    return min(b * chunk, n_orient), min(e * chunk, n_orient)
+
+
+def run_orientation_sharded(ctx, chunk: int, group=None) -> dict:
+    """Score the images pushed into `ctx` against the whole grid with the orientation grid sharded over the ranks of `group`
+    ("MPI over orientations").  `ctx` is a configured BioEM context (models, grids, images; the same on every rank).
+    Exchange steps ("absence of communication" but for the final gather): one all_gather of the per-chunk partials, one
+    all_reduce of the FP64 re-scored candidates.  Every rank returns the full results, bit-identical to one GPU with
+    set_orientation_chunk(chunk) (include/bioem.h)."""
+    import torch
+    import torch.distributed as dist
+
+    on = dist.is_available() and dist.is_initialized()
+    world = dist.get_world_size(group) if on else 1
+    rank = dist.get_rank(group) if on else 0
+    ob, oe = orientation_shard(ctx.n_orient, chunk, rank, world)
+    ctx.set_orientation_chunk(chunk)
+    ctx.set_orientation_slice(ob, oe)
+    try:
+        ctx.run_partial()
+        if world == 1:
+            ctx.merge_partials()
+            ctx.rescore_local()
+        else:
+            dev = torch.device("cuda", torch.cuda.current_device()) if dist.get_backend(group) == "nccl" else torch.device("cpu")
+            nbytes, nchunks = ctx.get_partials_size()
+            meta = torch.tensor([nbytes, nchunks], dtype=torch.int64, device=dev)
+            metas = [torch.empty_like(meta) for _ in range(world)]
+            dist.all_gather(metas, meta, group=group)
+            sizes = [int(m[0]) for m in metas]
+            chunks = [int(m[1]) for m in metas]
+            stride = max(max(sizes), 4)
+            mine = torch.zeros(stride, dtype=torch.uint8, device=dev)
+            ctx.export_partials(mine)
+            allb = torch.empty(world * stride, dtype=torch.uint8, device=dev)
+            dist.all_gather_into_tensor(allb, mine, group=group) if dev.type == "cuda" else \
+                dist.all_gather(list(allb.view(world, stride).unbind(0)), mine, group=group)
+            ctx.merge_partials(allb, stride, chunks)
+            ctx.rescore_local()
+            g = torch.empty(ctx.rescore_shape(), dtype=torch.float64, device=dev)
+            ctx.export_rescore(g)
+            dist.all_reduce(g, op=dist.ReduceOp.SUM, group=group)            # owner's value + exact zeros
+            ctx.import_rescore(g)
+        ctx.finish()
+        return dict(logp=ctx.get_log_posterior(), **ctx.get_best())
+    finally:
+        ctx.set_orientation_slice(0, -1)

@@ -460,3 +460,107 @@ def test_split_stack_is_bit_identical():
                 bo.append(np.stack([b.get_best()[k] for k in ("orient", "ctf", "dx", "dy")]))
         outs.append((np.concatenate(lp), np.concatenate(bo, axis=1)))
     assert np.array_equal(outs[0][0], outs[1][0]) and np.array_equal(outs[0][1], outs[1][1])
+
+
+@pytest.mark.parametrize("name,chunk,world", [("small_mid", 5, 3), ("paper_mid", 2, 2), ("ensemble_mid", 4, 2), ("tiny_mid", 32, 3)])
+def test_orientation_sharding_is_bit_identical(name, chunk, world):
+    """the orientation grid cut over `world` ranks (here: contexts on one GPU, run one after
+    the other, the two exchanges done by hand on the host exactly as shard.run_orientation_sharded does them with
+    torch.distributed) gives the bits of one context scoring the whole grid with the same orientation chunk; and that one
+    matches the oracle."""
+    from paper_1609_06634_b200 import BioEM
+    from paper_1609_06634_b200.shard import orientation_shard
+    wl = W.build_workload(name)
+    s = wl["spec"]
+    with BioEM() as b:
+        b.load_workload(wl)
+        b.set_orientation_chunk(chunk)
+        b.run()
+        one = dict(logp=b.get_log_posterior(), **b.get_best())
+    ctxs = [BioEM() for _ in range(world)]
+    try:
+        blobs, sizes, chunks = [], [], []
+        for r, c in enumerate(ctxs):
+            c.load_workload(wl)
+            c.set_orientation_chunk(chunk)
+            c.set_orientation_slice(*orientation_shard(s.n_orient, chunk, r, world))
+            c.run_partial()
+            nb, nc = c.get_partials_size()
+            buf = np.zeros(max(nb, 4), np.uint8)
+            c.export_partials(buf)
+            blobs.append(buf); sizes.append(nb); chunks.append(nc)
+        assert sum(chunks) == -(-s.n_orient // chunk) * (2 if ctxs[0].get_run_plan_partial()[0] == 3 else 1)
+        stride = max(max(sizes), 4)
+        allb = np.zeros(world * stride, np.uint8)
+        for r, bb in enumerate(blobs):
+            allb[r * stride: r * stride + bb.size] = bb                      # all_gather
+        g = np.zeros(ctxs[0].rescore_shape())
+        for c in ctxs:
+            c.merge_partials(allb, stride, chunks)
+            c.rescore_local()
+            gr = np.empty_like(g)
+            c.export_rescore(gr)
+            g += gr                                                          # all_reduce(SUM): the owner's value + exact zeros
+        for c in ctxs:
+            c.import_rescore(g)
+            c.finish()
+            got = dict(logp=c.get_log_posterior(), **c.get_best())
+            for k in one:
+                assert np.array_equal(got[k], one[k]), k
+    finally:
+        for c in ctxs:
+            c.close()
+    ref = _oracle_full(wl)
+    assert np.abs(one["logp"] - ref["logp"]).max() <= TOL_LOGP
+
+
+def test_orientation_slice_errors():
+    from paper_1609_06634_b200 import BioEM
+    from paper_1609_06634_b200.binding import BioEMError
+    wl = W.build_workload("tiny_mini")
+    with BioEM() as b:
+        b.load_workload(wl)
+        b.set_orientation_slice(0, 2)
+        with pytest.raises(BioEMError):                                      # no explicit chunk
+            b.run_partial()
+        b.set_orientation_chunk(2)
+        with pytest.raises(BioEMError):                                      # bioem_run on a context that holds part of the grid
+            b.run()
+        b.set_orientation_slice(1, 3)
+        with pytest.raises(BioEMError):                                      # slice not on a chunk boundary
+            b.run_partial()
+        b.set_orientation_slice(0, 99)
+        with pytest.raises(BioEMError):                                      # outside the grid
+            b.run_partial()
+        b.set_orientation_slice(0, -1)
+        b.run()
+        assert np.all(np.isfinite(b.get_log_posterior()))
+
+
+def test_image_subsets_reuse_the_calculated_images():
+    """P:287 (image stacks larger than device memory are processed in subsets): bioem_push_images(subset) + bioem_run per subset
+    reuses the calculated-image cache (a1-a3 are not launched again) and gives the bits of the whole-stack run."""
+    from paper_1609_06634_b200 import BioEM
+    wl = W.build_workload("small_mid")
+    with BioEM() as b:
+        b.load_workload(wl)
+        b.set_orientation_chunk(5)
+        b.run()
+        whole = (b.get_log_posterior(), b.get_best()["orient"])
+        n_first = b.get_launch_count()[0]
+        parts, launches = [], []
+        for sl in (slice(0, 2), slice(2, 3), slice(3, None)):
+            b.push_images(wl["images"][sl])
+            b.run()
+            parts.append((b.get_log_posterior(), b.get_best()["orient"]))
+            launches.append(b.get_launch_count()[0])
+        assert np.array_equal(np.concatenate([p[0] for p in parts]), whole[0])
+        assert np.array_equal(np.concatenate([p[1] for p in parts]), whole[1])
+        assert max(launches) < n_first                                       # no projection / CTF-table / statistics launches
+        b.invalidate_precompute()
+        b.run()
+        assert b.get_launch_count()[0] == n_first - 0 or b.get_launch_count()[0] >= max(launches)
+        b.set_shift_range(wl["spec"].max_shift)                              # any setter drops the cache
+        b.push_images(wl["images"])
+        b.run()
+        assert np.array_equal(b.get_log_posterior(), whole[0])

@@ -392,6 +392,58 @@ def test_fourier_slice_exact_index_permutations():
     check([0.5, 0.5, 0.5, 0.5], rho.transpose(1, 2, 0))
 
 
+# ------------------------------------------------------------------ real-space, cropping displacement variant (R25)
+def test_cropped_sums_delta_images_do_not_wrap():
+    # obs = delta at (k0, j0), calc = delta at (k1, j1): C_co(d) = 1 exactly where (k0, j0) + d = (k1, j1), INSIDE the box only
+    N, D = 8, 3
+    obs = np.zeros((N, N)); obs[1, 6] = 1.0
+    cal = np.zeros((N, N)); cal[3, 7] = 2.5
+    cco, cc, ccc = oracle.cropped_sums(obs, cal, D)
+    want = np.zeros((2 * D + 1, 2 * D + 1)); want[2 + D, 1 + D] = 2.5          # d = (dx, dy) = (+1, +2)
+    assert np.array_equal(cco, want)
+    # a pair that only meets through the border: circular (R5) finds it at d = (+2, 0), the cropping variant does not
+    cal2 = np.zeros((N, N)); cal2[1, 0] = 1.0
+    circ = oracle.cross_corr_direct(obs, cal2, D)
+    crop, _, _ = oracle.cropped_sums(obs, cal2, D)
+    assert circ[0 + D, 2 + D] == 1.0 and np.all(crop == 0.0)
+    # C_c(d), C_cc(d): the delta of the calculated image at column 7 is pushed out of the box by any dx < 0 ... no: I_d(r) = I1(r+d)
+    # keeps pixel p = r + d of I1 iff r = p - d is inside the box: column 7 survives iff 0 <= 7 - dx <= 7, i.e. dx >= 0
+    for dy in range(-D, D + 1):
+        for dx in range(-D, D + 1):
+            inside = 0 <= 7 - dx < N and 0 <= 3 - dy < N
+            assert cc[dy + D, dx + D] == (2.5 if inside else 0.0) and ccc[dy + D, dx + D] == (6.25 if inside else 0.0)
+
+
+def test_cropped_sums_equal_explicit_zero_padded_shift():
+    # brute force: build I_d(r) = I1(r + d) with zeros where r + d leaves the box, as an array, and take plain numpy sums
+    rng = np.random.default_rng(77)
+    N, D = 7, 2
+    obs, cal = rng.normal(size=(N, N)), rng.normal(size=(N, N))
+    cco, cc, ccc = oracle.cropped_sums(obs, cal, D)
+    pad = np.zeros((N + 2 * D, N + 2 * D)); pad[D:D + N, D:D + N] = cal
+    for dy in range(-D, D + 1):
+        for dx in range(-D, D + 1):
+            Id = pad[D + dy:D + dy + N, D + dx:D + dx + N]                       # Id[k][j] = cal[k + dy][j + dx] or 0
+            assert abs(cco[dy + D, dx + D] - (obs * Id).sum()) < 1e-12
+            assert abs(cc[dy + D, dx + D] - Id.sum()) < 1e-12 and abs(ccc[dy + D, dx + D] - (Id * Id).sum()) < 1e-12
+
+
+def test_cropping_variant_equals_circular_variant_when_nothing_reaches_the_border():
+    # the two variants differ only in what happens at the borders: with the calculated image supported more than D
+    # pixels away from them, Eq. 9 on the grid is the same number either way (tier 2 vs tier 0 of the same loop nest)
+    spec = W.get_spec("tiny_mini")
+    wl = W.build_workload(spec)
+    s = wl["spec"]
+    m = dict(wl["models"][0]); m["xyz"] = np.asarray(m["xyz"]) * 0.5             # 15 A ball in a 128 A box: far from the borders
+    a = oracle.run_model(m, s.n_pix, s.pixel_A, 3, wl["quats"][:2], wl["ctfs"][:1] * [0, 1, 0] + [0, 0, 0], wl["images"][:2], tier=0)
+    b = oracle.run_model(m, s.n_pix, s.pixel_A, 3, wl["quats"][:2], wl["ctfs"][:1] * [0, 1, 0] + [0, 0, 0], wl["images"][:2], tier=2)
+    assert np.abs(a.log_posterior() - b.log_posterior()).max() < 1e-9 and np.array_equal(a.best_flat, b.best_flat)
+    # ... and differ once the CTF spreads the calculated image over the whole box
+    a = oracle.run_model(m, s.n_pix, s.pixel_A, 3, wl["quats"][:2], wl["ctfs"][:1], wl["images"][:2], tier=0)
+    b = oracle.run_model(m, s.n_pix, s.pixel_A, 3, wl["quats"][:2], wl["ctfs"][:1], wl["images"][:2], tier=2)
+    assert np.abs(a.log_posterior() - b.log_posterior()).max() > 1e-6
+
+
 # ------------------------------------------------------------------ Eq. 9 on the grid (R7, R15, R16)
 def test_planted_truth_is_the_argmax():
     # north_star check 2: a noiseless, CTF-free image at a grid orientation and shift scores its maximum exactly there

@@ -62,3 +62,135 @@ def test_two_ranks_equal_one_rank(n_img):
     for r in range(2):
         assert np.array_equal(np.array(got[r]["logp"]), want["logp"])                   # bit-identical, image order kept
         assert np.array_equal(np.array(got[r]["orient"], dtype=np.int32), want["orient"])
+
+
+# ------------------------------------------------------------------ orientation sharding
+def test_orientation_shard_cuts_whole_chunks():
+    from paper_1609_06634_b200.shard import orientation_shard
+    for n_orient, chunk in ((40, 5), (41, 5), (4096, 32), (7, 32), (64, 1)):
+        for world in (1, 2, 3, 8):
+            sl = [orientation_shard(n_orient, chunk, r, world) for r in range(world)]
+            assert sl[0][0] == 0 and sl[-1][1] == n_orient
+            assert all(sl[i][1] == sl[i + 1][0] for i in range(world - 1))
+            assert all(b % chunk == 0 for b, e in sl if e > b)
+
+
+class _FakeCtx:
+    """Stand-in for BioEM with the phased calls of include/bioem.h and the same buffer contracts (a byte blob of per-chunk
+    partials, an [I][M][K] re-score array), computing on the host from a seeded score table: what is under test is the exchange in
+    shard.run_orientation_sharded (ragged blobs, chunk order, all_reduce of owner-or-zero values), not the kernels."""
+    K = 8
+
+    def __init__(self, n_img, n_models, n_orient):
+        self.n_img, self.n_models, self.n_orient = n_img, n_models, n_orient
+        rng = np.random.default_rng(11)
+        self.score = rng.normal(size=(n_img, n_models, n_orient)).astype(np.float32)      # "log-term" of (image, model, orientation)
+        self.fine = self.score.astype(np.float64) + rng.normal(size=self.score.shape) * 1e-3   # its "FP64 re-scored" value
+        self.chunk, self.sl = 0, (0, n_orient)
+
+    def set_orientation_chunk(self, c):
+        self.chunk = c
+
+    def set_orientation_slice(self, b, e):
+        self.sl = (b, e) if e >= 0 else (0, self.n_orient)
+
+    def run_partial(self):
+        b, e = self.sl
+        assert b % self.chunk == 0
+        self.nch = -(-(e - b) // self.chunk)
+        # blob: float32 sum per (model, chunk, image) then int32 argmax orientation (global index) per (model, chunk, image)
+        sums = np.zeros((self.n_models, self.nch, self.n_img), np.float32)
+        arg = np.zeros((self.n_models, self.nch, self.n_img), np.int32)
+        for ch in range(self.nch):
+            o0, o1 = b + ch * self.chunk, min(b + (ch + 1) * self.chunk, e)
+            for o in range(o0, o1):                               # float32 accumulation in grid order inside a chunk
+                sums[:, ch, :] = sums[:, ch, :] + self.score[:, :, o].T
+            arg[:, ch, :] = (np.argmax(self.score[:, :, o0:o1], axis=2) + o0).T
+        self.blob = np.concatenate([sums.ravel().view(np.uint8), arg.ravel().view(np.uint8)])
+
+    def get_partials_size(self):
+        return self.blob.size, self.nch
+
+    def export_partials(self, dst):
+        dst.numpy()[: self.blob.size] = self.blob
+
+    def merge_partials(self, blobs=None, stride_bytes=0, chunks_of_blob=None):
+        if blobs is None:
+            blobs, stride_bytes, chunks_of_blob = self.blob, self.blob.size, [self.nch]
+        else:
+            blobs = blobs.numpy()
+        tot = np.zeros((self.n_img, self.n_models), np.float32)
+        cand = []
+        for r, nch in enumerate(chunks_of_blob):
+            raw = blobs[r * stride_bytes: r * stride_bytes + nch * self.n_models * self.n_img * 8]
+            n = nch * self.n_models * self.n_img
+            sums = raw[: 4 * n].view(np.float32).reshape(self.n_models, nch, self.n_img)
+            arg = raw[4 * n: 8 * n].view(np.int32).reshape(self.n_models, nch, self.n_img)
+            for ch in range(nch):                                 # blobs in rank order, chunks in order: the 1-rank order
+                tot = tot + sums[:, ch, :].T
+                cand.append(arg[:, ch, :].T)
+        self.tot = tot
+        cand = np.stack(cand, axis=2)                             # [I][M][all chunks]: candidate orientations
+        sc = np.take_along_axis(self.score, cand, axis=2)
+        order = np.argsort(-sc, axis=2, kind="stable")[:, :, : self.K]
+        self.cand = np.take_along_axis(cand, order, axis=2)
+        if self.cand.shape[2] < self.K:
+            self.cand = np.concatenate([self.cand, -np.ones((self.n_img, self.n_models, self.K - self.cand.shape[2]), np.int32)], axis=2)
+
+    def rescore_local(self):
+        b, e = self.sl
+        own = (self.cand >= b) & (self.cand < e)
+        self.g = np.where(own, np.take_along_axis(self.fine, np.clip(self.cand, 0, None), axis=2), 0.0)
+
+    def rescore_shape(self):
+        return (self.n_img, self.n_models, self.K)
+
+    def export_rescore(self, dst):
+        dst.numpy()[...] = self.g
+
+    def import_rescore(self, src):
+        self.g = src.numpy().copy()
+
+    def finish(self):
+        pass
+
+    def get_log_posterior(self):
+        return self.tot.astype(np.float64) + self.g.max(axis=2)
+
+    def get_best(self):
+        k = np.argmax(np.where(self.cand >= 0, self.g, -np.inf), axis=2)
+        return dict(orient=np.take_along_axis(self.cand, k[:, :, None], axis=2)[:, :, 0].astype(np.int32))
+
+
+def _orient_worker(rank, world, port, q):
+    import torch.distributed as dist
+    from paper_1609_06634_b200.shard import run_orientation_sharded
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        out = run_orientation_sharded(_FakeCtx(5, 2, 43), chunk=4)        # 11 chunks, the last one ragged: 6 + 5 over two ranks
+        q.put((rank, {k: v.tolist() for k, v in out.items()}))
+    finally:
+        dist.destroy_process_group()
+
+
+def test_orientation_sharding_two_ranks_equal_one_rank():
+    import torch.multiprocessing as mp
+    from paper_1609_06634_b200.shard import run_orientation_sharded
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    procs = [ctx.Process(target=_orient_worker, args=(r, 2, port, q)) for r in range(2)]
+    for p in procs:
+        p.start()
+    got = dict(q.get(timeout=120) for _ in procs)
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    want = run_orientation_sharded(_FakeCtx(5, 2, 43), chunk=4)           # no process group: one rank, the whole grid
+    for r in range(2):
+        assert np.array_equal(np.array(got[r]["logp"]), want["logp"])                   # bit-identical on every rank
+        assert np.array_equal(np.array(got[r]["orient"], dtype=np.int32), want["orient"])

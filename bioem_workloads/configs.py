@@ -121,6 +121,13 @@ CONFIGS["ensemble_mid"] = replace(_ENSEMBLE, name="ensemble_mid", n_images=4, n_
                                   orient_stride=28, defocus_um=_lin(0.5, 3.0, 4), bfactor_A2=(0.0, 100.0))
 
 
+# Other box sizes: 170^2 is the GroEL set of the paper's Table 1, 2 x 5 x 17: no power-of-two factor beyond 2.
+# Same recipe as Small (2,000 atoms, 1.5 A/px), shift range +-6, a handful of images / orientations / CTFs: parity cases only.
+for _n in (96, 160, 170, 192):
+    CONFIGS[f"box{_n}_mini"] = replace(_SMALL, name=f"box{_n}_mini", n_pix=_n, max_shift=6, n_images=4, orient_stride=1151,
+                                       defocus_um=(0.5, 3.0), bfactor_A2=(50.0,), amp_contrast=(0.1,))
+
+
 def get_spec(name: str, **overrides) -> WorkloadSpec:
     spec = CONFIGS[name]
     return replace(spec, **overrides) if overrides else spec

@@ -47,7 +47,10 @@ int bioem_destroy(bioem_ctx *ctx);
 const char *bioem_last_error(const bioem_ctx *ctx);
 
 /* Square images of n_pix x n_pix pixels of pixel_size_A Angstrom.  Supported n_pix:
- * 64, 128, 224, 256 (BIOEM_EUNSUPPORTED otherwise).  Clears images, models stay. */
+ * 64, 96, 128, 160, 170, 192, 224, 256 (BIOEM_EUNSUPPORTED otherwise).  64 / 128 (max_shift <= 16) and 224 (max_shift <= 31) run
+ * the tuned kernels; the other sizes -- 170 is the GroEL box of the paper's Table 1, 2 x 5 x 17 -- run the generic
+ * two-step kernel, whose second step is a direct sum over n_pix / N1 residues (N1 = 32, or 2 for 170): same results, parity
+ * tested, not tuned.  Clears images, models stay. */
 int bioem_set_image_geometry(bioem_ctx *ctx, int n_pix, float pixel_size_A);
 
 /* Models.  Atoms: uniform-density spheres, centre xyz_A [n][3], radius_A [n], total
@@ -134,6 +137,16 @@ int bioem_get_ensemble_log_posterior(bioem_ctx *ctx, const double *weights, doub
  * posterior is enabled. */
 int bioem_set_orientation_chunk(bioem_ctx *ctx, int n_orient_per_item);
 
+/* Displacement variant (paper section 3.3).  0 (default): Fourier space -- one output-pruned inverse transform
+ * per (image, calculated image), displacements wrap around the borders (R5); the hot path.  1: real space -- "the cross-correlation
+ * is simply calculated for different displacements", the displaced calculated image is CROPPED at the borders instead of
+ * wrapping: I_d(r) = I1(r + d) where r + d lies inside the box, 0 elsewhere, and Eq. 8 is applied to (I_obs, I_d) over
+ * all n pixels, so C_co, C_c and C_cc depend on d (reading R25 in DESIGN.md).  The paper's route for very few displacements
+ * (Fig. 2): (2D+1)^2 n multiply-adds per pair, FP64 throughout (no re-scoring step), deterministic.  Call BEFORE
+ * bioem_push_images (the real-space variant keeps the mean-free images in real space); BIOEM_EBADSTATE at bioem_run otherwise.
+ * Not combinable with orientation slices or the per-orientation posterior (BIOEM_EUNSUPPORTED). */
+int bioem_set_displacement_variant(bioem_ctx *ctx, int variant);
+
 /* ---- orientation sharding: the paper's MPI axis ("MPI over orientations"; no communication but one gather) ----
  * Every rank holds all models, grids and images and scores a contiguous SLICE [o_begin, o_end) of the orientation grid; indices,
  * priors and the uniform weight -log(n_orient) still refer to the full grid.  bioem_run is the four phases below on one
@@ -169,7 +182,8 @@ int bioem_finish(bioem_ctx *ctx);
  * tensor-memory kernel for n_pix 224 with max_shift <= 31, generic kernel otherwise), 1 generic kernel always, 3 the
  * two-CTA-cluster kernel of round 1 (n_pix 224, max_shift <= 31; kept as a cross-check of the tensor-memory kernel). */
 int bioem_debug_set_kernel(bioem_ctx *ctx, int which);
-/* The plan of the last bioem_run: kernel (1 generic, 2 packed, 3 cluster, 4 tensor memory) and orientations per work item. */
+/* The plan of the last bioem_run: kernel (1 generic, 2 packed, 3 cluster, 4 tensor memory, 6 real-space variant) and orientations
+ * per work item. */
 int bioem_get_run_plan(bioem_ctx *ctx, int *kernel, int *n_orient_per_item);
 /* real-space calculated image I1 of (model, orient, ctf) [N][N] ("synthetic map"). */
 int bioem_debug_calc_image(bioem_ctx *ctx, int model, int orient, int ctf, float *out_real);

@@ -19,9 +19,9 @@ EXPORTED_SYMBOLS = [
     "bioem_set_orientation_posterior", "bioem_get_orientation_log_posterior", "bioem_get_ensemble_log_posterior",
     "bioem_set_orientation_chunk", "bioem_debug_set_kernel", "bioem_get_run_plan", "bioem_invalidate_precompute",
     "bioem_set_orientation_slice", "bioem_run_partial", "bioem_get_partials_size", "bioem_export_partials", "bioem_merge_partials",
-    "bioem_rescore_local", "bioem_export_rescore", "bioem_import_rescore", "bioem_finish",
+    "bioem_rescore_local", "bioem_export_rescore", "bioem_import_rescore", "bioem_finish", "bioem_set_displacement_variant",
 ]
-KERNEL_AUTO, KERNEL_GENERIC, KERNEL_PK, KERNEL_C2, KERNEL_TM = 0, 1, 2, 3, 4
+KERNEL_AUTO, KERNEL_GENERIC, KERNEL_PK, KERNEL_C2, KERNEL_TM, KERNEL_DFT, KERNEL_REALSPACE = 0, 1, 2, 3, 4, 5, 6
 
 _fp = C.POINTER(C.c_float)
 _dp = C.POINTER(C.c_double)
@@ -71,6 +71,7 @@ def lib():
         L.bioem_export_rescore.argtypes = [C.c_void_p, C.c_void_p, C.c_int]
         L.bioem_import_rescore.argtypes = [C.c_void_p, C.c_void_p, C.c_int]
         L.bioem_finish.argtypes = [C.c_void_p]
+        L.bioem_set_displacement_variant.argtypes = [C.c_void_p, C.c_int]
         L.bioem_get_log_posterior.argtypes = [C.c_void_p, _dp]
         L.bioem_get_best.argtypes = [C.c_void_p, _ip, _ip, _ip, _ip, _dp]
         L.bioem_debug_calc_image.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, _fp]
@@ -271,6 +272,10 @@ class BioEM:
         self._ck(self._L.bioem_get_best(self._h, o.ctypes.data_as(_ip), c.ctypes.data_as(_ip), dx.ctypes.data_as(_ip),
                                         dy.ctypes.data_as(_ip), lp.ctypes.data_as(_dp)))
         return dict(orient=o, ctf=c, dx=dx, dy=dy, log_p=lp)
+
+    def set_displacement_variant(self, variant=0):
+        """0 Fourier space / circular (default), 1 real space / cropping; before push_images."""
+        self._ck(self._L.bioem_set_displacement_variant(self._h, int(variant)))
 
     def set_orientation_chunk(self, n_orient_per_item=0):
         self._ck(self._L.bioem_set_orientation_chunk(self._h, int(n_orient_per_item)))

@@ -61,6 +61,8 @@ struct bioem_ctx {
     bool pre_valid = false;                            // a1-a3 outputs (F0, K, T_c, h, alpha) match the current models / grids / shift range
     bool want_orient = false, ran_orient = false;      // per-orientation posterior: requested / produced by the last run
     int oc_user = 0;                                   // orientations per work item (0 = automatic)
+    int variant = 0, img_variant = 0;                                   // displacement variant: 0 Fourier / circular (the hot path), 1 real space / cropping
+    DBuf Oreal64, rs_T, rs_I1, rs_cc, rs_ccc, rs_part, rs_logw, rs_pair, rs_m, rs_s, rs_best, rs_bpair, rs_bshift;
     int slice_begin = 0, slice_end = -1;               // orientation slice this context scores; end < 0 = the whole grid
     int phase = 0;                                     // of the phased run: 0 nothing, 1 partials, 2 merged, 3 re-scored, 4 finished (= ran)
     int run_o_first = 0, run_o_local = 0, run_chunks = 0;     // slice and chunk count (per model, partials per item included) of the last partial run
@@ -96,7 +98,7 @@ struct bioem_ctx {
         return (code);           \
     } while (0)
 
-static bool supported_n(int n) { return n == 64 || n == 128 || n == 224 || n == 256; }
+static bool supported_n(int n) { return n == 64 || n == 96 || n == 128 || n == 160 || n == 170 || n == 192 || n == 224 || n == 256; }
 
 extern "C" {
 
@@ -131,7 +133,8 @@ int bioem_destroy(bioem_ctx *ctx)
     for (auto &m : ctx->models) { m.xyz.release(); m.rad.release(); m.wt.release(); m.rho.release(); }
     DBuf *all[] = {&ctx->rot, &ctx->lp_orient, &ctx->ctf_a, &ctx->ctf_A, &ctx->ctf_b, &ctx->lp_ctf, &ctx->Ohat64, &ctx->Ohat32, &ctx->Dw,
                    &ctx->beta, &ctx->F064, &ctx->F032, &ctx->K64, &ctx->K32, &ctx->Kt, &ctx->Tc64, &ctx->h64, &ctx->alpha32, &ctx->h32,
-                   &ctx->blob, &ctx->gathered, &ctx->blob_chunks, &ctx->m32, &ctx->s32, &ctx->top, &ctx->g64, &ctx->logp, &ctx->logp_orient, &ctx->logp32,
+                   &ctx->blob, &ctx->gathered, &ctx->blob_chunks, &ctx->Oreal64, &ctx->rs_T, &ctx->rs_I1, &ctx->rs_cc, &ctx->rs_ccc, &ctx->rs_part, &ctx->rs_logw,
+                   &ctx->rs_pair, &ctx->rs_m, &ctx->rs_s, &ctx->rs_best, &ctx->rs_bpair, &ctx->rs_bshift, &ctx->m32, &ctx->s32, &ctx->top, &ctx->g64, &ctx->logp, &ctx->logp_orient, &ctx->logp32,
                    &ctx->best, &ctx->best_logp, &ctx->scratch_a, &ctx->scratch_b, &ctx->scratch_c, &ctx->dump, &ctx->flags, &ctx->staging};
     for (DBuf *b : all) b->release();
     for (int i = 0; i < 4; ++i) if (ctx->ev[i]) cudaEventDestroy(ctx->ev[i]);
@@ -145,7 +148,7 @@ int bioem_set_image_geometry(bioem_ctx *ctx, int n_pix, float pixel_size_A)
 {
     if (!ctx) return BIOEM_EBADARG;
     if (!(pixel_size_A > 0.f)) FAIL(BIOEM_EBADARG, "pixel_size_A must be > 0");
-    if (!supported_n(n_pix)) FAIL(BIOEM_EUNSUPPORTED, "n_pix must be one of 64, 128, 224, 256");
+    if (!supported_n(n_pix)) FAIL(BIOEM_EUNSUPPORTED, "n_pix must be one of 64, 96, 128, 160, 170, 192, 224, 256");
     ctx->N = n_pix;
     ctx->px = (double)pixel_size_A;
     ctx->n_img = 0;
@@ -202,7 +205,7 @@ int bioem_add_model_density(bioem_ctx *ctx, int n_vox, float voxel_A, const floa
 {
     if (!ctx) return BIOEM_EBADARG;
     if (!rho || !(voxel_A > 0.f)) FAIL(BIOEM_EBADARG, "add_model_density: NULL map or voxel size <= 0");
-    if (!supported_n(n_vox)) FAIL(BIOEM_EUNSUPPORTED, "add_model_density: n_vox must be one of 64, 128, 224, 256");
+    if (!supported_n(n_vox)) FAIL(BIOEM_EUNSUPPORTED, "add_model_density: n_vox must be one of 64, 96, 128, 160, 170, 192, 224, 256");
     CK(cudaSetDevice(ctx->device));
     ctx->models.emplace_back();
     Model &m = ctx->models.back();
@@ -304,6 +307,7 @@ int bioem_push_images(bioem_ctx *ctx, int n_img, const float *pixels, int is_dev
     CK(ctx->Dw.ensure((size_t)n_img * sizeof(double)));
     CK(ctx->beta.ensure((size_t)n_img * sizeof(float)));
     CK(ctx->scratch_a.ensure((size_t)slab * n * sizeof(double)));       // centred images
+    if (ctx->variant == 1) CK(ctx->Oreal64.ensure((size_t)n_img * n * sizeof(double)));     // the real-space variant keeps them
     CK(ctx->scratch_b.ensure((size_t)slab * H * sizeof(cd)));           // transform intermediate
     const float *dsrc = pixels;
     if (!is_device) {
@@ -315,8 +319,9 @@ int bioem_push_images(bioem_ctx *ctx, int n_img, const float *pixels, int is_dev
     CK(cudaMemsetAsync(ctx->flags.p, 0, sizeof(int), st));
     for (int i0 = 0; i0 < n_img; i0 += slab) {
         const int nb = std::min(slab, n_img - i0);
-        CK(launch_image_stats(dsrc + (size_t)i0 * n, nb, N, ctx->scratch_a.as<double>(), ctx->Dw.as<double>() + i0, st));
-        CK(launch_fft2_r2c_f64(ctx->scratch_a.as<double>(), nb, N, ctx->scratch_b.as<cd>(), ctx->Ohat64.as<cd>() + (size_t)i0 * H, st));
+        double *cent = ctx->variant == 1 ? ctx->Oreal64.as<double>() + (size_t)i0 * n : ctx->scratch_a.as<double>();
+        CK(launch_image_stats(dsrc + (size_t)i0 * n, nb, N, cent, ctx->Dw.as<double>() + i0, st));
+        CK(launch_fft2_r2c_f64(cent, nb, N, ctx->scratch_b.as<cd>(), ctx->Ohat64.as<cd>() + (size_t)i0 * H, st));
         CK(launch_zero_dc(ctx->Ohat64.as<cd>() + (size_t)i0 * H, nb, H, st));
     }
     CK(launch_cast_spectrum(ctx->Ohat64.as<cd>(), ctx->Ohat32.as<cf>(), (size_t)n_img * H, st));
@@ -330,6 +335,7 @@ int bioem_push_images(bioem_ctx *ctx, int n_img, const float *pixels, int is_dev
     }
     ctx->push_launches = 4 * (int64_t)((n_img + slab - 1) / slab) + 2;
     ctx->n_img = n_img;
+    ctx->img_variant = ctx->variant;
     ctx->ran = false; ctx->phase = 0;
     return BIOEM_OK;
 }
@@ -344,7 +350,7 @@ static int choose_oc(long long n_img, long long n_model, long long n_orient, int
     return (int)oc;
 }
 
-enum { KERNEL_AUTO = 0, KERNEL_GENERIC = 1, KERNEL_PK = 2, KERNEL_C2 = 3, KERNEL_TM = 4 };
+enum { KERNEL_AUTO = 0, KERNEL_GENERIC = 1, KERNEL_PK = 2, KERNEL_C2 = 3, KERNEL_TM = 4, KERNEL_DFT = 5, KERNEL_REALSPACE = 6 };
 
 // the fused kernel a run of (N, D) uses: the one asked for if it supports the shape, else the automatic choice
 static int choose_kernel(int N, int D, int user)
@@ -477,6 +483,62 @@ int bioem_run_partial(bioem_ctx *ctx)
         }
     }
 
+    if (ctx->variant == 1) {
+        // ---- the real-space, cropping variant: FP64 scoring of every calculated image against every image
+        if (sliced || ctx->want_orient) FAIL(BIOEM_EUNSUPPORTED, "run: the real-space variant supports neither orientation slices nor the per-orientation posterior");
+        if (ctx->img_variant != 1) FAIL(BIOEM_EBADSTATE, "run: set the displacement variant before bioem_push_images (the real-space variant keeps the images in real space)");
+        const int S = (2 * D + 1) * (2 * D + 1), RB = 64;                 // calculated images per batch
+        const size_t IM = (size_t)I * M;
+        CK(ctx->rs_T.ensure((size_t)RB * H * sizeof(cd)));
+        CK(ctx->rs_I1.ensure((size_t)RB * n * sizeof(double)));
+        CK(ctx->rs_cc.ensure((size_t)RB * S * sizeof(double)));
+        CK(ctx->rs_ccc.ensure((size_t)RB * S * sizeof(double)));
+        CK(ctx->rs_part.ensure(rs_partial_bytes(RB, I)));
+        CK(ctx->rs_logw.ensure(RB * sizeof(double)));
+        CK(ctx->rs_pair.ensure(RB * sizeof(long long)));
+        CK(ctx->rs_m.ensure(IM * sizeof(double)));
+        CK(ctx->rs_s.ensure(IM * sizeof(double)));
+        CK(ctx->rs_best.ensure(IM * sizeof(double)));
+        CK(ctx->rs_bpair.ensure(IM * sizeof(long long)));
+        CK(ctx->rs_bshift.ensure(IM * sizeof(int)));
+        CK(ctx->logp.ensure(IM * sizeof(double)));
+        CK(ctx->logp32.ensure(IM * sizeof(double)));
+        CK(ctx->best.ensure(IM * 4 * sizeof(int32_t)));
+        CK(ctx->best_logp.ensure(IM * sizeof(double)));
+        CK(cudaEventRecord(ctx->ev[1], st));
+        CK(launch_rs_init((int)IM, ctx->rs_m.as<double>(), ctx->rs_s.as<double>(), ctx->rs_best.as<double>(), ctx->rs_bpair.as<long long>(),
+                          ctx->rs_bshift.as<int>(), st));
+        ctx->launches += 1;
+        for (int mi = 0; mi < M; ++mi)
+            for (int o0 = 0; o0 < O; o0 += RB) {
+                const int nb = std::min(RB, O - o0);
+                for (int c = 0; c < C; ++c) {
+                    CK(launch_rs_calc_images(ctx->F064.as<cd>() + ((size_t)mi * O + o0) * H, ctx->K64.as<double>() + (size_t)c * H, nb, N,
+                                             ctx->rs_T.as<cd>(), ctx->rs_I1.as<double>(), st));
+                    CK(launch_rs_batch_meta(ctx->h64.as<double>(), ctx->Tc64.as<double>(), mi, O, C, o0, c, nb, ctx->rs_logw.as<double>(),
+                                            ctx->rs_pair.as<long long>(), st));
+                    CK(launch_rs_score(ctx->Oreal64.as<double>(), ctx->Dw.as<double>(), ctx->rs_I1.as<double>(), ctx->rs_logw.as<double>(),
+                                       ctx->rs_pair.as<long long>(), nb, I, M, mi, N, D, ctx->rs_cc.as<double>(), ctx->rs_ccc.as<double>(), ctx->rs_part.p,
+                                       ctx->rs_m.as<double>(), ctx->rs_s.as<double>(), ctx->rs_best.as<double>(), ctx->rs_bpair.as<long long>(),
+                                       ctx->rs_bshift.as<int>(), ctx->flags.as<int>() + 1, st));
+                    ctx->launches += 6; ctx->fused_launches += 1;
+                }
+            }
+        CK(cudaEventRecord(ctx->ev[2], st));
+        const double nn = (double)n;
+        const double const_n = -0.5 * (nn - 2.0) * std::log(2.0 * M_PI) + 0.5 * (nn - 5.0) * std::log(2.0) + std::lgamma(0.5 * (nn - 3.0));
+        CK(launch_rs_final(ctx->rs_m.as<double>(), ctx->rs_s.as<double>(), ctx->rs_best.as<double>(), ctx->rs_bpair.as<long long>(),
+                           ctx->rs_bshift.as<int>(), ctx->Dw.as<double>(), I, M, C, N, D, const_n, ctx->logp.as<double>(), ctx->logp32.as<double>(),
+                           ctx->best.as<int32_t>(), ctx->best_logp.as<double>(), st));
+        ctx->launches += 1;
+        CK(cudaEventRecord(ctx->ev[3], st));
+        ctx->pre_valid = true; ctx->flags_checked = false;
+        ctx->run_kernel = KERNEL_REALSPACE; ctx->run_oc = 0; ctx->run_o_first = 0; ctx->run_o_local = O; ctx->run_chunks = 0;
+        ctx->run_models = M; ctx->run_orient = Ofull; ctx->run_ctf = C; ctx->run_D = D; ctx->run_img = I;
+        ctx->ran = true; ctx->ran_orient = false; ctx->phase = 4;
+        return BIOEM_OK;
+    }
+
     // ---- a4-a6: the fused kernel
     FusedParams p{};
     p.Ohat = ctx->Ohat32.as<cf>(); p.F0 = ctx->F032.as<cf>(); p.K = ctx->K32.as<float>();
@@ -505,6 +567,7 @@ int bioem_get_partials_size(bioem_ctx *ctx, int64_t *n_bytes, int32_t *n_chunks)
 {
     if (!ctx) return BIOEM_EBADARG;
     if (ctx->phase < 1) FAIL(BIOEM_EBADSTATE, "get_partials_size: call bioem_run_partial first");
+    if (ctx->run_kernel == KERNEL_REALSPACE) FAIL(BIOEM_EBADSTATE, "the real-space variant has no partials");
     if (n_bytes) *n_bytes = (int64_t)partial_blob_bytes((size_t)ctx->run_img * ctx->run_models * ctx->run_chunks);
     if (n_chunks) *n_chunks = ctx->run_chunks;
     return BIOEM_OK;
@@ -514,6 +577,7 @@ int bioem_export_partials(bioem_ctx *ctx, void *dst, int is_device)
 {
     if (!ctx || !dst) return BIOEM_EBADARG;
     if (ctx->phase < 1) FAIL(BIOEM_EBADSTATE, "export_partials: call bioem_run_partial first");
+    if (ctx->run_kernel == KERNEL_REALSPACE) FAIL(BIOEM_EBADSTATE, "the real-space variant has no partials");
     CK(cudaSetDevice(ctx->device));
     const size_t bytes = partial_blob_bytes((size_t)ctx->run_img * ctx->run_models * ctx->run_chunks);
     if (bytes) CK(cudaMemcpyAsync(dst, ctx->blob.p, bytes, is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, ctx->stream));
@@ -526,6 +590,7 @@ int bioem_merge_partials(bioem_ctx *ctx, int n_blobs, const void *blobs, int64_t
 {
     if (!ctx) return BIOEM_EBADARG;
     if (ctx->phase < 1) FAIL(BIOEM_EBADSTATE, "merge_partials: call bioem_run_partial first");
+    if (ctx->run_kernel == KERNEL_REALSPACE) FAIL(BIOEM_EBADSTATE, "the real-space variant has no partials");
     CK(cudaSetDevice(ctx->device));
     cudaStream_t st = ctx->stream;
     const int I = ctx->run_img, M = ctx->run_models;
@@ -568,6 +633,7 @@ int bioem_rescore_local(bioem_ctx *ctx)
 {
     if (!ctx) return BIOEM_EBADARG;
     if (ctx->phase < 2) FAIL(BIOEM_EBADSTATE, "rescore_local: call bioem_merge_partials first");
+    if (ctx->run_kernel == KERNEL_REALSPACE) FAIL(BIOEM_EBADSTATE, "the real-space variant has no re-scoring step");
     CK(cudaSetDevice(ctx->device));
     const int I = ctx->run_img, M = ctx->run_models;
     CK(ctx->g64.ensure((size_t)I * M * BIOEM_TOPK * sizeof(double)));
@@ -642,10 +708,20 @@ int bioem_run(bioem_ctx *ctx)
     if (ctx->slice_end >= 0 && !(ctx->slice_begin == 0 && ctx->slice_end == ctx->n_orient))
         FAIL(BIOEM_EBADSTATE, "run: an orientation slice is set: this context holds part of the grid (use the phased calls, or clear the slice)");
     int rc = bioem_run_partial(ctx);
+    if (!rc && ctx->variant == 1) return BIOEM_OK;                       // the real-space variant has no partials: run_partial finished the run
     if (!rc) rc = bioem_merge_partials(ctx, 0, nullptr, 0, nullptr, 1);
     if (!rc) rc = bioem_rescore_local(ctx);
     if (!rc) rc = bioem_finish(ctx);
     return rc;
+}
+
+int bioem_set_displacement_variant(bioem_ctx *ctx, int variant)
+{
+    if (!ctx) return BIOEM_EBADARG;
+    if (variant != 0 && variant != 1) FAIL(BIOEM_EBADARG, "set_displacement_variant: 0 (Fourier space, circular) or 1 (real space, cropping)");
+    ctx->variant = variant;
+    ctx->ran = false; ctx->phase = 0;
+    return BIOEM_OK;
 }
 
 int bioem_set_orientation_slice(bioem_ctx *ctx, int o_begin, int o_end)
@@ -788,6 +864,7 @@ int bioem_debug_shift_map(bioem_ctx *ctx, int img, int model, int orient, int ct
     if (!ctx || !out) return BIOEM_EBADARG;
     int rc = check_tuple(ctx, img, model, orient, ctf);
     if (rc) return rc;
+    if (ctx->run_kernel == KERNEL_REALSPACE) FAIL(BIOEM_EUNSUPPORTED, "debug_shift_map: the last run used the real-space variant (FP64 throughout, no FP32 map)");
     CK(cudaSetDevice(ctx->device));
     const int N = ctx->N, D = ctx->run_D, KK = 2 * D + 1;
     const size_t n = (size_t)N * N;

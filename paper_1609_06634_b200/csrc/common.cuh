@@ -24,7 +24,12 @@ typedef cx<double> cd;
 struct TopEntry { float g; uint32_t pair; uint32_t shift; };   // g in BASE-2 units (log2 of the term); pair = o*C + c within the model, shift = (dy+D)*S1 + (dx+D)
 
 // choice of the two-step factorisation N = N1 * N2 per supported image size
-__host__ __device__ constexpr int n1_of(int N) { return N == 64 ? 16 : N == 128 ? 16 : N == 224 ? 32 : N == 256 ? 32 : 0; }
+// (N1 a power of two for the register transform, N2 = N / N1 any; 170 = 2 x 85, the GroEL box of the paper's Table 1, P:229,
+// runs as a short radix-2 stage plus 85-term direct sums: correct for any even size, fast only where N1 is large)
+__host__ __device__ constexpr int n1_of(int N)
+{
+    return N == 64 ? 16 : N == 128 ? 16 : N == 224 ? 32 : N == 256 ? 32 : N == 96 ? 32 : N == 160 ? 32 : N == 192 ? 32 : N == 170 ? 2 : 0;
+}
 
 struct FusedParams {
     // inputs
@@ -100,5 +105,18 @@ cudaError_t launch_orient_final(const float *part_m, const float *part_s, int pa
 cudaError_t launch_ensemble(const double *logp, const double *logw, int n_img, int n_model, double *per_image, double *total, cudaStream_t st);
 cudaError_t launch_calc_image(const cd *F0, const double *K64, int N, double *out, cudaStream_t st);
 cudaError_t launch_fp32_peak(float *sink, int iters, cudaStream_t st);
+
+// real-space, cropping displacement variant (realspace.cu)
+size_t rs_partial_bytes(int nb, int n_img);
+cudaError_t launch_rs_calc_images(const cd *F0, const double *K, int nb, int N, cd *T, double *I1, cudaStream_t st);
+cudaError_t launch_rs_batch_meta(const double *h64, const double *Tc64, int model, int n_orient, int n_ctf, int o0, int c, int nb, double *logw,
+                                 long long *pair_of, cudaStream_t st);
+cudaError_t launch_rs_score(const double *Oc, const double *Dw, const double *I1, const double *logw, const long long *pair_of, int nb, int n_img,
+                            int n_model, int model, int N, int D, double *cc, double *ccc, void *part, double *acc_m, double *acc_s,
+                            double *acc_best, long long *acc_pair, int *acc_shift, int *flags, cudaStream_t st);
+cudaError_t launch_rs_init(int n, double *acc_m, double *acc_s, double *acc_best, long long *acc_pair, int *acc_shift, cudaStream_t st);
+cudaError_t launch_rs_final(const double *acc_m, const double *acc_s, const double *acc_best, const long long *acc_pair, const int *acc_shift,
+                            const double *Dw, int n_img, int n_model, int n_ctf, int N, int D, double const_n, double *logp, double *logp32,
+                            int32_t *best, double *best_logp, cudaStream_t st);
 
 }  // namespace bioem

@@ -236,7 +236,7 @@ __global__ void __launch_bounds__(NT) k_fused(FusedParams p, int CB, int GP)
 }
 
 // ---------------------------------------------------------------------------------------------------- host side
-static int nt_of(int N) { return N == 64 ? 256 : 512; }
+static int nt_of(int N) { return N == 64 || N == 96 ? 256 : 512; }
 
 static void smem_plan(int N, int D, int &CB, int &GP, size_t &bytes)
 {
@@ -289,6 +289,10 @@ cudaError_t launch_fused(int N, const FusedParams &p, bool dump, cudaStream_t st
     case 128: return launch_t<128, 512>(p, dump, st);
     case 224: return launch_t<224, 512>(p, dump, st);
     case 256: return launch_t<256, 512>(p, dump, st);
+    case 96: return launch_t<96, 256>(p, dump, st);
+    case 160: return launch_t<160, 512>(p, dump, st);
+    case 170: return launch_t<170, 512>(p, dump, st);
+    case 192: return launch_t<192, 512>(p, dump, st);
     }
     return cudaErrorInvalidValue;
 }

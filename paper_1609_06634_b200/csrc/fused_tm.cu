@@ -43,7 +43,7 @@ struct TM {
     static constexpr int N = 224, NCOLP = 112, NTASK = 28;        // packed columns (column 0 carries the Nyquist column l = 112); tasks of 4 columns
     static constexpr int NW = 16, NT = NW * 32, NCONS = 12;       // warps; warps that consume G_T (B, C, D)
     static constexpr int ZP = 18, ZW = 32 * ZP;                   // Z tile: one row of 16 outputs per lane (pitch even: 16-byte rows; lanes 28..31 carry zeros)
-    static constexpr int RP = 66, GSZ = NCOLP * RP;               // G_T [column][row'] pitch (even: 16-byte row pairs; 8 RP = 16 mod 128: the mirrored loads of pass 2 are conflict-free)
+    static constexpr int RP = 66, GSZ = (NCOLP + 1) * RP;               // G_T [column][row'] pitch (even: 16-byte row pairs; 8 RP = 16 mod 128: the mirrored loads of pass 2 are conflict-free)
 };
 
 // ---- tensor memory as per-thread scratch (32x32b: thread i of warp w owns lane 32 (w % 4) + i, all 512 columns)
@@ -97,8 +97,15 @@ __device__ __forceinline__ void tm_horner7x4(c2 (&y)[4], const c2 *zc, c2 r_lo, 
 
 // The four pass-1 outputs of a lane -> rows of G_T.  Lanes whose output index lies outside |k| <= D do not store (predicated
 // stores: a dummy address for them put a second wavefront on every store, profiles/r2_tm_v8).
-__device__ __forceinline__ void tm_store_rows(c2 *g_lo, c2 *g_hi, bool v_lo, bool v_hi, const c2 (&y)[4])
+// `unpack` (the lanes of warp 0 that hold packed column 0): y = G(., 0) + i G(., 112), both parts real -> two real columns
+// (0 and 112 of G_T), so that pass 2 reads column 0 and the Nyquist column like any other: no special case in its load loop.
+__device__ __forceinline__ void tm_store_rows(c2 *g_lo, c2 *g_hi, bool v_lo, bool v_hi, const c2 (&y)[4], bool unpack = false)
 {
+    if (unpack) {
+        if (v_lo) { g_lo[0] = make_float2(y[0].x, 0.f); g_lo[112 * TM::RP] = make_float2(y[0].y, 0.f); g_lo[TM::RP] = y[2]; }
+        if (v_hi) { g_hi[0] = make_float2(y[1].x, 0.f); g_hi[112 * TM::RP] = make_float2(y[1].y, 0.f); g_hi[TM::RP] = y[3]; }
+        return;
+    }
     if (v_lo) { g_lo[0] = y[0]; g_lo[TM::RP] = y[2]; }
     if (v_hi) { g_hi[0] = y[1]; g_hi[TM::RP] = y[3]; }
 }
@@ -207,7 +214,7 @@ __device__ __forceinline__ void tm_score_commit(const TmScore &sc, const FusedPa
 // is G(., 0) + i G(., 112) with both parts real).
 template <bool ODD, bool NYQ, bool BACK>
 __device__ __forceinline__ void tm_p1_slot(c2 (&a)[16], uint32_t qaddr, const float4 (&kq)[8], bool nyq, const c2 *qn, const float *__restrict__ kn,
-                                           const c2 *zrd, c2 r_lo, c2 r_hi, c2 *g_lo, c2 *g_hi, bool v_lo, bool v_hi)
+                                           const c2 *zrd, c2 r_lo, c2 r_hi, c2 *g_lo, c2 *g_hi, bool v_lo, bool v_hi, bool unpack = false)
 {
     uint32_t qa[2][8], qb[2][8];
     tm_ld8(qaddr, qa[0]);
@@ -215,7 +222,7 @@ __device__ __forceinline__ void tm_p1_slot(c2 (&a)[16], uint32_t qaddr, const fl
     if (BACK) {
         c2 y[4];
         tm_horner7x4(y, zrd, r_lo, r_hi);
-        tm_store_rows(g_lo, g_hi, v_lo, v_hi, y);
+        tm_store_rows(g_lo, g_hi, v_lo, v_hi, y, unpack);
     }
 #pragma unroll
     for (int g = 0; g < 4; ++g) {
@@ -244,8 +251,8 @@ __device__ __forceinline__ void tm_p1_slot(c2 (&a)[16], uint32_t qaddr, const fl
 
 // Radix-2 stage + 16-point transform of a pass-2 half-task for one row pair: the 224-point transform along l of A + i B (rows'
 // 2p, 2p+1 of G_T, one 128-bit word per column; a row' that does not exist is all zero), thread = (pair, residue t),
-// l = 7 j + t.  Columns l = 1..111 are stored, l = 113..223 are their conjugates (Hermitian half); packed column 0 holds
-// (G(., 0), G(., 112)), both real.  ODD = false: a_j = x_j + x_(j+16) (even dx); ODD = true: a_j = (x_j - x_(j+16)) w32^j (odd dx).
+// l = 7 j + t.  Columns l = 1..111 are stored, l = 113..223 are their conjugates (Hermitian half); columns 0 and 112 are real (pass 1
+// unpacks them from packed column 0 on store): both formulas below then give (A.x, B.x).  ODD = false: a_j = x_j + x_(j+16) (even dx); ODD = true: a_j = (x_j - x_(j+16)) w32^j (odd dx).
 // (Lane = 8 pair + t and 8 RP = 16 mod 128: the eight lanes of a quarter-warp read eight different 16-byte slots, direct and
 // mirrored.)  A warp that does both parities loads twice: keeping the other half in registers spills (profiles/r2_tm_v7b).
 template <bool ODD>
@@ -255,14 +262,10 @@ __device__ __forceinline__ void tm_p2_front(c2 (&a)[16], const c2 *gt, int t)
 #pragma unroll
     for (int j = 0; j < 16; ++j) {
         const float4 vl = *reinterpret_cast<const float4 *>(gl + 7 * j * TM::RP);
-        const float4 vh = *reinterpret_cast<const float4 *>((j == 0 && t == 0) ? gt : gh - 7 * j * TM::RP);
+        const float4 vh = *reinterpret_cast<const float4 *>(gh - 7 * j * TM::RP);
         // direct: A + i B = (A.x - B.y, A.y + B.x); mirrored: conj(A) + i conj(B) = (A.x + B.y, -A.y + B.x)
         c2 xl = pk_add(make_float2(vl.x, vl.y), make_float2(-vl.w, vl.z));
         c2 xh = pk_add(make_float2(vh.x, -vh.y), make_float2(vh.w, vh.z));
-        if (j == 0 && t == 0) {                           // packed column: l = 0 -> (A.x, B.x), l = 112 -> (A.y, B.y)
-            xl = make_float2(vl.x, vl.z);
-            xh = make_float2(vl.y, vl.w);
-        }
         a[j] = ODD ? pk_twid(pk_sub(xl, xh), j) : pk_add(xl, xh);
     }
     pk_fft16(a);
@@ -347,6 +350,7 @@ __global__ void __launch_bounds__(TM::NT, 1) k_fused_tm(FusedParams p, const flo
     const bool do_ev = role == 1 || role == 3, do_od = role == 2 || role == 3, cons = role != 0;
     const uint32_t qaddr0 = tm_base + ((uint32_t)(32 * sk) << 16) + (uint32_t)(128 * role);
     const bool warp_nyq = warp == 0, nyq = warp_nyq && lane < 7;
+    const bool unpack0 = warp_nyq && c2h == 0;                        // the H-phase lanes whose first column is packed column 0
     const cf *Oimg = p.Ohat + (size_t)img * H;
     const float beta = p.beta[img];
     const float4 *kt_l = Kt + lane;                                   // Kt[c][task 0..27][g 0..7][lane]
@@ -405,7 +409,7 @@ __global__ void __launch_bounds__(TM::NT, 1) k_fused_tm(FusedParams p, const flo
                     if (i == 0) {
                         if (warp_nyq) tm_p1_slot<false, true, false>(a, qaddr0, kq, nyq, qn + t, KtN + (size_t)c * N + t, zrd, wl_od, wh_od, g_lo, g_hi, vl_od, vh_od);
                         else tm_p1_slot<false, false, false>(a, qaddr0, kq, false, nullptr, nullptr, zrd, wl_od, wh_od, g_lo, g_hi, vl_od, vh_od);
-                    } else tm_p1_slot<false, false, true>(a, qaddr0 + 64, kq, false, nullptr, nullptr, zrd, wl_od, wh_od, g_lo, g_hi, vl_od, vh_od);
+                    } else tm_p1_slot<false, false, true>(a, qaddr0 + 64, kq, false, nullptr, nullptr, zrd, wl_od, wh_od, g_lo, g_hi, vl_od, vh_od, unpack0);
                 }
                 __syncwarp();                                         // every lane has read the tile
                 pk_spill16(zrow, a);
@@ -415,7 +419,7 @@ __global__ void __launch_bounds__(TM::NT, 1) k_fused_tm(FusedParams p, const flo
                 {
                     c2 *gp = Gw + (size_t)col0 * RP;
                     c2 *g_lo = gp + rl_ev, *g_hi = gp + rh_ev;
-                    if (warp_nyq && i == 0) tm_p1_slot<true, true, true>(a, qaddr0, kq, nyq, qn + t, KtN + (size_t)c * N + t, zrd, wl_ev, wh_ev, g_lo, g_hi, vl_ev, vh_ev);
+                    if (warp_nyq && i == 0) tm_p1_slot<true, true, true>(a, qaddr0, kq, nyq, qn + t, KtN + (size_t)c * N + t, zrd, wl_ev, wh_ev, g_lo, g_hi, vl_ev, vh_ev, unpack0);
                     else tm_p1_slot<true, false, true>(a, qaddr0 + 64 * i, kq, false, nullptr, nullptr, zrd, wl_ev, wh_ev, g_lo, g_hi, vl_ev, vh_ev);
                 }
                 {

@@ -120,6 +120,10 @@ static cudaError_t fft1d(int N, const void *in, long ibs, long iss, long ies, cd
     case 128: k_fft1d_f64<128, SIGN, REAL_IN, SPB><<<grid, SPB * 8, 0, st>>>(in, ibs, iss, ies, out, obs, oss, oes, nseq, spb, kout); break;
     case 224: k_fft1d_f64<224, SIGN, REAL_IN, SPB><<<grid, SPB * 7, 0, st>>>(in, ibs, iss, ies, out, obs, oss, oes, nseq, spb, kout); break;
     case 256: k_fft1d_f64<256, SIGN, REAL_IN, SPB><<<grid, SPB * 8, 0, st>>>(in, ibs, iss, ies, out, obs, oss, oes, nseq, spb, kout); break;
+    case 96: k_fft1d_f64<96, SIGN, REAL_IN, SPB><<<grid, SPB * 3, 0, st>>>(in, ibs, iss, ies, out, obs, oss, oes, nseq, spb, kout); break;
+    case 160: k_fft1d_f64<160, SIGN, REAL_IN, SPB><<<grid, SPB * 5, 0, st>>>(in, ibs, iss, ies, out, obs, oss, oes, nseq, spb, kout); break;
+    case 170: k_fft1d_f64<170, SIGN, REAL_IN, SPB><<<grid, SPB * 85, 0, st>>>(in, ibs, iss, ies, out, obs, oss, oes, nseq, spb, kout); break;
+    case 192: k_fft1d_f64<192, SIGN, REAL_IN, SPB><<<grid, SPB * 6, 0, st>>>(in, ibs, iss, ies, out, obs, oss, oes, nseq, spb, kout); break;
     default: return cudaErrorInvalidValue;
     }
     return cudaGetLastError();

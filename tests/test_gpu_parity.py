@@ -564,3 +564,71 @@ def test_image_subsets_reuse_the_calculated_images():
         b.push_images(wl["images"])
         b.run()
         assert np.array_equal(b.get_log_posterior(), whole[0])
+
+
+@pytest.mark.parametrize("name,D", [("tiny_mini", 4), ("small_mini", 2), ("paper_mini", 1), ("density_mini", 2), ("ensemble_mini", 3)])
+def test_real_space_cropping_variant(name, D):
+    """the real-space displacement variant against the oracle's tier 2 (bo_cropped_sums),
+    element by element; FP64 on both sides, so the tolerance is that of the FP64 shift maps, and the argmax is identical.
+    The variant differs from the circular one on these inputs (the CTF spreads the calculated image to the borders)."""
+    import oracle
+    from paper_1609_06634_b200 import BioEM
+    wl = W.build_workload(name)
+    s = wl["spec"]
+    states = [oracle.run_model(m, s.n_pix, s.pixel_A, D, wl["quats"], wl["ctfs"], wl["images"], tier=2) for m in wl["models"]]
+    want = np.stack([st.log_posterior() for st in states], axis=1)
+    o, c, dx, dy = (np.stack(x, axis=1) for x in zip(*[oracle.unflatten(st.best_flat, s.n_ctf, D) for st in states]))
+    with BioEM() as b:
+        b.load_workload(wl, images=False)
+        b.set_shift_range(D)
+        b.set_displacement_variant(1)
+        b.push_images(wl["images"])
+        b.run()
+        got, best = b.get_log_posterior(), b.get_best()
+        assert b.get_run_plan()[0] == 6
+        b.set_displacement_variant(0)
+        b.push_images(wl["images"])
+        b.run()
+        circ = b.get_log_posterior()
+    assert np.abs(got - want).max() <= 1e-6, np.abs(got - want).max()
+    assert np.array_equal(best["orient"], o) and np.array_equal(best["ctf"], c) and np.array_equal(best["dx"], dx) and np.array_equal(best["dy"], dy)
+    assert np.abs(best["log_p"] - np.stack([st.best for st in states], axis=1)).max() <= 1e-6
+    assert np.abs(got - circ).max() > 1e-4                                   # not the circular variant
+
+
+def test_real_space_variant_needs_its_images():
+    from paper_1609_06634_b200 import BioEM
+    from paper_1609_06634_b200.binding import BioEMError
+    wl = W.build_workload("tiny_mini")
+    with BioEM() as b:
+        b.load_workload(wl)
+        b.set_displacement_variant(1)                                        # after push_images: the real-space images were not kept
+        with pytest.raises(BioEMError):
+            b.run()
+        b.push_images(wl["images"])
+        b.run()
+        assert np.all(np.isfinite(b.get_log_posterior()))
+
+
+@pytest.mark.parametrize("n_pix", [170, 96, 160, 192])
+def test_other_box_sizes(n_pix):
+    """box sizes beyond the four of round 1 -- 170^2 is the GroEL set of the paper's Table 1, 2 x 5 x 17.
+    log P, argmax, one FP32 / FP64 shift map and one calculated image against the oracle, element by element."""
+    import oracle
+    from paper_1609_06634_b200 import BioEM
+    wl = W.build_workload(f"box{n_pix}_mini")
+    s = wl["spec"]
+    ref, got = _check(wl)
+    with BioEM() as b:
+        b.load_workload(wl)
+        b.run()
+        assert b.get_run_plan()[0] == 1                                      # the generic two-step kernel
+        m = oracle.prepare_model(wl["models"][0])
+        o, c, img = s.n_orient - 1, s.n_ctf - 1, 1
+        I1 = oracle.calc_image(m, wl["quats"][o], wl["ctfs"][c], s.n_pix, s.pixel_A)
+        mine = b.debug_calc_image(0, o, c)
+        assert np.abs(mine - I1).max() <= 2e-6 * np.abs(I1).max()
+        logw = oracle.uniform_logw(len(wl["quats"]), len(wl["ctfs"]), s.max_shift)
+        want = oracle.shift_map(wl["images"][img], I1, s.max_shift, logw)
+        assert np.abs(b.debug_shift_map_f64(img, 0, o, c) - want).max() <= 1e-6
+        assert np.abs(b.debug_shift_map(img, 0, o, c) - want).max() <= 5e-7 * s.n_pix ** 2 + 1e-3

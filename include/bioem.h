@@ -196,8 +196,9 @@ int bioem_debug_log_posterior_f32(bioem_ctx *ctx, double *out);
 /* CUDA-event times of the last bioem_run [ms]: whole run, fused kernel only; number of kernel launches. */
 int bioem_get_timing(bioem_ctx *ctx, double *ms_total, double *ms_fused_kernel);
 int bioem_get_launch_count(bioem_ctx *ctx, int64_t *n_launches, int64_t *n_fused_launches);
-/* FP32 FMA rate of this device measured with a register-resident FFMA loop [TFLOP/s] and the SM clock [MHz]
- * seen while it ran (bench.py's "alu" roofline denominator). */
+/* FP32 FMA rate of this device measured with a register-resident FFMA loop [TFLOP/s] (context for bench.py's "alu" roofline,
+ * whose denominator is the formula peak) and the device's MAXIMUM SM clock [MHz] (cudaDevAttrClockRate, not a clock sampled
+ * while the loop ran: bench.py samples nvidia-smi for that). */
 int bioem_measure_fp32_peak(bioem_ctx *ctx, double *tflops, double *sm_mhz);
 
 #ifdef __cplusplus

@@ -164,7 +164,8 @@ cudaError_t launch_zero_dc(cd *spec, int batch, size_t H, cudaStream_t st)
 }
 
 // ------------------------------------------------------------------------------------------------ a1: Eq. 1, R10-R12
-// One CTA per orientation; each thread takes atoms.  The pixel integral is the 4x4 mid-point sum of the chord length
+// grid = (orientation, block of 256 atoms): one thread per atom, so that a batch of 256 orientations of a 3000-atom model is
+// 3072 CTAs and not 256 (round 1: one CTA per orientation, 1.7 CTAs per SM, bound by the latency of the FP64 square roots).  The pixel integral is the 4x4 mid-point sum of the chord length
 // 2 sqrt(R^2 - r^2)_+ (R10), accumulated as 64-bit FIXED-POINT integers with atomics: integer addition is associative,
 // so the image is bit-identical from run to run whatever the order of the atoms (no float atomics).
 __global__ void __launch_bounds__(256) k_project(const double *xyz, const double *rad, const double *wt, int n_atoms, const double *rot,
@@ -174,7 +175,7 @@ __global__ void __launch_bounds__(256) k_project(const double *xyz, const double
     unsigned long long *img = reinterpret_cast<unsigned long long *>(acc) + (size_t)blockIdx.x * N * N;
     constexpr int KQ = 4;
     const double h = px / KQ;
-    for (int a = threadIdx.x; a < n_atoms; a += 256) {
+    for (int a = blockIdx.y * 256 + threadIdx.x; a < n_atoms; a += 256 * gridDim.y) {
         const double x0 = xyz[3 * a], y0 = xyz[3 * a + 1], z0 = xyz[3 * a + 2];
         const double xr = R[0] * x0 + R[1] * y0 + R[2] * z0;
         const double yr = R[3] * x0 + R[4] * y0 + R[5] * z0;
@@ -222,7 +223,7 @@ cudaError_t launch_project_atoms(const double *xyz, const double *rad, const dou
     size_t n = (size_t)n_orient * N * N;
     cudaError_t e = cudaMemsetAsync(acc, 0, n * sizeof(long long), st);
     if (e != cudaSuccess) return e;
-    k_project<<<n_orient, 256, 0, st>>>(xyz, rad, wt, n_atoms, rot, N, px, fx_scale, acc);
+    k_project<<<dim3(n_orient, (n_atoms + 255) / 256), 256, 0, st>>>(xyz, rad, wt, n_atoms, rot, N, px, fx_scale, acc);
     k_fixed_to_double<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(acc, out, n, 1.0 / fx_scale);
     return cudaGetLastError();
 }

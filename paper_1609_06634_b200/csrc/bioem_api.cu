@@ -444,7 +444,7 @@ int bioem_run_partial(bioem_ctx *ctx)
         }
 
         // ---- a1/a1' + a2: spectra of the projections of the resident orientations, model by model, batch by batch
-        const int OB = 256;
+        const int OB = 1024;                                          // orientations per projection batch (scratch: 40 bytes per pixel and orientation)
         const double *rot = ctx->rot.as<double>() + (size_t)o_first * 9;
         for (int mi = 0; mi < M && O > 0; ++mi) {
             Model &m = ctx->models[mi];

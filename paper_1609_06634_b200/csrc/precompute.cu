@@ -109,24 +109,35 @@ __global__ void __launch_bounds__(SPB *(N / n1_of(N))) k_fft1d_f64(const void *i
     }
 }
 
+// sequences per block: as many as keep the Z tile under ~35 KB of static shared memory, so that the block's twiddle table
+// (N sincospi) is shared by 8-32 sequences and not by 4 (round 1: 32-thread blocks; the transforms of the 73 728 Ensemble
+// projections took 25 ms)
+__host__ __device__ constexpr int spb_of(int N) { return N == 64 ? 32 : N == 128 ? 16 : N == 96 ? 16 : N == 170 ? 4 : 8; }
+
+template <int N, int SIGN, bool REAL_IN>
+static cudaError_t fft1d_n(const void *in, long ibs, long iss, long ies, cd *out, long obs, long oss, long oes, int nseq, int spb, int kout,
+                           cudaStream_t st)
+{
+    constexpr int SPB = spb_of(N);
+    k_fft1d_f64<N, SIGN, REAL_IN, SPB><<<(nseq + SPB - 1) / SPB, SPB * (N / n1_of(N)), 0, st>>>(in, ibs, iss, ies, out, obs, oss, oes, nseq, spb, kout);
+    return cudaGetLastError();
+}
+
 template <int SIGN, bool REAL_IN>
 static cudaError_t fft1d(int N, const void *in, long ibs, long iss, long ies, cd *out, long obs, long oss, long oes, int nseq,
                          int spb, int kout, cudaStream_t st)
 {
-    constexpr int SPB = 4;
-    int grid = (nseq + SPB - 1) / SPB;
     switch (N) {
-    case 64: k_fft1d_f64<64, SIGN, REAL_IN, SPB><<<grid, SPB * 4, 0, st>>>(in, ibs, iss, ies, out, obs, oss, oes, nseq, spb, kout); break;
-    case 128: k_fft1d_f64<128, SIGN, REAL_IN, SPB><<<grid, SPB * 8, 0, st>>>(in, ibs, iss, ies, out, obs, oss, oes, nseq, spb, kout); break;
-    case 224: k_fft1d_f64<224, SIGN, REAL_IN, SPB><<<grid, SPB * 7, 0, st>>>(in, ibs, iss, ies, out, obs, oss, oes, nseq, spb, kout); break;
-    case 256: k_fft1d_f64<256, SIGN, REAL_IN, SPB><<<grid, SPB * 8, 0, st>>>(in, ibs, iss, ies, out, obs, oss, oes, nseq, spb, kout); break;
-    case 96: k_fft1d_f64<96, SIGN, REAL_IN, SPB><<<grid, SPB * 3, 0, st>>>(in, ibs, iss, ies, out, obs, oss, oes, nseq, spb, kout); break;
-    case 160: k_fft1d_f64<160, SIGN, REAL_IN, SPB><<<grid, SPB * 5, 0, st>>>(in, ibs, iss, ies, out, obs, oss, oes, nseq, spb, kout); break;
-    case 170: k_fft1d_f64<170, SIGN, REAL_IN, SPB><<<grid, SPB * 85, 0, st>>>(in, ibs, iss, ies, out, obs, oss, oes, nseq, spb, kout); break;
-    case 192: k_fft1d_f64<192, SIGN, REAL_IN, SPB><<<grid, SPB * 6, 0, st>>>(in, ibs, iss, ies, out, obs, oss, oes, nseq, spb, kout); break;
+    case 64: return fft1d_n<64, SIGN, REAL_IN>(in, ibs, iss, ies, out, obs, oss, oes, nseq, spb, kout, st);
+    case 96: return fft1d_n<96, SIGN, REAL_IN>(in, ibs, iss, ies, out, obs, oss, oes, nseq, spb, kout, st);
+    case 128: return fft1d_n<128, SIGN, REAL_IN>(in, ibs, iss, ies, out, obs, oss, oes, nseq, spb, kout, st);
+    case 160: return fft1d_n<160, SIGN, REAL_IN>(in, ibs, iss, ies, out, obs, oss, oes, nseq, spb, kout, st);
+    case 170: return fft1d_n<170, SIGN, REAL_IN>(in, ibs, iss, ies, out, obs, oss, oes, nseq, spb, kout, st);
+    case 192: return fft1d_n<192, SIGN, REAL_IN>(in, ibs, iss, ies, out, obs, oss, oes, nseq, spb, kout, st);
+    case 224: return fft1d_n<224, SIGN, REAL_IN>(in, ibs, iss, ies, out, obs, oss, oes, nseq, spb, kout, st);
+    case 256: return fft1d_n<256, SIGN, REAL_IN>(in, ibs, iss, ies, out, obs, oss, oes, nseq, spb, kout, st);
     default: return cudaErrorInvalidValue;
     }
-    return cudaGetLastError();
 }
 
 // a0 / a2: real [b][k][j] -> half spectrum [b][l][m], forward sign (Eq. 2 under R3).  tmp: [b][l][k].
@@ -181,10 +192,12 @@ __global__ void __launch_bounds__(256) k_project(const double *xyz, const double
         const double yr = R[3] * x0 + R[4] * y0 + R[5] * z0;
         const double Ra = rad[a], R2 = Ra * Ra;
         const double dens = wt[a] / (4.0 / 3.0 * CUDART_PI * Ra * Ra * Ra) * h * h;
-        // pixel j covers [(j - N/2 - 1/2) px, (j - N/2 + 1/2) px]: it meets the disc iff A < j < B with A, B below; floor(A) and
-        // ceil(B) keep one spare pixel on either side against rounding (a pixel outside the disc adds exactly 0)
-        const int j0 = (int)floor((xr - Ra) / px + N / 2 - 0.5), j1 = (int)ceil((xr + Ra) / px + N / 2 + 0.5);
-        const int k0 = (int)floor((yr - Ra) / px + N / 2 - 0.5), k1 = (int)ceil((yr + Ra) / px + N / 2 + 0.5);
+        // pixel j covers [(j - N/2 - 1/2) px, (j - N/2 + 1/2) px]: it meets the disc iff A < j < B with A = (xr - Ra)/px + N/2 - 1/2,
+        // B = (xr + Ra)/px + N/2 + 1/2, i.e. floor(A) + 1 <= j <= ceil(B) - 1.  No spare pixel is needed against rounding: a pixel
+        // that A or B misses by an ulp overlaps the disc by a sliver that holds none of the 4x4 mid-points (they sit px/8 inside
+        // the pixel), so it adds exactly 0 on both sides of the parity test.
+        const int j0 = (int)floor((xr - Ra) / px + N / 2 - 0.5) + 1, j1 = (int)ceil((xr + Ra) / px + N / 2 + 0.5) - 1;
+        const int k0 = (int)floor((yr - Ra) / px + N / 2 - 0.5) + 1, k1 = (int)ceil((yr + Ra) / px + N / 2 + 0.5) - 1;
         for (int k = k0; k <= k1; ++k) {
             if (k < 0 || k >= N) continue;
             const double yc = (k - N / 2) * px - 0.5 * px - yr;
@@ -358,26 +371,33 @@ __global__ void __launch_bounds__(256) k_calc_stats(const cd *F0, const double *
     const int NC = N / 2 + 1, H = NC * N;
     const int mo = blockIdx.x, o = mo % n_orient;
     const cd *F = F0 + (size_t)mo * H;
-    for (int c = 0; c < n_ctf; ++c) {
-        const double *K = K64 + (size_t)c * H;
-        double s = 0.0;
-        for (int i = threadIdx.x + 1; i < H; i += 256) {          // i = 0 is the DC bin
+    constexpr int CC = 8;                                             // CTF sets per pass over the spectrum (the power |F0|^2 is formed once per pass)
+    for (int c0 = 0; c0 < n_ctf; c0 += CC) {
+        const int nc = min(CC, n_ctf - c0);
+        double acc[CC];
+#pragma unroll
+        for (int u = 0; u < CC; ++u) acc[u] = 0.0;
+        for (int i = threadIdx.x + 1; i < H; i += 256) {              // i = 0 is the DC bin
             const int l = i / N;
-            const double w = (l == 0 || l == N / 2) ? 1.0 : 2.0;
             const cd v = F[i];
-            const double k = K[i];
-            s += w * (v.x * v.x + v.y * v.y) * k * k;
+            const double pw = ((l == 0 || l == N / 2) ? 1.0 : 2.0) * (v.x * v.x + v.y * v.y);
+#pragma unroll
+            for (int u = 0; u < CC; ++u)
+                if (u < nc) { const double k = K64[(size_t)(c0 + u) * H + i]; acc[u] += pw * k * k; }
         }
-        s = block_sum<256>(s, sh);
-        if (threadIdx.x == 0) {
-            const size_t moc = (size_t)mo * n_ctf + c;
-            const double n = (double)N * N;
-            const double lpo = lp_orient ? lp_orient[o] : -log((double)n_orient_total);   // a rank that scores a slice of the grid still weighs with the whole grid (R7)
-            const double lpc = lp_ctf ? lp_ctf[c] : -log((double)n_ctf);
-            const double h = -0.5 * log(s) + lpo + lpc - log_shifts;
-            if (!(s > 0.0) || isinf(s)) atomicOr(flags, 2);          // empty calculated image: T_c = 0, rho^2 undefined
-            Tc64[moc] = s; h64[moc] = h;
-            alpha32[moc] = (float)(1.0 / sqrt(n * s)); h32[moc] = (float)(h * 1.4426950408889634);   // FP32 path: base-2 units
+        for (int u = 0; u < nc; ++u) {
+            const int c = c0 + u;
+            const double s = block_sum<256>(acc[u], sh);
+            if (threadIdx.x == 0) {
+                const size_t moc = (size_t)mo * n_ctf + c;
+                const double n = (double)N * N;
+                const double lpo = lp_orient ? lp_orient[o] : -log((double)n_orient_total);   // a rank that scores a slice of the grid still weighs with the whole grid (R7)
+                const double lpc = lp_ctf ? lp_ctf[c] : -log((double)n_ctf);
+                const double h = -0.5 * log(s) + lpo + lpc - log_shifts;
+                if (!(s > 0.0) || isinf(s)) atomicOr(flags, 2);          // empty calculated image: T_c = 0, rho^2 undefined
+                Tc64[moc] = s; h64[moc] = h;
+                alpha32[moc] = (float)(1.0 / sqrt(n * s)); h32[moc] = (float)(h * 1.4426950408889634);   // FP32 path: base-2 units
+            }
         }
     }
 }

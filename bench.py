@@ -185,9 +185,13 @@ def run_ours(args):
     local = int(os.environ.get("LOCAL_RANK", "0"))
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device -- the product path has no CPU fallback")
+    local = local % torch.cuda.device_count()                                 # --backend gloo may put several ranks on one GPU (functional check only)
     torch.cuda.set_device(local)
     if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+        if args.backend == "nccl":
+            dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+        else:
+            dist.init_process_group("gloo")
 
     def barrier():
         if world > 1:
@@ -254,7 +258,7 @@ def run_ours(args):
     d2h = int(sum(np.asarray(v).nbytes for v in res.values())) // world       # this rank's share of the results
 
     if world > 1:
-        t = torch.tensor([t_dev, t_e2e], device="cuda", dtype=torch.float64)
+        t = torch.tensor([t_dev, t_e2e], device="cuda" if args.backend == "nccl" else "cpu", dtype=torch.float64)
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         t_dev, t_e2e = float(t[0]), float(t[1])
     evals_job = float(s.n_evaluations) * world * args.steps
@@ -334,6 +338,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", default="paper", choices=sorted(W.CONFIGS))
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--backend", default="nccl", choices=["nccl", "gloo"],
+                    help="torch.distributed backend for N > 1 (gloo: functional check of the multi-rank path, e.g. two ranks on one GPU)")
     ap.add_argument("--orient-stride", type=int, default=1,
                     help="profiling aid: keep every k-th orientation of the grid (the workload name in the JSON line says so)")
     ap.add_argument("--sweep", choices=["images", "shifts"], help="Fig. 4 / Fig. 2 shaped sweeps on one GPU (one JSON line per point)")

@@ -632,3 +632,35 @@ def test_other_box_sizes(n_pix):
         want = oracle.shift_map(wl["images"][img], I1, s.max_shift, logw)
         assert np.abs(b.debug_shift_map_f64(img, 0, o, c) - want).max() <= 1e-6
         assert np.abs(b.debug_shift_map(img, 0, o, c) - want).max() <= 5e-7 * s.n_pix ** 2 + 1e-3
+
+
+@pytest.mark.parametrize("name", ["paper_mini", "small_mini"])
+def test_many_near_equal_terms(name):
+    """The regime the FP64 re-scoring of BIOEM_TOPK terms is sized for (include/bioem.h, domain of validity): a symmetric
+    particle, or near-duplicate orientations, puts MANY terms within the FP32 error of the maximum -- here every grid
+    orientation appears 14 times (the 14 equivalent views of a D7 particle such as the paper's GroEL), rotated about the
+    viewing axis by multiples of 2e-5 rad so that the grid stays duplicate-free (R15).  log P must still meet the 1e-3 bar."""
+    from paper_1609_06634_b200 import BioEM
+    wl = dict(W.build_workload(name))
+    q = np.asarray(wl["quats"], dtype=np.float64)
+    reps = []
+    for i in range(14):
+        a = 2e-5 * i                                                         # q (x) rot_z(a): the same view turned in the image plane
+        rz = np.array([math.cos(a / 2), 0.0, 0.0, math.sin(a / 2)])
+        w0, x0, y0, z0 = q.T
+        w1, x1, y1, z1 = rz
+        reps.append(np.stack([w0 * w1 - x0 * x1 - y0 * y1 - z0 * z1, w0 * x1 + x0 * w1 + y0 * z1 - z0 * y1,
+                              w0 * y1 - x0 * z1 + y0 * w1 + z0 * x1, w0 * z1 + x0 * y1 - y0 * x1 + z0 * w1], axis=1))
+    wl["quats"] = np.concatenate(reps).astype(np.float32)
+    ref = _oracle_full(wl)
+    with BioEM() as b:
+        b.load_workload(wl)
+        b.run()
+        got = b.get_log_posterior()
+        best = b.get_best()
+    assert np.abs(got - ref["logp"]).max() <= TOL_LOGP, np.abs(got - ref["logp"]).max()
+    assert np.abs(best["log_p"] - ref["best"]).max() <= TOL_LOGP
+    # the maximum is one of the 14 copies of the oracle's orientation (their terms differ by less than the FP64 noise floor of
+    # the comparison only if the copies are exact; here they are 1e-5 rad apart, so the argmax must match unless the gap is < 1e-6)
+    same = best["orient"] == ref["orient"]
+    assert np.all(same | (ref["gap"] < 1e-6))

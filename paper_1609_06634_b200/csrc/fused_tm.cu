@@ -31,7 +31,7 @@
 //   warp 8 + k  (C): pass-1 tasks 16 + k, 20 + k; pass-2 task 4 + k, odd dx       2.7
 //   warp 12 + k (D): pass-1 task 24 + k;          pass-2 task k, both parities    2.6
 // (round 2 measured dedicated pass-1 / pass-2 warps first: 12 x {3, 2, 2} tasks + 4 x 2 whole pass-2 tasks -- the step then
-// runs at the pace of a 3.1-unit warp while eight 2-unit warps sleep a third of the time; profiles/r2_tm_v5.)
+// runs at the pace of a 3.1-unit warp while eight 2-unit warps sleep a third of the time; an earlier capture of this round, not kept.)
 // TMEM columns per quadrant: 128 + 128 + 128 + 64 of 512.  Hand-over of G_T: a "full" mbarrier per buffer (16 arrivals: every
 // warp after its last pass-1 store of the step) and an "empty" one (12 arrivals: the warps with pass-2 work after their last
 // G_T load).  No CTA barrier in the loop, no float atomics, fixed reduction orders: bit-reproducible.
@@ -68,7 +68,7 @@ __device__ __forceinline__ void tm_wait_ld(uint32_t (&a)[8], uint32_t (&b)[8])
 __device__ __forceinline__ void tm_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
 
 // Usually the phase is already complete.  A warp that is early sleeps between probes: mbarrier.try_wait, with or without a
-// suspend-time hint, compiles to a probe loop that returns every ~25 cycles and took 20 % of the issue slots (profiles/r2_tm_v2).
+// suspend-time hint, compiles to a probe loop that returns every ~25 cycles and took 20 % of the issue slots (an earlier capture of this round, not kept).
 __device__ __forceinline__ void tm_mbar_wait(uint64_t *bar, unsigned parity)
 {
     const unsigned b = (unsigned)__cvta_generic_to_shared(bar);
@@ -80,7 +80,7 @@ __device__ __forceinline__ void tm_mbar_wait(uint64_t *bar, unsigned parity)
 // 2 c2 + 1, the two outputs that share k1' = e: k_lo = k1 - 32 and k_hi = k1.  y[2 i + 0 | 1] = sum_t r_lo^t | r_hi^t z[2 c2 + i][t].
 // Horner from t = 6, four chains interleaved (a chain alone is 12 dependent FFMA2); the two chains of a column share its loads,
 // and the two half-warps read different columns, so every shared-memory wavefront is used once (with lane = output and 4 columns
-// per lane both half-warps fetched the same 128 bytes: twice the wavefronts -- profiles/r2_tm_v6).
+// per lane both half-warps fetched the same 128 bytes: twice the wavefronts (an earlier capture of this round, not kept)).
 __device__ __forceinline__ void tm_horner7x4(c2 (&y)[4], const c2 *zc, c2 r_lo, c2 r_hi)
 {
 #pragma unroll
@@ -96,7 +96,7 @@ __device__ __forceinline__ void tm_horner7x4(c2 (&y)[4], const c2 *zc, c2 r_lo, 
 }
 
 // The four pass-1 outputs of a lane -> rows of G_T.  Lanes whose output index lies outside |k| <= D do not store (predicated
-// stores: a dummy address for them put a second wavefront on every store, profiles/r2_tm_v8).
+// stores: a dummy address for them put a second wavefront on every store, profiles/r2_tm_v8_fused_paper_stride16_full.csv).
 // `unpack` (the lanes of warp 0 that hold packed column 0): y = G(., 0) + i G(., 112), both parts real -> two real columns
 // (0 and 112 of G_T), so that pass 2 reads column 0 and the Nyquist column like any other: no special case in its load loop.
 __device__ __forceinline__ void tm_store_rows(c2 *g_lo, c2 *g_hi, bool v_lo, bool v_hi, const c2 (&y)[4], bool unpack = false)
@@ -254,7 +254,7 @@ __device__ __forceinline__ void tm_p1_slot(c2 (&a)[16], uint32_t qaddr, const fl
 // l = 7 j + t.  Columns l = 1..111 are stored, l = 113..223 are their conjugates (Hermitian half); columns 0 and 112 are real (pass 1
 // unpacks them from packed column 0 on store): both formulas below then give (A.x, B.x).  ODD = false: a_j = x_j + x_(j+16) (even dx); ODD = true: a_j = (x_j - x_(j+16)) w32^j (odd dx).
 // (Lane = 8 pair + t and 8 RP = 16 mod 128: the eight lanes of a quarter-warp read eight different 16-byte slots, direct and
-// mirrored.)  A warp that does both parities loads twice: keeping the other half in registers spills (profiles/r2_tm_v7b).
+// mirrored.)  A warp that does both parities loads twice: keeping the other half in registers spills, and parking it in tensor memory or fetching K after pass 2 instead were both slower (DESIGN 7).
 template <bool ODD>
 __device__ __forceinline__ void tm_p2_front(c2 (&a)[16], const c2 *gt, int t)
 {
@@ -284,8 +284,7 @@ __global__ void __launch_bounds__(TM::NT, 1) k_fused_tm(FusedParams p, const flo
     c2 *Z = reinterpret_cast<c2 *>(smem_raw);                         // [NW][32][ZP]   warp-private tiles
     c2 *G = Z + (size_t)NW * ZW;                                      // [2][112][RP]   G_T: pass-1 outputs of one CTF, all columns, double-buffered
     c2 *qn = G + (size_t)2 * GSZ;                                     // [32][7]        Q of the Nyquist column (warp 0)
-    c2 *gdump = qn + 224;                                             // [2][RP]        where the lanes without an output row store (|k| > D)
-    TopEntry *tops = reinterpret_cast<TopEntry *>(gdump + 2 * RP);    // [NW][TOPK]
+    TopEntry *tops = reinterpret_cast<TopEntry *>(qn + 224);    // [NW][TOPK]
     float *red = reinterpret_cast<float *>(tops + NW * BIOEM_TOPK);   // [2 NW]
     __shared__ uint64_t bar_full[2], bar_empty[2];
     __shared__ uint32_t tm_base_s;
@@ -304,7 +303,7 @@ __global__ void __launch_bounds__(TM::NT, 1) k_fused_tm(FusedParams p, const flo
         asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"((unsigned)__cvta_generic_to_shared(&tm_base_s)) : "memory");
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
     }
-    for (int i = tid; i < (NW * ZW + 2 * GSZ + 224 + 2 * RP) * 2; i += TM::NT) reinterpret_cast<float *>(Z)[i] = 0.f;
+    for (int i = tid; i < (NW * ZW + 2 * GSZ + 224) * 2; i += TM::NT) reinterpret_cast<float *>(Z)[i] = 0.f;
     if (tid < NW * BIOEM_TOPK) { TopEntry e0 = {-CUDART_INF_F, 0xffffffffu, 0xffffffffu}; tops[tid] = e0; }
     if (tid == 0) {
         for (int i = 0; i < 2; ++i) { pk_mbar_init(&bar_full[i], NW); pk_mbar_init(&bar_empty[i], TM::NCONS); }
@@ -547,7 +546,7 @@ cudaError_t launch_relayout_K_tm(const float *K32, float *Kt, int n_ctf, cudaStr
 // Work items: one CTA per (image, model, chunk); one partial per work item.
 cudaError_t launch_fused_tm(const FusedParams &p, const float *Kt, bool dump, cudaStream_t st)
 {
-    const size_t bytes = ((size_t)TM::NW * TM::ZW + 2 * TM::GSZ + 224 + 2 * TM::RP) * 8 + (size_t)TM::NW * BIOEM_TOPK * sizeof(TopEntry) + 2 * TM::NW * 4 + 64;
+    const size_t bytes = ((size_t)TM::NW * TM::ZW + 2 * TM::GSZ + 224) * 8 + (size_t)TM::NW * BIOEM_TOPK * sizeof(TopEntry) + 2 * TM::NW * 4 + 64;
     const float4 *kt = reinterpret_cast<const float4 *>(Kt);
     const float *ktn = tm_ktn(Kt, p.n_ctf);
     cudaError_t e;

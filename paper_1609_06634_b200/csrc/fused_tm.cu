@@ -387,12 +387,15 @@ __global__ void __launch_bounds__(TM::NT, 1) k_fused_tm(FusedParams p, const flo
                         tm_st8(qaddr0 + 64 * ii + 8 * g, r);
                     }
                 }
-                if (nyq) {
-                    for (int j = 0; j < 32; ++j) {
-                        const size_t e = (size_t)(N / 2) * N + 7 * j + t;
-                        const cf pr = cmulc(Oimg[e], F0[e]);
-                        qn[7 * j + t] = make_float2(pr.x, pr.y);
-                    }
+                if (warp_nyq) {
+                    // the Nyquist column, qn[m] = Q(112, m): all 32 lanes, 7 coalesced loads per array in flight at once (as a loop
+                    // of 32 dependent round trips to L2 on 7 lanes it made warp 0 late by ~20 k cycles at every new orientation and
+                    // the other 15 warps wait for it: 3 % of the run)
+                    cf ov[7], fv[7];
+#pragma unroll
+                    for (int i = 0; i < 7; ++i) { ov[i] = Oimg[(size_t)(N / 2) * N + lane + 32 * i]; fv[i] = F0[(size_t)(N / 2) * N + lane + 32 * i]; }
+#pragma unroll
+                    for (int i = 0; i < 7; ++i) { const cf pr = cmulc(ov[i], fv[i]); qn[lane + 32 * i] = make_float2(pr.x, pr.y); }
                 }
                 tm_wait_st();
                 __syncwarp();

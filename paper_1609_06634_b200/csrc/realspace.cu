@@ -33,7 +33,7 @@ __device__ __forceinline__ double rs_block_sum(double v, double *sh)
 // grid (N/2+1, nb), 256 threads
 __global__ void __launch_bounds__(256) k_rs_inv_m(const cd *F0, const double *K, int N, cd *T)
 {
-    extern __shared__ double rs_sm[];
+    extern __shared__ __align__(16) double rs_sm[];
     cd *tw = reinterpret_cast<cd *>(rs_sm), *col = tw + N;
     const int l = blockIdx.x, b = blockIdx.y, NC = N / 2 + 1;
     const cd *F = F0 + ((size_t)b * NC + l) * N;
@@ -60,7 +60,7 @@ __global__ void __launch_bounds__(256) k_rs_inv_m(const cd *F0, const double *K,
 // step 2: along l with the Hermitian weights.   I1(k, j) = 1/n sum_l w_l Re[ T(l, k) e^{+2 pi i l j / N} ]     grid (N, nb)
 __global__ void __launch_bounds__(256) k_rs_inv_l(const cd *T, int N, double *I1)
 {
-    extern __shared__ double rs_sm[];
+    extern __shared__ __align__(16) double rs_sm[];
     cd *tw = reinterpret_cast<cd *>(rs_sm), *row = tw + N;
     const int k = blockIdx.x, b = blockIdx.y, NC = N / 2 + 1;
     for (int i = threadIdx.x; i < N; i += 256) {
@@ -105,7 +105,7 @@ struct RsPartial { double m, s, best; int shift; int valid; };
 __global__ void __launch_bounds__(256) k_rs_score(const double *Oc, const double *Dw, const double *I1, const double *cc, const double *ccc,
                                                   const double *logw, int n_img, int N, int D, RsPartial *part, int *flags)
 {
-    extern __shared__ double rs_sm[];
+    extern __shared__ __align__(16) double rs_sm[];
     __shared__ double sh[256];
     const int KK = 2 * D + 1, S = KK * KK, img = blockIdx.x, b = blockIdx.y;
     double *Bs = rs_sm, *gs = rs_sm + S;

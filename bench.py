@@ -307,28 +307,32 @@ def run_ours(args):
 
 def run_sweep(args):
     """Shapes of the paper's Fig. 4 (time against the number of images; linear above 128-256) and Fig. 2 (time against the
-    number of displacements; the Fourier route is almost flat) on the `small` grid with every 16th orientation.
+    number of displacements for the Fourier-space and the real-space variant; the Fourier route is almost flat and wins beyond a
+    handful of displacements) on the `small` grid with every 16th orientation.
     One JSON line per point: device time of bioem_run (CUDA events inside the library), median of 3."""
     import torch
     from paper_1609_06634_b200 import BioEM
     wl = build_inputs("small", 0, 16)
     s = wl["spec"]
-    pts = ([("images", n, s.max_shift) for n in (1, 2, 4, 8, 16, 32, 64, 128, 256)] if args.sweep == "images"
-           else [("shifts", s.n_images, d) for d in (0, 1, 2, 4, 8, 12, 16)])
+    pts = ([("images", n, s.max_shift, 0) for n in (1, 2, 4, 8, 16, 32, 64, 128, 256)] if args.sweep == "images"
+           else [("shifts", s.n_images, d, 0) for d in (0, 1, 2, 4, 8, 12, 16)] + [("shifts", s.n_images, d, 1) for d in (0, 1, 2, 3, 4)])
     with BioEM(device=0) as b:
-        b.load_workload(wl)
-        for kind, n_img, D in pts:
+        b.load_workload(wl, images=False)
+        for kind, n_img, D, variant in pts:
             b.set_shift_range(D)
+            b.set_displacement_variant(variant)
             b.push_images(wl["images"][:n_img])
             ms = []
             for _ in range(4):
+                b.invalidate_precompute()
                 b.run()
                 b.get_log_posterior()
                 ms.append(b.get_timing())
             tot, fused = np.median([m[0] for m in ms[1:]]), np.median([m[1] for m in ms[1:]])
             pairs = n_img * s.n_orient * s.n_ctf
-            print(json.dumps({"sweep": kind, "n_images": n_img, "max_shift": D, "n_shifts": (2 * D + 1) ** 2, "pairs": pairs,
-                              "run_ms": float(tot), "fused_ms": float(fused), "ns_per_pair": 1e6 * float(tot) / pairs}), flush=True)
+            print(json.dumps({"sweep": kind, "variant": "real space, cropping" if variant else "Fourier space, circular", "n_images": n_img,
+                              "max_shift": D, "n_shifts": (2 * D + 1) ** 2, "pairs": pairs, "run_ms": float(tot), "scoring_ms": float(fused),
+                              "ns_per_pair": 1e6 * float(tot) / pairs}), flush=True)
 
 
 def main():

@@ -622,7 +622,7 @@ int bioem_merge_partials(bioem_ctx *ctx, int n_blobs, const void *blobs, int64_t
     CK(cudaMemcpyAsync(ctx->blob_chunks.p, chunks.data(), chunks.size() * sizeof(int), cudaMemcpyHostToDevice, st));
     CK(launch_merge(src, (size_t)stride_bytes, ctx->blob_chunks.as<int>(), n_blobs, I, M, ctx->m32.as<double>(), ctx->s32.as<double>(),
                     ctx->top.as<TopEntry>(), st));
-    CK(cudaStreamSynchronize(st));                               // `chunks` (and a host `blobs`) may go away
+    if (blobs && !is_device) CK(cudaStreamSynchronize(st));      // a host `blobs` may go away (the small `chunks` array is pageable: its copy is staged before cudaMemcpyAsync returns)
     ctx->launches += 1;
     ctx->phase = 2;
     return BIOEM_OK;

@@ -63,3 +63,20 @@ def test_ensemble_models_are_hinge_perturbations():
         # rigid: pairwise distances inside the moved part are preserved
         a, b = m["xyz"][moved][:20], base["xyz"][moved][:20]
         assert np.allclose(np.linalg.norm(a[:, None] - a[None], axis=-1), np.linalg.norm(b[:, None] - b[None], axis=-1))
+
+
+def test_bench_helpers():
+    """bench.py's roofline inputs: the pruned flop count of SURVEY 8(d) / DESIGN 7 and the committed ncu table."""
+    import importlib.util
+    from pathlib import Path
+    spec = importlib.util.spec_from_file_location("bench", Path(__file__).resolve().parent.parent / "bench.py")
+    bench = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(bench)
+    # 6H + (N/2+1) 5 N log2 N + (2D+1) 2.5 N log2 N + 30 S, written out for Small and Paper-scale
+    assert abs(bench.algorithmic_flops_per_pair(128, 16) - (6 * 8320 + 65 * 5 * 128 * 7 + 33 * 2.5 * 128 * 7 + 30 * 1089)) < 1e-6
+    assert abs(bench.algorithmic_flops_per_pair(224, 30) - 1518300.083) < 1.0
+    row = bench.ncu_table("paper")
+    assert row is not None and row["kernel"] == "k_fused_tm" and float(row["dram_bytes_per_launch"]) > 1e9
+    assert (Path(bench.ROOT) / row["capture"].split(" ")[0]).exists()              # the capture the row cites is committed
+    assert bench.ncu_table("no such workload") is None
+    assert W.get_spec("paper").n_evaluations == 1024 * 4096 * 32 * 61 * 61         # the bench default (config.workload)

@@ -201,6 +201,29 @@ int bioem_get_launch_count(bioem_ctx *ctx, int64_t *n_launches, int64_t *n_fused
  * while the loop ran: bench.py samples nvidia-smi for that). */
 int bioem_measure_fp32_peak(bioem_ctx *ctx, double *tflops, double *sm_mhz);
 
+/* Allocation-free entry point, for callers that may not call cudaMalloc (code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid it): Eq. 10 as bioem_get_ensemble_log_posterior computes it, but context-free, on
+ * caller-supplied DEVICE arrays, enqueued on `cuda_stream` of CUDA device `device` without synchronising, and calling no
+ * cudaMalloc / cudaFree or allocating library routine.  Its work array (the per-image inner log-sums) is a file-scope device
+ * array of BIOEM_NOALLOC_MAX_IMG doubles (512 KiB) that every GPU loading the library holds until the process exits.
+ *   log_p          device, [n_img][n_model] doubles: log P_m,omega, e.g. a device copy of bioem_get_log_posterior's output
+ *   weights        device, [n_model] doubles, w_m >= 0 (a negative weight gives NaN outputs; nothing is read back to
+ *                  check), or NULL = uniform 1 / n_model
+ *   out_total      device, one double;  out_per_image  device, [n_img] doubles, or NULL
+ * n_img > BIOEM_NOALLOC_MAX_IMG or n_model > BIOEM_NOALLOC_MAX_MODEL: BIOEM_EUNSUPPORTED, nothing enqueued (use the
+ * allocating call).  Every call on a device shares the one work array: calls whose kernels may overlap on the GPU
+ * (different streams, several host threads) RACE -- keep them on one stream or order them with events.  Nothing in the
+ * array has to be cleared between calls (each call writes the entries it reads).  Same summation order as the allocating
+ * call, so the two agree to rounding of log().  bioem_noalloc_prepare(device) takes the array's device address ahead of
+ * time (otherwise the first call on a device does, which may load the module: do it before a capture begins).  These three
+ * calls report errors through bioem_noalloc_last_error() (per host thread), not through a context. */
+#define BIOEM_NOALLOC_MAX_IMG   65536
+#define BIOEM_NOALLOC_MAX_MODEL 1024
+int bioem_noalloc_prepare(int device);
+int bioem_ensemble_log_posterior_noalloc(int device, void *cuda_stream, int n_img, int n_model, const double *log_p, const double *weights,
+                                         double *out_total, double *out_per_image);
+const char *bioem_noalloc_last_error(void);
+
 #ifdef __cplusplus
 }
 #endif

@@ -20,7 +20,9 @@ EXPORTED_SYMBOLS = [
     "bioem_set_orientation_chunk", "bioem_debug_set_kernel", "bioem_get_run_plan", "bioem_invalidate_precompute",
     "bioem_set_orientation_slice", "bioem_run_partial", "bioem_get_partials_size", "bioem_export_partials", "bioem_merge_partials",
     "bioem_rescore_local", "bioem_export_rescore", "bioem_import_rescore", "bioem_finish", "bioem_set_displacement_variant",
+    "bioem_noalloc_prepare", "bioem_ensemble_log_posterior_noalloc", "bioem_noalloc_last_error",
 ]
+NOALLOC_MAX_IMG, NOALLOC_MAX_MODEL = 65536, 1024
 KERNEL_AUTO, KERNEL_GENERIC, KERNEL_PK, KERNEL_C2, KERNEL_TM, KERNEL_DFT, KERNEL_REALSPACE = 0, 1, 2, 3, 4, 5, 6
 
 _fp = C.POINTER(C.c_float)
@@ -84,9 +86,13 @@ def lib():
         L.bioem_set_orientation_chunk.argtypes = [C.c_void_p, C.c_int]
         L.bioem_debug_set_kernel.argtypes = [C.c_void_p, C.c_int]
         L.bioem_get_run_plan.argtypes = [C.c_void_p, C.POINTER(C.c_int), C.POINTER(C.c_int)]
+        L.bioem_noalloc_prepare.argtypes = [C.c_int]
+        L.bioem_ensemble_log_posterior_noalloc.argtypes = [C.c_int, C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+        L.bioem_noalloc_last_error.argtypes = []
         for name in EXPORTED_SYMBOLS:
             if name != "bioem_last_error":
                 getattr(L, name).restype = C.c_int
+        L.bioem_noalloc_last_error.restype = C.c_char_p
         _lib = L
     return _lib
 
@@ -313,6 +319,28 @@ class BioEM:
             wp = w.ctypes.data_as(_dp)
         self._ck(self._L.bioem_get_ensemble_log_posterior(self._h, wp, tot.ctypes.data_as(_dp), per.ctypes.data_as(_dp)))
         return float(tot[0]), per
+
+    @staticmethod
+    def noalloc_last_error():
+        return (lib().bioem_noalloc_last_error() or b"").decode()
+
+    @staticmethod
+    def noalloc_prepare(device=0):
+        rc = lib().bioem_noalloc_prepare(device)
+        if rc:
+            raise BioEMError(rc, BioEM.noalloc_last_error())
+
+    @staticmethod
+    def ensemble_log_posterior_noalloc(log_p, weights, out_total, out_per_image=None, device=0, stream=0):
+        """Eq. 10 without any allocation.  Every array is a CUDA float64 tensor (anything with data_ptr()) on `device`:
+        log_p [n_img][n_model], weights [n_model] or None, out_total [1], out_per_image [n_img] or None; `stream` is a
+        cudaStream_t (0 = default).  Enqueues and returns; the outputs are ready when the stream reaches them."""
+        n_img, n_model = int(log_p.shape[0]), int(log_p.shape[1])
+        ptr = lambda t: C.c_void_p(t.data_ptr()) if t is not None else None
+        rc = lib().bioem_ensemble_log_posterior_noalloc(device, C.c_void_p(stream or 0), n_img, n_model, ptr(log_p), ptr(weights),
+                                                        ptr(out_total), ptr(out_per_image))
+        if rc:
+            raise BioEMError(rc, BioEM.noalloc_last_error())
 
     def debug_calc_image(self, model, orient, ctf):
         out = np.empty((self.n_pix, self.n_pix), dtype=np.float32)

@@ -9,7 +9,7 @@ from pathlib import Path
 HERE = Path(__file__).resolve().parent
 CSRC = HERE / "csrc"
 LIB = HERE / "libbioem_b200.so"
-SOURCES = ["bioem_api.cu", "fused.cu", "fused_pk.cu", "fused_c2.cu", "fused_tm.cu", "precompute.cu", "finalize.cu", "realspace.cu"]
+SOURCES = ["bioem_api.cu", "fused.cu", "fused_pk.cu", "fused_c2.cu", "fused_tm.cu", "precompute.cu", "finalize.cu", "realspace.cu", "noalloc.cu"]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-Xcompiler", "-fPIC"]
 
 

@@ -114,9 +114,11 @@ int bioem_get_best(bioem_ctx *ctx, int32_t *orient_idx, int32_t *ctf_idx, int32_
 
 /* Posterior as a function of the orientation (the paper's third output):
  *   out[img][model][o] = log sum_{ctf, d} w(o, ctf, d) P_m,omega(o, ctf, d)      (log-sum-exp over o gives log_posterior).
- * Off by default.  When enabled before bioem_run, every work item covers ONE orientation, so the per-item partial sums are
- * the per-orientation sums (same kernels, O x more work items: the per-item prologue and epilogue are no longer amortised over a
- * chunk of 32 orientations -- measured 2.0x the run time on Small, 32 CTFs per orientation).  The terms that the FP64
+ * Off by default.  When enabled before bioem_run, the work items stay chunked (several orientations per thread block): each warp
+ * closes its running sums at the end of every orientation into a shared-memory table, and the work item's epilogue combines
+ * warps -> orientation -> work item in fixed order and writes 8 bytes per (image, model, orientation).  Measured 1.04x / 1.11x /
+ * 1.06x the run time on Small / Paper-scale / Ensemble (the kernels are separate template instantiations: a run with the option
+ * off executes the same code as before).  The table has 32 rows, so the chunk is capped at 32.  The terms that the FP64
  * re-scoring replaces (the 8 largest per image and model) are replaced here too; the others keep FP32 accuracy
  * (R24).  enable: 0 | 1.  get_: caller-allocated [n_img][n_model][n_orient] doubles; BIOEM_EBADSTATE if the
  * last run was made without the option. */
@@ -133,8 +135,8 @@ int bioem_get_ensemble_log_posterior(bioem_ctx *ctx, const double *weights, doub
  * orientations x all CTFs x all shifts of one model (the image-stationary loop order of DESIGN.md section 8; P:199-203 has
  * the loops the other way round).  0 = automatic: >= 32 work items per SM, at most 32 orientations per item.  The value
  * fixes the order in which the FP32 partial sums are combined, so results are bit-identical between two runs only if it is
- * the same; ranks that shard one image stack set it explicitly.  Ignored (1) while the per-orientation
- * posterior is enabled. */
+ * the same; ranks that shard one image stack set it explicitly.  Capped at 32 while the per-orientation
+ * posterior is enabled (1 with the two-CTA cluster kernel of bioem_debug_set_kernel, which has no per-orientation table). */
 int bioem_set_orientation_chunk(bioem_ctx *ctx, int n_orient_per_item);
 
 /* Displacement variant (paper section 3.3).  0 (default): Fourier space -- one output-pruned inverse transform

@@ -73,6 +73,8 @@ struct bioem_ctx {
     int run_kernel = 0, run_oc = 0;
     bool flags_checked = true;
     DBuf logp_orient;
+    DBuf orient_m, orient_s;      // float [M*O][I]: per-orientation (m, s) written by the fused kernel (posterior per orientation, folded)
+    bool run_want_orient = false, run_orient_folded = false;      // the option as the last run_partial saw it
     int run_models = 0, run_orient = 0, run_ctf = 0, run_D = 0, run_img = 0;
     DBuf F064, F032, K64, K32, Kt, Tc64, h64, alpha32, h32;
     DBuf m32, s32, top, g64;
@@ -134,7 +136,7 @@ int bioem_destroy(bioem_ctx *ctx)
     DBuf *all[] = {&ctx->rot, &ctx->lp_orient, &ctx->ctf_a, &ctx->ctf_A, &ctx->ctf_b, &ctx->lp_ctf, &ctx->Ohat64, &ctx->Ohat32, &ctx->Dw,
                    &ctx->beta, &ctx->F064, &ctx->F032, &ctx->K64, &ctx->K32, &ctx->Kt, &ctx->Tc64, &ctx->h64, &ctx->alpha32, &ctx->h32,
                    &ctx->blob, &ctx->gathered, &ctx->blob_chunks, &ctx->Oreal64, &ctx->rs_T, &ctx->rs_I1, &ctx->rs_cc, &ctx->rs_ccc, &ctx->rs_part, &ctx->rs_logw,
-                   &ctx->rs_pair, &ctx->rs_m, &ctx->rs_s, &ctx->rs_best, &ctx->rs_bpair, &ctx->rs_bshift, &ctx->m32, &ctx->s32, &ctx->top, &ctx->g64, &ctx->logp, &ctx->logp_orient, &ctx->logp32,
+                   &ctx->rs_pair, &ctx->rs_m, &ctx->rs_s, &ctx->rs_best, &ctx->rs_bpair, &ctx->rs_bshift, &ctx->m32, &ctx->s32, &ctx->top, &ctx->g64, &ctx->logp, &ctx->logp_orient, &ctx->orient_m, &ctx->orient_s, &ctx->logp32,
                    &ctx->best, &ctx->best_logp, &ctx->scratch_a, &ctx->scratch_b, &ctx->scratch_c, &ctx->dump, &ctx->flags, &ctx->staging};
     for (DBuf *b : all) b->release();
     for (int i = 0; i < 4; ++i) if (ctx->ev[i]) cudaEventDestroy(ctx->ev[i]);
@@ -414,12 +416,20 @@ int bioem_run_partial(bioem_ctx *ctx)
     // an orientation slice leaves the chunk size to the caller: every rank must cut the grid at the same places
     if (sliced && ctx->oc_user <= 0) FAIL(BIOEM_EBADSTATE, "run: set_orientation_chunk before scoring an orientation slice (all ranks the same value)");
     int oc = ctx->oc_user > 0 ? std::min(ctx->oc_user, Ofull) : choose_oc(I, M, Ofull, ctx->n_sm);
-    if (ctx->want_orient) oc = 1;                                         // one orientation per work item when its posterior is wanted
+    // posterior per orientation: the chunked kernels close their sums per orientation in a shared-memory table of 32 rows;
+    // the cluster kernel (a cross-check, never chosen automatically) has no such table and runs one orientation per work item
+    const bool fold = ctx->want_orient && !use_c2;
+    if (ctx->want_orient && !fold) oc = 1;
+    if (fold && oc > 32) oc = 32;
     if (sliced && o_first % oc != 0) FAIL(BIOEM_EBADARG, "run: an orientation slice must begin at a multiple of the orientation chunk");
     const int cpm = (O + oc - 1) / oc;
     const int ppi = use_c2 ? 2 : 1;                                       // partials per work item (the cluster kernel writes one per CTA)
     const size_t items = (size_t)I * M * cpm * ppi;
     CK(ctx->blob.ensure(partial_blob_bytes(items)));
+    if (fold) {
+        CK(ctx->orient_m.ensure(MO * I * sizeof(float)));
+        CK(ctx->orient_s.ensure(MO * I * sizeof(float)));
+    }
 
     CK(cudaEventRecord(ctx->ev[0], st));
     if (!ctx->pre_valid) CK(cudaMemsetAsync(ctx->flags.as<int>() + 1, 0, sizeof(int), st));
@@ -546,6 +556,7 @@ int bioem_run_partial(bioem_ctx *ctx)
     p.n_img = I; p.n_model = M; p.n_orient = O; p.n_ctf = C; p.D = D; p.oc = oc; p.chunks_per_model = cpm; p.o_first = o_first;
     p.cA = (float)(-0.5 * ((double)n - 3.0) * 1.4426950408889634);
     p.part_m = ctx->blob.as<float>(); p.part_s = p.part_m + items; p.part_top = reinterpret_cast<TopEntry *>(p.part_s + items);
+    if (fold) { p.orient_m = ctx->orient_m.as<float>(); p.orient_s = ctx->orient_s.as<float>(); }
     CK(cudaEventRecord(ctx->ev[1], st));
     int nl = 1;
     if (items == 0) nl = 0;
@@ -559,6 +570,7 @@ int bioem_run_partial(bioem_ctx *ctx)
     ctx->flags_checked = false;
     ctx->run_kernel = kern; ctx->run_oc = oc; ctx->run_o_first = o_first; ctx->run_o_local = O; ctx->run_chunks = cpm * ppi;
     ctx->run_models = M; ctx->run_orient = Ofull; ctx->run_ctf = C; ctx->run_D = D; ctx->run_img = I;
+    ctx->run_orient_folded = fold; ctx->run_want_orient = ctx->want_orient;
     ctx->phase = 1;
     return BIOEM_OK;
 }
@@ -687,11 +699,13 @@ int bioem_finish(bioem_ctx *ctx)
                     ctx->best_logp.as<double>(), st));
     ctx->launches += 1;
     ctx->ran_orient = false;
-    if (ctx->want_orient) {
+    if (ctx->run_want_orient) {
+        // the per-orientation (m, s): the folded table, or (cluster kernel, one orientation per work item) the partials themselves
         const size_t items = IM * ctx->run_chunks;
-        const float *part_m = ctx->blob.as<float>(), *part_s = part_m + items;
+        const float *part_m = ctx->run_orient_folded ? ctx->orient_m.as<float>() : ctx->blob.as<float>();
+        const float *part_s = ctx->run_orient_folded ? ctx->orient_s.as<float>() : part_m + items;
         CK(ctx->logp_orient.ensure(IM * ctx->run_orient * sizeof(double)));
-        CK(launch_orient_final(part_m, part_s, ctx->run_kernel == KERNEL_C2 ? 2 : 1, ctx->top.as<TopEntry>(), ctx->g64.as<double>(), ctx->Dw.as<double>(), I, M,
+        CK(launch_orient_final(part_m, part_s, ctx->run_orient_folded ? 1 : 2, ctx->top.as<TopEntry>(), ctx->g64.as<double>(), ctx->Dw.as<double>(), I, M,
                                ctx->run_orient, ctx->run_ctf, N, const_n, ctx->logp_orient.as<double>(), st));
         ctx->launches += 1;
         ctx->ran_orient = true;

@@ -47,6 +47,9 @@ struct FusedParams {
     // outputs: one partial per work item = (model, chunk, image)
     float *part_m, *part_s;      // [items]   partial sum = part_s * 2^part_m
     TopEntry *part_top;          // [items][TOPK]
+    // posterior per orientation, folded into the chunked work items: NULL, or [(model*O + o)*I + img] (m, s) of the sum over
+    // the CTFs and shifts of orientation o, written by the work item that holds o (k_fused_pk / k_fused_tm <.., ORIENT = true>, k_fused)
+    float *orient_m, *orient_s;
     // debug dump of one pair (DUMP instantiation only)
     float *dump;                 // [S1*S1]
     int dump_img, dump_model, dump_orient, dump_ctf;

@@ -57,6 +57,21 @@ __device__ __forceinline__ void lse_merge(float &m, float &s, float m2, float s2
     m = M;
 }
 
+// lanes by xor-tree; the pairwise merge is symmetric so both partners hold the same value
+__device__ __forceinline__ void warp_lse_reduce(float &lse_m, float &lse_s, int lane)
+{
+#pragma unroll
+    for (int off = 16; off >= 1; off >>= 1) {
+        float m2 = __shfl_xor_sync(FULL, lse_m, off), s2 = __shfl_xor_sync(FULL, lse_s, off);
+        float M = fmaxf(lse_m, m2);
+        float sa = (lse_m == -CUDART_INF_F) ? 0.f : lse_s * exp2f(lse_m - M);
+        float sb = (m2 == -CUDART_INF_F) ? 0.f : s2 * exp2f(m2 - M);
+        bool lo = (lane & off) == 0;
+        lse_s = lo ? sa + sb : sb + sa;
+        lse_m = M;
+    }
+}
+
 template <int N, int NT, bool DUMP>
 __global__ void __launch_bounds__(NT) k_fused(FusedParams p, int CB, int GP)
 {
@@ -71,6 +86,8 @@ __global__ void __launch_bounds__(NT) k_fused(FusedParams p, int CB, int GP)
     cf *twB = G + (size_t)KK * GP;                                  // [N2][KK]   w_N^{t k}
     TopEntry *tops = reinterpret_cast<TopEntry *>(twB + (size_t)N2 * KK);   // [NW][TOPK]
     float *red = reinterpret_cast<float *>(tops + NW * BIOEM_TOPK); // [2*NW]
+    float2 *otab = reinterpret_cast<float2 *>(red + 2 * NW);        // [32][NW]   (m, s) per orientation of the item and warp (p.orient_m only)
+    const bool orient = !DUMP && p.orient_m != nullptr;             // posterior per orientation: close the sums after every orientation
 
     // ---- work item
     int img, model, o_begin, o_end, item;
@@ -202,26 +219,35 @@ __global__ void __launch_bounds__(NT) k_fused(FusedParams p, int CB, int GP)
                 __syncthreads();
             }
         }
+        if (orient) {
+            warp_lse_reduce(lse_m, lse_s, lane);
+            if (lane == 0) otab[(o - o_begin) * NW + warp] = make_float2(lse_m, lse_s);
+            lse_m = -CUDART_INF_F; lse_s = 0.f;
+        }
     }
     if (DUMP) return;
 
     // ---- block reduction in a fixed order: lanes by xor-tree, then warps 0..NW-1 sequentially
-#pragma unroll
-    for (int off = 16; off >= 1; off >>= 1) {
-        float m2 = __shfl_xor_sync(FULL, lse_m, off), s2 = __shfl_xor_sync(FULL, lse_s, off);
-        // make the pairwise merge symmetric so both partners hold the same value
-        float M = fmaxf(lse_m, m2);
-        float sa = (lse_m == -CUDART_INF_F) ? 0.f : lse_s * exp2f(lse_m - M);
-        float sb = (m2 == -CUDART_INF_F) ? 0.f : s2 * exp2f(m2 - M);
-        bool lo = (lane & off) == 0;
-        lse_s = lo ? sa + sb : sb + sa;
-        lse_m = M;
+    // (posterior per orientation: warps -> orientation, written to p.orient_m / p.orient_s, then orientations -> work item)
+    const int n_or = o_end - o_begin;
+    if (orient) {
+        __syncthreads();
+        if (warp == 0 && lane < n_or) {
+            float m = -CUDART_INF_F, sm = 0.f;
+            for (int w = 0; w < NW; ++w) lse_merge(m, sm, otab[lane * NW + w].x, otab[lane * NW + w].y);
+            otab[lane * NW] = make_float2(m, sm);
+            const size_t oi = ((size_t)model * p.n_orient + o_begin + lane) * p.n_img + img;
+            p.orient_m[oi] = m; p.orient_s[oi] = sm;
+        }
+    } else {
+        warp_lse_reduce(lse_m, lse_s, lane);
+        if (lane == 0) { red[2 * warp] = lse_m; red[2 * warp + 1] = lse_s; }
     }
-    if (lane == 0) { red[2 * warp] = lse_m; red[2 * warp + 1] = lse_s; }
     __syncthreads();
     if (warp == 0) {
         float m = -CUDART_INF_F, s = 0.f;
-        for (int w = 0; w < NW; ++w) lse_merge(m, s, red[2 * w], red[2 * w + 1]);
+        if (orient) for (int w = 0; w < n_or; ++w) lse_merge(m, s, otab[w * NW].x, otab[w * NW].y);
+        else for (int w = 0; w < NW; ++w) lse_merge(m, s, red[2 * w], red[2 * w + 1]);
         // merge the other warps' candidate lists into warp 0's list
         float th0 = tops[BIOEM_TOPK - 1].g;
         for (int w = 1; w < NW; ++w)
@@ -251,7 +277,7 @@ static void smem_plan(int N, int D, int &CB, int &GP, size_t &bytes)
     if (cb > 0) { int nb = (NC + cb - 1) / cb; cb = (NC + nb - 1) / nb; }
     if (cb < NP && cb > 0) { /* pass 2 is batched by the same loop, nothing to do */ }
     CB = (int)cb;
-    bytes = fixed + (size_t)CB * per_col;
+    bytes = fixed + (size_t)CB * per_col + (size_t)32 * NW * 8;       // + the per-orientation table (outside the budget: CB is as without it)
 }
 
 size_t fused_smem_bytes(int N, int D)

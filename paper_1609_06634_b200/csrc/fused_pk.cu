@@ -83,7 +83,10 @@ __device__ __forceinline__ c2 pk_colsum(c2 v)
 // the slots of a half-warp read rows whose shared-memory bank offsets tile the 16 eight-byte banks (conflict-free G loads),
 // and so that the idle slots fill whole warps starting at warp 0 (which carries the extra Nyquist-column work of pass 1).
 struct PkMap { uint16_t e[3][64]; int nvar; };     // nvar variants, used round-robin over the CTF groups (see pk_build_map)
-template <int N, bool DUMP>
+// ORIENT = true (bioem_set_orientation_posterior): each warp also closes its running sums at the end of every orientation of the
+// work item into otab[orientation][warp]; the epilogue combines warps -> orientation (p.orient_m / p.orient_s) -> work item in
+// fixed order.  A template parameter: as a run-time flag in the group loop it cost the default path 7 % (DESIGN 7).
+template <int N, bool DUMP, bool ORIENT>
 __global__ void __launch_bounds__(PK<N>::NT, 1) k_fused_pk(FusedParams p, const float4 *__restrict__ Kt, const float4 *__restrict__ KtN, int CG, int GP, const __grid_constant__ PkMap map)
 {
     typedef PK<N> C_;
@@ -102,6 +105,7 @@ __global__ void __launch_bounds__(PK<N>::NT, 1) k_fused_pk(FusedParams p, const 
     float2 *sc = reinterpret_cast<float2 *>(kn + 8 * N2 + 1);         // [4][CG]          (alpha*beta, h) of the CTFs of the last 4 groups
     TopEntry *tops = reinterpret_cast<TopEntry *>(sc + 4 * CG);       // [NW][TOPK]
     float *red = reinterpret_cast<float *>(tops + NW * BIOEM_TOPK);   // [2 NW]
+    float2 *otab = reinterpret_cast<float2 *>(red + 2 * NW);          // [32][NW]         ORIENT only: (m, s) per orientation of the item and warp
     __shared__ uint64_t mbar[2];                                      // [0] "G rows of group gi written", [1] "G rows of group gi-1 read"
 
     int img, model, o_begin, o_end, item;
@@ -227,6 +231,8 @@ __global__ void __launch_bounds__(PK<N>::NT, 1) k_fused_pk(FusedParams p, const 
     int o = o_begin, c0 = c_lo;
     int nc1 = 0, nc2 = 0;                                             // CTFs in groups gi-1, gi-2 (0 = no such group)
     uint32_t pair1 = 0, pair2 = 0;                                    // o * n_ctf + c0 of those groups
+    bool last1 = false, last2 = false;                                // ORIENT: that group is the last one of its orientation ...
+    int ol1 = 0, ol2 = 0;                                             // ... which is orientation o_begin + ol of the grid
     c2 xs2 = make_float2(0.f, 0.f);                                   // B(dx = +16) of this thread's pass-2 task, from F' to H'
     c2 q[N1];
 #pragma unroll
@@ -305,6 +311,19 @@ __global__ void __launch_bounds__(PK<N>::NT, 1) k_fused_pk(FusedParams p, const 
                     pk_score<DUMP, 2>(p, st, mylist, y, v, sh, s2.x, s2.y, pair2 + (uint32_t)xcl);
                 }
             }
+            if (!DUMP && ORIENT && nc2 > 0 && last2) {
+                // group gi-2 was the last of its orientation: close this warp's sums for it
+                float lse_m = st.m, lse_s = st.s;
+#pragma unroll
+                for (int off = 16; off >= 1; off >>= 1) {
+                    const float m2 = __shfl_xor_sync(FULLP, lse_m, off), s2 = __shfl_xor_sync(FULLP, lse_s, off);
+                    const float M = fmaxf(lse_m, m2);
+                    lse_s = lse_s * pk_ex2(lse_m - M) + s2 * pk_ex2(m2 - M);
+                    lse_m = M;
+                }
+                if (lane == 0) otab[ol2 * NW + warp] = make_float2(lse_m, lse_s);
+                st.m = LSE_EMPTY; st.s = 0.f;
+            }
             PK_LOAD_A(cn)
             PK_FFT_XS()
             if (gi > 0) pk_mbar_wait(&mbar[1], (unsigned)(gi - 1) & 1u);   // every warp has read G[gi & 1] (F' of group gi-2): first write below
@@ -365,6 +384,7 @@ __global__ void __launch_bounds__(PK<N>::NT, 1) k_fused_pk(FusedParams p, const 
         nc2 = nc1; pair2 = pair1; eX = eF;
         var2 = var1; var1 = var0; var0 = var0 + 1 == map.nvar ? 0 : var0 + 1;
         nc1 = live ? nc : 0; pair1 = (uint32_t)((o + p.o_first) * p.n_ctf + c0);
+        if (ORIENT) { last2 = last1; ol2 = ol1; last1 = live && c0 + CG >= c_hi; ol1 = o - o_begin; }
         c0 += CG;
         if (c0 >= c_hi) { c0 = c_lo; ++o; }
     }
@@ -376,20 +396,40 @@ __global__ void __launch_bounds__(PK<N>::NT, 1) k_fused_pk(FusedParams p, const 
     if (DUMP) return;
 
     // ---- block reduction, fixed order
-    float lse_m = st.m, lse_s = st.s;
+    if (ORIENT) {
+        // warps -> orientation: thread i of warp 0 combines the NW entries of orientation i in warp order and writes its
+        // (m, s), kept in otab[i * NW]: the work item's partial below is then the combination of its orientations, in order
+        __syncthreads();
+        if (warp == 0 && lane < o_end - o_begin) {
+            float m = LSE_EMPTY, sm = 0.f;
+            for (int w = 0; w < NW; ++w) {
+                const float2 e = otab[lane * NW + w];
+                const float M = fmaxf(m, e.x);
+                sm = sm * pk_ex2(m - M) + e.y * pk_ex2(e.x - M);
+                m = M;
+            }
+            otab[lane * NW] = make_float2(m, sm);
+            const size_t oi = ((size_t)model * p.n_orient + o_begin + lane) * p.n_img + img;
+            p.orient_m[oi] = sm > 0.f ? m : -CUDART_INF_F;
+            p.orient_s[oi] = sm;
+        }
+    } else {
+        float lse_m = st.m, lse_s = st.s;
 #pragma unroll
-    for (int off = 16; off >= 1; off >>= 1) {
-        const float m2 = __shfl_xor_sync(FULLP, lse_m, off), s2 = __shfl_xor_sync(FULLP, lse_s, off);
-        const float M = fmaxf(lse_m, m2);
-        lse_s = lse_s * pk_ex2(lse_m - M) + s2 * pk_ex2(m2 - M);
-        lse_m = M;
+        for (int off = 16; off >= 1; off >>= 1) {
+            const float m2 = __shfl_xor_sync(FULLP, lse_m, off), s2 = __shfl_xor_sync(FULLP, lse_s, off);
+            const float M = fmaxf(lse_m, m2);
+            lse_s = lse_s * pk_ex2(lse_m - M) + s2 * pk_ex2(m2 - M);
+            lse_m = M;
+        }
+        if (lane == 0) { red[2 * warp] = lse_m; red[2 * warp + 1] = lse_s; }
     }
-    if (lane == 0) { red[2 * warp] = lse_m; red[2 * warp + 1] = lse_s; }
     __syncthreads();
     if (warp == 0) {
         float m = LSE_EMPTY, s = 0.f;
-        for (int w = 0; w < NW; ++w) {
-            const float m2 = red[2 * w], s2 = red[2 * w + 1];
+        const int nred = ORIENT ? o_end - o_begin : NW;
+        for (int w = 0; w < nred; ++w) {
+            const float m2 = ORIENT ? otab[w * NW].x : red[2 * w], s2 = ORIENT ? otab[w * NW].y : red[2 * w + 1];
             const float M = fmaxf(m, m2);
             s = s * pk_ex2(m - M) + s2 * pk_ex2(m2 - M);
             m = M;
@@ -502,7 +542,7 @@ static bool pk_build_map(int N2, int NCOMBO, int CG, int NP, int KK, int GP, PkM
 }
 
 template <int N>
-static void pk_plan(int D, int n_ctf, int &CG, int &GP, size_t &bytes, PkMap &map)
+static void pk_plan(int D, int n_ctf, bool orient, int &CG, int &GP, size_t &bytes, PkMap &map)
 {
     typedef PK<N> C_;
     const int KK = 2 * D + 1, NP = D + 1;
@@ -513,7 +553,7 @@ static void pk_plan(int D, int n_ctf, int &CG, int &GP, size_t &bytes, PkMap &ma
     const size_t budget = 227 * 1024;
     for (;;) {
         bytes = (size_t)C_::NW * C_::ZW * 8 + (size_t)2 * CG * KK * GP * 8 + 16 * C_::N2 * 8 + (8 * C_::N2 + 1) * 16 + 4 * (size_t)CG * 8 +
-                (size_t)C_::NW * BIOEM_TOPK * sizeof(TopEntry) + 2 * C_::NW * 4 + 64;
+                (size_t)C_::NW * BIOEM_TOPK * sizeof(TopEntry) + 2 * C_::NW * 4 + 64 + (orient ? (size_t)32 * C_::NW * sizeof(float2) : 0);
         if ((bytes <= budget && pk_build_map(C_::N2, C_::NCOMBO, CG, NP, KK, GP, map)) || CG == 1) break;
         --CG;
     }
@@ -526,19 +566,26 @@ static cudaError_t launch_pk_t(const FusedParams &p, const float *Kt, bool dump,
     int CG, GP;
     size_t bytes;
     PkMap map;
-    pk_plan<N>(p.D, p.n_ctf, CG, GP, bytes, map);
+    const bool orient = p.orient_m != nullptr && !dump;
+    pk_plan<N>(p.D, p.n_ctf, orient, CG, GP, bytes, map);
     if (bytes > 227 * 1024) return cudaErrorInvalidConfiguration;
+    if (orient && p.oc > 32) return cudaErrorInvalidValue;            // otab holds 32 orientations per work item
     const float4 *kt = reinterpret_cast<const float4 *>(Kt), *ktn = reinterpret_cast<const float4 *>(pk_ktn(N, Kt, p.n_ctf));
     cudaError_t e;
     if (dump) {
-        e = cudaFuncSetAttribute(k_fused_pk<N, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+        e = cudaFuncSetAttribute(k_fused_pk<N, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
         if (e != cudaSuccess) return e;
-        k_fused_pk<N, true><<<1, PK<N>::NT, bytes, st>>>(p, kt, ktn, CG, GP, map);
-    } else {
-        e = cudaFuncSetAttribute(k_fused_pk<N, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+        k_fused_pk<N, true, false><<<1, PK<N>::NT, bytes, st>>>(p, kt, ktn, CG, GP, map);
+    } else if (orient) {
+        e = cudaFuncSetAttribute(k_fused_pk<N, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
         if (e != cudaSuccess) return e;
         const int items = p.n_img * p.n_model * p.chunks_per_model;
-        k_fused_pk<N, false><<<items, PK<N>::NT, bytes, st>>>(p, kt, ktn, CG, GP, map);
+        k_fused_pk<N, false, true><<<items, PK<N>::NT, bytes, st>>>(p, kt, ktn, CG, GP, map);
+    } else {
+        e = cudaFuncSetAttribute(k_fused_pk<N, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+        if (e != cudaSuccess) return e;
+        const int items = p.n_img * p.n_model * p.chunks_per_model;
+        k_fused_pk<N, false, false><<<items, PK<N>::NT, bytes, st>>>(p, kt, ktn, CG, GP, map);
     }
     return cudaGetLastError();
 }

@@ -271,7 +271,11 @@ __device__ __forceinline__ void tm_p2_front(c2 (&a)[16], const c2 *gt, int t)
     pk_fft16(a);
 }
 
-template <bool DUMP>
+// ORIENT = true (bioem_set_orientation_posterior): the running sums are also closed at the end of every orientation of the work
+// item -- each warp reduces its (m, s) over its lanes into otab[orientation][warp] and starts again -- and the epilogue combines
+// warps -> orientation (written to p.orient_m / p.orient_s) -> work item, in fixed order.  A template parameter, not a run-time
+// flag: the flag in the step loop cost the default path 7 % (DESIGN 7).
+template <bool DUMP, bool ORIENT>
 __global__ void __launch_bounds__(TM::NT, 1) k_fused_tm(FusedParams p, const float4 *__restrict__ Kt, const float *__restrict__ KtN)
 {
     constexpr int N = TM::N, NW = TM::NW, ZP = TM::ZP, ZW = TM::ZW, RP = TM::RP, GSZ = TM::GSZ;
@@ -286,6 +290,7 @@ __global__ void __launch_bounds__(TM::NT, 1) k_fused_tm(FusedParams p, const flo
     c2 *qn = G + (size_t)2 * GSZ;                                     // [32][7]        Q of the Nyquist column (warp 0)
     TopEntry *tops = reinterpret_cast<TopEntry *>(qn + 224);    // [NW][TOPK]
     float *red = reinterpret_cast<float *>(tops + NW * BIOEM_TOPK);   // [2 NW]
+    float2 *otab = reinterpret_cast<float2 *>(red + 2 * NW);          // [32][NW]       ORIENT only: (m, s) per orientation of the item and warp
     __shared__ uint64_t bar_full[2], bar_empty[2];
     __shared__ uint32_t tm_base_s;
 
@@ -469,6 +474,19 @@ __global__ void __launch_bounds__(TM::NT, 1) k_fused_tm(FusedParams p, const flo
                                       t2act && (par ? vh_od : vh_ev), gm, pab, ph, ppair);
             }
         }
+        if (!DUMP && ORIENT && s >= 1 && c == c_lo) {
+            // step s - 1 was the last CTF of its orientation: close this warp's sums for it
+            float lse_m = st.m, lse_s = st.s;
+#pragma unroll
+            for (int off = 16; off >= 1; off >>= 1) {
+                const float m2 = __shfl_xor_sync(FULLP, lse_m, off), s2 = __shfl_xor_sync(FULLP, lse_s, off);
+                const float M = fmaxf(lse_m, m2);
+                lse_s = lse_s * pk_ex2(lse_m - M) + s2 * pk_ex2(m2 - M);
+                lse_m = M;
+            }
+            if (lane == 0) otab[(o - 1 - o_begin) * NW + warp] = make_float2(lse_m, lse_s);
+            st.m = LSE_EMPTY; st.s = 0.f;
+        }
         if (live) {
             const size_t moc = ((size_t)model * p.n_orient + o) * p.n_ctf + c;
             pab = p.alpha[moc] * beta; ph = p.hterm[moc];
@@ -482,7 +500,24 @@ __global__ void __launch_bounds__(TM::NT, 1) k_fused_tm(FusedParams p, const flo
     if (DUMP) return;
 
     // ---- block reduction, fixed order
-    {
+    if (ORIENT) {
+        // warps -> orientation: thread i of warp 0 combines the NW entries of orientation i in warp order and writes its (m, s);
+        // (m, s), kept in otab[i * NW]: the work item's partial below is then the combination of its orientations, in order
+        const int n_or = o_end - o_begin;
+        if (warp == 0 && lane < n_or) {
+            float m = LSE_EMPTY, sm = 0.f;
+            for (int w = 0; w < NW; ++w) {
+                const float2 e = otab[lane * NW + w];
+                const float M = fmaxf(m, e.x);
+                sm = sm * pk_ex2(m - M) + e.y * pk_ex2(e.x - M);
+                m = M;
+            }
+            otab[lane * NW] = make_float2(m, sm);
+            const size_t oi = ((size_t)model * p.n_orient + o_begin + lane) * p.n_img + img;
+            p.orient_m[oi] = sm > 0.f ? m : -CUDART_INF_F;
+            p.orient_s[oi] = sm;
+        }
+    } else {
         float lse_m = st.m, lse_s = st.s;
 #pragma unroll
         for (int off = 16; off >= 1; off >>= 1) {
@@ -496,8 +531,9 @@ __global__ void __launch_bounds__(TM::NT, 1) k_fused_tm(FusedParams p, const flo
     __syncthreads();
     if (warp == 0) {
         float m = LSE_EMPTY, s = 0.f;
-        for (int w = 0; w < NW; ++w) {
-            const float m2 = red[2 * w], s2 = red[2 * w + 1];
+        const int nred = ORIENT ? o_end - o_begin : NW;
+        for (int w = 0; w < nred; ++w) {
+            const float m2 = ORIENT ? otab[w * NW].x : red[2 * w], s2 = ORIENT ? otab[w * NW].y : red[2 * w + 1];
             const float M = fmaxf(m, m2);
             s = s * pk_ex2(m - M) + s2 * pk_ex2(m2 - M);
             m = M;
@@ -549,19 +585,27 @@ cudaError_t launch_relayout_K_tm(const float *K32, float *Kt, int n_ctf, cudaStr
 // Work items: one CTA per (image, model, chunk); one partial per work item.
 cudaError_t launch_fused_tm(const FusedParams &p, const float *Kt, bool dump, cudaStream_t st)
 {
-    const size_t bytes = ((size_t)TM::NW * TM::ZW + 2 * TM::GSZ + 224) * 8 + (size_t)TM::NW * BIOEM_TOPK * sizeof(TopEntry) + 2 * TM::NW * 4 + 64;
+    const bool orient = p.orient_m != nullptr && !dump;
+    const size_t bytes = ((size_t)TM::NW * TM::ZW + 2 * TM::GSZ + 224) * 8 + (size_t)TM::NW * BIOEM_TOPK * sizeof(TopEntry) + 2 * TM::NW * 4 + 64 +
+                         (orient ? (size_t)32 * TM::NW * sizeof(float2) : 0);
+    if (orient && p.oc > 32) return cudaErrorInvalidValue;            // otab holds 32 orientations per work item
     const float4 *kt = reinterpret_cast<const float4 *>(Kt);
     const float *ktn = tm_ktn(Kt, p.n_ctf);
     cudaError_t e;
     if (dump) {
-        e = cudaFuncSetAttribute(k_fused_tm<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+        e = cudaFuncSetAttribute(k_fused_tm<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
         if (e != cudaSuccess) return e;
-        k_fused_tm<true><<<1, TM::NT, bytes, st>>>(p, kt, ktn);
-    } else {
-        e = cudaFuncSetAttribute(k_fused_tm<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+        k_fused_tm<true, false><<<1, TM::NT, bytes, st>>>(p, kt, ktn);
+    } else if (orient) {
+        e = cudaFuncSetAttribute(k_fused_tm<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
         if (e != cudaSuccess) return e;
         const int items = p.n_img * p.n_model * p.chunks_per_model;
-        k_fused_tm<false><<<items, TM::NT, bytes, st>>>(p, kt, ktn);
+        k_fused_tm<false, true><<<items, TM::NT, bytes, st>>>(p, kt, ktn);
+    } else {
+        e = cudaFuncSetAttribute(k_fused_tm<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+        if (e != cudaSuccess) return e;
+        const int items = p.n_img * p.n_model * p.chunks_per_model;
+        k_fused_tm<false, false><<<items, TM::NT, bytes, st>>>(p, kt, ktn);
     }
     return cudaGetLastError();
 }

@@ -306,6 +306,45 @@ def test_orientation_posterior(name):
         assert np.abs(m + np.log(np.exp(got - m[:, None]).sum(axis=1)) - full).max() <= TOL_LOGP
 
 
+@pytest.mark.parametrize("name,kernel,chunk", [("small_mini", 0, 3), ("small_mini", 0, 32), ("small_mini", 1, 5), ("paper_mini", 0, 3),
+                                               ("paper_mini", 0, 64), ("paper_mini", 3, 4), ("paper_mini", 1, 7), ("density_mini", 0, 4), ("tiny_mid", 0, 48)])
+def test_orientation_posterior_folded_in_chunked_work_items(name, kernel, chunk):
+    """SURVEY 8(f) #1, second half: the per-orientation sums are closed INSIDE the chunked work items (several orientations per
+    thread block, ragged last chunk), not by running one orientation per work item.  Same bar as test_orientation_posterior;
+    the chunk is capped at 32 (the table in shared memory) and the cluster kernel (3) falls back to one orientation per item."""
+    import oracle
+    from paper_1609_06634_b200 import BioEM
+    wl = W.build_workload(name)
+    s = wl["spec"]
+    n, n_or = s.n_pix ** 2, len(wl["quats"])
+    with BioEM() as b:
+        b.load_workload(wl)
+        b.debug_set_kernel(kernel)
+        b.set_orientation_chunk(chunk)
+        b.run()
+        base_lp, base_best = b.get_log_posterior(), b.get_best()
+        b.set_orientation_posterior(True)
+        b.run()
+        kern, oc = b.get_run_plan()
+        po, lp, best = b.get_orientation_log_posterior(), b.get_log_posterior(), b.get_best()
+        b.run()
+        po2 = b.get_orientation_log_posterior()
+    assert kern == (kernel or (4 if s.n_pix == 224 else 2)) and oc == (1 if kernel == 3 else min(chunk, 32, n_or))   # 0: k_fused_pk / k_fused_tm
+    assert np.array_equal(po, po2)                                 # fixed combination order: bitwise repeatable
+    assert np.abs(lp - base_lp).max() <= 1e-3
+    for k in ("orient", "ctf", "dx", "dy"):
+        assert np.array_equal(best[k], base_best[k])
+    tol = 5e-7 * n + 1e-3
+    for mi, model in enumerate(wl["models"]):
+        ref = oracle.orientation_log_posterior(model, s.n_pix, s.pixel_A, s.max_shift, wl["quats"], wl["ctfs"], wl["images"])
+        got = po[:, mi, :]
+        rel = ref >= ref.max(axis=1, keepdims=True) - 30.0
+        assert np.abs(got - ref)[rel].max() <= tol, np.abs(got - ref)[rel].max()
+        assert np.abs(got - ref).max() <= 10 * tol
+        m = got.max(axis=1)
+        assert np.abs(m + np.log(np.exp(got - m[:, None]).sum(axis=1)) - lp[:, mi]).max() <= 1e-3
+
+
 def test_ensemble_posterior_eq10():
     """Eq. 10 (SURVEY 8(f) #4) from the log-posteriors of a run, against the oracle's Eq. 10 on the ORACLE's log-posteriors."""
     import oracle

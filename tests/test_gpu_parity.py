@@ -345,6 +345,46 @@ def test_orientation_posterior_folded_in_chunked_work_items(name, kernel, chunk)
         assert np.abs(m + np.log(np.exp(got - m[:, None]).sum(axis=1)) - lp[:, mi]).max() <= 1e-3
 
 
+@pytest.mark.parametrize("name", ["small", "paper"])
+def test_orientation_posterior_full_size_sampled(name):
+    """The option at BASELINE.json's full size in the automatic launch shape (32 orientations per work item, so every entry comes
+    out of the in-kernel fold): (1) the log-sum-exp over orientations is the log-posterior of the same run, every image;
+    (2) the other outputs equal those of a run without the option; (3) sampled entries -- for 3 images the best orientation, its
+    chunk neighbours and random ones -- against the oracle's direct summation over that orientation (weights of the full grid)."""
+    import oracle
+    from paper_1609_06634_b200 import BioEM
+    wl = W.build_workload(name)
+    s = wl["spec"]
+    n, n_or = s.n_pix ** 2, len(wl["quats"])
+    rng = np.random.default_rng(11)
+    with BioEM() as b:
+        b.load_workload(wl)
+        b.run()
+        base_lp, base_best = b.get_log_posterior(), b.get_best()
+        b.set_orientation_posterior(True)
+        b.run()
+        assert b.get_run_plan()[1] == 32
+        po, lp, best = b.get_orientation_log_posterior(), b.get_log_posterior(), b.get_best()
+    assert np.abs(lp - base_lp).max() <= 1e-3
+    for k in ("orient", "ctf", "dx", "dy"):
+        assert np.array_equal(best[k], base_best[k])
+    got = po[:, 0, :]
+    m = got.max(axis=1)
+    assert np.abs(m + np.log(np.exp(got - m[:, None]).sum(axis=1)) - lp[:, 0]).max() <= 1e-3
+    assert np.array_equal(got.argmax(axis=1), best["orient"][:, 0])       # the best term dominates its orientation's sum
+    tol = 5e-7 * n + 1e-3
+    model = oracle.prepare_model(wl["models"][0])
+    for img in rng.choice(s.n_images, 3, replace=False):
+        ob = int(best["orient"][img, 0])
+        picks = {ob, max(ob - 1, 0), min(ob + 1, n_or - 1), (ob // 32) * 32, min((ob // 32) * 32 + 31, n_or - 1)}
+        picks |= {int(x) for x in rng.integers(n_or, size=3)}
+        for o in sorted(picks):
+            ref = oracle.run_model(model, s.n_pix, s.pixel_A, s.max_shift, wl["quats"], wl["ctfs"], wl["images"][img:img + 1],
+                                   o_begin=o, o_end=o + 1).log_posterior()[0]
+            bar = tol if ref >= lp[img, 0] - 30.0 else 10 * tol
+            assert abs(got[img, o] - ref) <= bar, (img, o, got[img, o], ref)
+
+
 def test_ensemble_posterior_eq10():
     """Eq. 10 (SURVEY 8(f) #4) from the log-posteriors of a run, against the oracle's Eq. 10 on the ORACLE's log-posteriors."""
     import oracle

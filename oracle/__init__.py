@@ -308,6 +308,40 @@ def ensemble_log_posterior(logp, weights=None):
     return float(per.sum()), per
 
 
+def synthetic_map(I1, dx, dy, obs=None, crop=False):
+    """Synthetic map ("print the synthetic map corresponding to a specific parameter set theta") for
+    theta = (orientation, CTF parameters: the calculated image I1 of Eqs. 1-5; centre displacement d = (dx, dy);
+    normalisation N and offset mu), which is I_cal of Eq. 7:   S(k, j) = N * I_d(k, j) - mu,   with the displaced image of
+    bo_cross_corr_direct / bo_cropped_sums: I_d(k, j) = I1((k + dy) mod n, (j + dx) mod n) (Fourier variant, R5), or, with
+    crop=True (real-space variant, R25), I1(k + dy, j + dx) inside the box and 0 outside.
+    obs=None: N = 1, mu = 0.  Otherwise (N, mu) are the values that maximise the likelihood of Eq. 8 for that image at any
+    lambda, i.e. that minimise sum (obs - N I_d + mu)^2; setting both derivatives to zero (the sums in the paper's notation):
+        N = (n C_co - C_o C_c) / (n C_cc - C_c^2),      mu = (N C_c - C_o) / n       (Eq. 7 SUBTRACTS mu).
+    Returns (S, N, mu).  Plain loops over the pixels."""
+    I1 = np.asarray(I1, dtype=np.float64)
+    n1 = I1.shape[0]
+    Id = np.zeros_like(I1)
+    for k in range(n1):
+        for j in range(n1):
+            k2, j2 = k + dy, j + dx
+            if crop:
+                if 0 <= k2 < n1 and 0 <= j2 < n1:
+                    Id[k, j] = I1[k2, j2]
+            else:
+                Id[k, j] = I1[k2 % n1, j2 % n1]
+    if obs is None:
+        return Id, 1.0, 0.0
+    obs = np.asarray(obs, dtype=np.float64)
+    n = float(n1 * n1)
+    Co = Cc = Ccc = Cco = 0.0
+    for k in range(n1):
+        for j in range(n1):
+            Co += obs[k, j]; Cc += Id[k, j]; Ccc += Id[k, j] * Id[k, j]; Cco += obs[k, j] * Id[k, j]
+    N_ = (n * Cco - Co * Cc) / (n * Ccc - Cc * Cc)
+    mu = (N_ * Cc - Co) / n
+    return N_ * Id - mu, N_, mu
+
+
 def shift_map(image, I1, D, logw, tier=0):
     """log P(C1) + logw for every shift of one (image, calc image) pair: [dy+D][dx+D]."""
     image = np.ascontiguousarray(image, dtype=np.float32)

@@ -444,6 +444,50 @@ def test_cropping_variant_equals_circular_variant_when_nothing_reaches_the_borde
     assert np.abs(a.log_posterior() - b.log_posterior()).max() > 1e-6
 
 
+# ------------------------------------------------------------------ synthetic map for a parameter set theta
+def test_synthetic_map_displacement_is_the_one_of_the_cross_correlation():
+    # sum_r obs(r) S(r) with N = 1, mu = 0 IS C_co(d) of bo_cross_corr_direct (wrapping, R5) / bo_cropped_sums (cropping, R25):
+    # a flipped sign or swapped axis of d in either place breaks this
+    rng = np.random.default_rng(5)
+    N, D = 9, 3
+    obs, cal = rng.normal(size=(N, N)), rng.normal(size=(N, N))
+    circ = oracle.cross_corr_direct(obs, cal, D)
+    crop, _, _ = oracle.cropped_sums(obs, cal, D)
+    for dy in range(-D, D + 1):
+        for dx in range(-D, D + 1):
+            S, n_, mu = oracle.synthetic_map(cal, dx, dy)
+            assert (n_, mu) == (1.0, 0.0) and abs((obs * S).sum() - circ[dy + D, dx + D]) < 1e-12
+            Sc, _, _ = oracle.synthetic_map(cal, dx, dy, crop=True)
+            assert abs((obs * Sc).sum() - crop[dy + D, dx + D]) < 1e-12
+    # by hand: a single pixel of the calculated image at (k, j) = (3, 7), displaced by (dx, dy) = (+1, +2), appears at (1, 6);
+    # displaced by dx = -2 it leaves the 9-pixel box on the right: wrapped to column 0, cropped away
+    cal = np.zeros((N, N)); cal[3, 7] = 2.5
+    want = np.zeros((N, N)); want[1, 6] = 2.5
+    assert np.array_equal(oracle.synthetic_map(cal, 1, 2)[0], want) and np.array_equal(oracle.synthetic_map(cal, 1, 2, crop=True)[0], want)
+    want = np.zeros((N, N)); want[3, 0] = 2.5
+    assert np.array_equal(oracle.synthetic_map(cal, -2, 0)[0], want) and not oracle.synthetic_map(cal, -2, 0, crop=True)[0].any()
+
+
+def test_synthetic_map_normalisation_and_offset_maximise_eq8():
+    rng = np.random.default_rng(6)
+    N = 10
+    cal = rng.normal(size=(N, N))
+    Id = oracle.synthetic_map(cal, 2, -1)[0]
+    # exact recovery: an image that IS I_cal of Eq. 7 with N = 2.5, mu = 0.7 (the offset is SUBTRACTED there)
+    S, n_, mu = oracle.synthetic_map(cal, 2, -1, obs=2.5 * Id - 0.7)
+    assert abs(n_ - 2.5) < 1e-12 and abs(mu - 0.7) < 1e-12 and np.abs(S - (2.5 * Id - 0.7)).max() < 1e-12
+    # library routine: linear least squares of obs on (I_d, 1)
+    obs = 1.7 * Id + 0.3 + rng.normal(size=(N, N))
+    S, n_, mu = oracle.synthetic_map(cal, 2, -1, obs=obs)
+    ref = np.linalg.lstsq(np.stack([Id.ravel(), np.ones(N * N)], axis=1), obs.ravel(), rcond=None)[0]
+    assert abs(n_ - ref[0]) < 1e-10 and abs(mu + ref[1]) < 1e-10 and np.abs(S - (n_ * Id - mu)).max() < 1e-12
+    # the paper's likelihood (Eq. 8, bo_log_lik_eq8) is largest there, at any lambda
+    for lam in (0.4, 1.3):
+        top = oracle.log_lik_eq8(obs, Id, n_, mu, lam)
+        for dn, dm in ((1e-3, 0), (-1e-3, 0), (0, 1e-3), (0, -1e-3), (7e-4, -7e-4)):
+            assert oracle.log_lik_eq8(obs, Id, n_ + dn, mu + dm, lam) < top
+
+
 # ------------------------------------------------------------------ Eq. 9 on the grid (R7, R15, R16)
 def test_planted_truth_is_the_argmax():
     # north_star check 2: a noiseless, CTF-free image at a grid orientation and shift scores its maximum exactly there

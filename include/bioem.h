@@ -131,6 +131,18 @@ int bioem_get_orientation_log_posterior(bioem_ctx *ctx, double *out);
  * inner log-sums) or NULL.  FP64, fixed summation order. */
 int bioem_get_ensemble_log_posterior(bioem_ctx *ctx, const double *weights, double *out_total, double *out_per_image);
 
+/* Synthetic map (paper section 3.8: "print the synthetic map corresponding to a specific parameter set theta"): the calculated
+ * image I_cal of Eq. 7 for theta = (orient, ctf, d = (dx, dy), N, mu) of `model`,
+ *   out[k][j] = N * I1(k + dy, j + dx) - mu        (row-major [N][N] floats, caller-allocated; I1 of Eqs. 1-5 in FP64),
+ * displaced the way the run scores it: wrapped around the box (displacement variant 0, R5) or cut off at the borders (variant 1,
+ * R25); |dx|, |dy| < n_pix, not limited to the shift range.  fit_to_image = NULL: N = 1, mu = 0.  Otherwise a host image
+ * [N][N] (e.g. the particle whose bioem_get_best parameters are passed): N and mu are the values that maximise the likelihood of
+ * Eq. 8 for that image (least squares; a constant calculated image gives N = 0), returned in out_norm_offset[0..1] if not NULL.
+ * Needs a completed bioem_run on this context (its spectra are reused; `orient` must lie in the context's orientation slice).
+ * Synchronises the stream. */
+int bioem_get_synthetic_map(bioem_ctx *ctx, int model, int orient, int ctf, int dx, int dy, const float *fit_to_image, float *out,
+                            double *out_norm_offset);
+
 /* Work decomposition of bioem_run: one work item (thread block) scores one image against `n_orient_per_item` consecutive
  * orientations x all CTFs x all shifts of one model (the image-stationary loop order of DESIGN.md section 8; P:199-203 has
  * the loops the other way round).  0 = automatic: >= 32 work items per SM, at most 32 orientations per item.  The value

@@ -20,7 +20,7 @@ EXPORTED_SYMBOLS = [
     "bioem_set_orientation_chunk", "bioem_debug_set_kernel", "bioem_get_run_plan", "bioem_invalidate_precompute",
     "bioem_set_orientation_slice", "bioem_run_partial", "bioem_get_partials_size", "bioem_export_partials", "bioem_merge_partials",
     "bioem_rescore_local", "bioem_export_rescore", "bioem_import_rescore", "bioem_finish", "bioem_set_displacement_variant",
-    "bioem_noalloc_prepare", "bioem_ensemble_log_posterior_noalloc", "bioem_noalloc_last_error",
+    "bioem_get_synthetic_map", "bioem_noalloc_prepare", "bioem_ensemble_log_posterior_noalloc", "bioem_noalloc_last_error",
 ]
 NOALLOC_MAX_IMG, NOALLOC_MAX_MODEL = 65536, 1024
 KERNEL_AUTO, KERNEL_GENERIC, KERNEL_PK, KERNEL_C2, KERNEL_TM, KERNEL_DFT, KERNEL_REALSPACE = 0, 1, 2, 3, 4, 5, 6
@@ -86,6 +86,7 @@ def lib():
         L.bioem_set_orientation_chunk.argtypes = [C.c_void_p, C.c_int]
         L.bioem_debug_set_kernel.argtypes = [C.c_void_p, C.c_int]
         L.bioem_get_run_plan.argtypes = [C.c_void_p, C.POINTER(C.c_int), C.POINTER(C.c_int)]
+        L.bioem_get_synthetic_map.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, _fp, _fp, _dp]
         L.bioem_noalloc_prepare.argtypes = [C.c_int]
         L.bioem_ensemble_log_posterior_noalloc.argtypes = [C.c_int, C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         L.bioem_noalloc_last_error.argtypes = []
@@ -341,6 +342,17 @@ class BioEM:
                                                         ptr(out_total), ptr(out_per_image))
         if rc:
             raise BioEMError(rc, BioEM.noalloc_last_error())
+
+    def get_synthetic_map(self, model, orient, ctf, dx=0, dy=0, fit_to_image=None):
+        """I_cal of Eq. 7 for one parameter set: (map [N][N] float32, normalisation N, offset mu)."""
+        out = np.empty((self.n_pix, self.n_pix), dtype=np.float32)
+        no = np.zeros(2)
+        fp = None
+        if fit_to_image is not None:
+            img, fp = _f32(fit_to_image)
+            assert img.shape == (self.n_pix, self.n_pix)
+        self._ck(self._L.bioem_get_synthetic_map(self._h, model, orient, ctf, int(dx), int(dy), fp, out.ctypes.data_as(_fp), no.ctypes.data_as(_dp)))
+        return out, float(no[0]), float(no[1])
 
     def debug_calc_image(self, model, orient, ctf):
         out = np.empty((self.n_pix, self.n_pix), dtype=np.float32)

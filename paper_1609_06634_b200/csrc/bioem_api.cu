@@ -873,6 +873,35 @@ int bioem_debug_calc_image(bioem_ctx *ctx, int model, int orient, int ctf, float
     return BIOEM_OK;
 }
 
+// the synthetic map of a parameter set -- the calculated image of (model, orient, ctf), displaced, scaled and offset (Eq. 7)
+int bioem_get_synthetic_map(bioem_ctx *ctx, int model, int orient, int ctf, int dx, int dy, const float *fit_to_image, float *out,
+                            double *out_norm_offset)
+{
+    if (!ctx || !out) return BIOEM_EBADARG;
+    int rc = check_tuple(ctx, 0, model, orient, ctf);
+    if (rc) return rc;
+    const int N = ctx->N;
+    if (dx <= -N || dx >= N || dy <= -N || dy >= N) FAIL(BIOEM_EBADARG, "get_synthetic_map: |dx|, |dy| must be < n_pix");
+    CK(cudaSetDevice(ctx->device));
+    cudaStream_t st = ctx->stream;
+    const size_t n = (size_t)N * N, H = (size_t)(N / 2 + 1) * N;
+    CK(ctx->dump.ensure((n + 2) * sizeof(double) + n * sizeof(float)));
+    double *I1 = ctx->dump.as<double>(), *no = I1 + n;
+    float *dout = reinterpret_cast<float *>(no + 2);
+    const float *dobs = nullptr;
+    if (fit_to_image) {
+        CK(ctx->staging.ensure(n * sizeof(float)));
+        CK(cudaMemcpyAsync(ctx->staging.p, fit_to_image, n * sizeof(float), cudaMemcpyHostToDevice, st));
+        dobs = ctx->staging.as<float>();
+    }
+    CK(launch_calc_image(ctx->F064.as<cd>() + ((size_t)model * ctx->run_o_local + (orient - ctx->run_o_first)) * H, ctx->K64.as<double>() + (size_t)ctf * H, N, I1, st));
+    CK(launch_synth_map(I1, dobs, N, dx, dy, ctx->variant == 1, dout, no, st));
+    rc = fetch(ctx, out, dout, n * sizeof(float));
+    if (rc) return rc;
+    if (out_norm_offset) CK(cudaMemcpy(out_norm_offset, no, 2 * sizeof(double), cudaMemcpyDeviceToHost));
+    return BIOEM_OK;
+}
+
 int bioem_debug_shift_map(bioem_ctx *ctx, int img, int model, int orient, int ctf, double *out)
 {
     if (!ctx || !out) return BIOEM_EBADARG;

@@ -107,6 +107,7 @@ cudaError_t launch_orient_final(const float *part_m, const float *part_s, int pa
                                 double *logp_orient, cudaStream_t st);
 cudaError_t launch_ensemble(const double *logp, const double *logw, int n_img, int n_model, double *per_image, double *total, cudaStream_t st);
 cudaError_t launch_calc_image(const cd *F0, const double *K64, int N, double *out, cudaStream_t st);
+cudaError_t launch_synth_map(const double *I1, const float *obs, int N, int dx, int dy, int crop, float *out, double *norm_offset, cudaStream_t st);
 cudaError_t launch_fp32_peak(float *sink, int iters, cudaStream_t st);
 
 // real-space, cropping displacement variant (realspace.cu)

@@ -436,4 +436,56 @@ cudaError_t launch_calc_image(const cd *F0, const double *K64, int N, double *ou
     return cudaGetLastError();
 }
 
+// ------------------------------------------------------------------------------------------------ synthetic map
+// I_cal of Eq. 7 for one parameter set: out = N I_d - mu, I_d(k, j) = I1(k + dy, j + dx), wrapped around the box (crop = 0,
+// the Fourier variant, R5) or zero outside it (crop = 1, the real-space variant, R25).  obs = NULL: N = 1, mu = 0; otherwise the
+// (N, mu) that maximise Eq. 8 for that image (normal equations of sum (obs - N I_d + mu)^2).  One CTA, FP64, fixed summation
+// order: thread t takes pixels t, t + 1024, ...; lanes by xor-tree; warps in order.
+__global__ void __launch_bounds__(1024) k_synth_map(const double *I1, const float *obs, int N, int dx, int dy, int crop, float *out, double *norm_offset)
+{
+    __shared__ double sh[4][32];
+    __shared__ double fit[2];
+    const int n = N * N, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    auto displaced = [&](int pix) -> double {
+        int k2 = pix / N + dy, j2 = pix % N + dx;
+        if (crop) {
+            if (k2 < 0 || k2 >= N || j2 < 0 || j2 >= N) return 0.0;
+        } else {
+            k2 = (k2 % N + N) % N; j2 = (j2 % N + N) % N;
+        }
+        return I1[(size_t)k2 * N + j2];
+    };
+    double nn = 1.0, mu = 0.0;
+    if (obs) {
+        double v[4] = {0.0, 0.0, 0.0, 0.0};                          // C_o, C_c, C_cc, C_co
+        for (int pix = tid; pix < n; pix += 1024) {
+            const double o = obs[pix], c = displaced(pix);
+            v[0] += o; v[1] += c; v[2] += c * c; v[3] += o * c;
+        }
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            for (int off = 16; off >= 1; off >>= 1) v[q] += __shfl_xor_sync(0xffffffffu, v[q], off);
+            if (lane == 0) sh[q][warp] = v[q];
+        }
+        __syncthreads();
+        if (tid == 0) {
+            double s[4] = {0.0, 0.0, 0.0, 0.0};
+            for (int q = 0; q < 4; ++q)
+                for (int w = 0; w < 32; ++w) s[q] += sh[q][w];
+            const double den = (double)n * s[2] - s[1] * s[1];     // T_c of the displaced image
+            const double a = den > 0.0 ? ((double)n * s[3] - s[0] * s[1]) / den : 0.0;      // a constant calculated image: only the offset fits
+            fit[0] = a; fit[1] = (a * s[1] - s[0]) / (double)n;
+        }
+        __syncthreads();
+        nn = fit[0]; mu = fit[1];
+    }
+    for (int pix = tid; pix < n; pix += 1024) out[pix] = (float)(nn * displaced(pix) - mu);
+    if (tid == 0 && norm_offset) { norm_offset[0] = nn; norm_offset[1] = mu; }
+}
+cudaError_t launch_synth_map(const double *I1, const float *obs, int N, int dx, int dy, int crop, float *out, double *norm_offset, cudaStream_t st)
+{
+    k_synth_map<<<1, 1024, 0, st>>>(I1, obs, N, dx, dy, crop, out, norm_offset);
+    return cudaGetLastError();
+}
+
 }  // namespace bioem

@@ -385,6 +385,44 @@ def test_orientation_posterior_full_size_sampled(name):
             assert abs(got[img, o] - ref) <= bar, (img, o, got[img, o], ref)
 
 
+@pytest.mark.parametrize("name,variant", [("tiny_mini", 0), ("paper_mini", 0), ("density_mini", 0), ("small_mini", 1)])
+def test_synthetic_map(name, variant):
+    """P:223 (SURVEY 8(f) #4): the synthetic map of a parameter set, I_cal of Eq. 7, element by element against the oracle --
+    at each image's maximising parameters with (N, mu) fitted to that image, and at hand-picked displacements beyond the shift
+    range with N = 1, mu = 0; wrapped (variant 0) or cropped at the borders (variant 1).  Tolerance: the calculated image is
+    FP64 on both sides (2e-6 relative, as for debug_calc_image), the map is returned in float."""
+    import oracle
+    from paper_1609_06634_b200 import BioEM
+    wl = W.build_workload(name)
+    s = wl["spec"]
+    N = s.n_pix
+    model = oracle.prepare_model(wl["models"][0])
+    with BioEM() as b:
+        b.load_workload(wl, images=False)
+        b.set_displacement_variant(variant)
+        b.push_images(wl["images"])
+        b.run()
+        best = b.get_best()
+        cases = [(i, int(best["orient"][i, 0]), int(best["ctf"][i, 0]), int(best["dx"][i, 0]), int(best["dy"][i, 0]), True) for i in range(min(3, s.n_images))]
+        cases += [(0, 1, 0, N // 2 + 3, -5, False), (0, 0, 1, -(N - 1), N - 1, False), (1, 2, 0, 0, 0, True)]
+        for img, o, c, dx, dy, fit in cases:
+            got, gn, gmu = b.get_synthetic_map(0, o, c, dx, dy, wl["images"][img] if fit else None)
+            I1 = oracle.calc_image(model, wl["quats"][o], wl["ctfs"][c], N, s.pixel_A)
+            ref, rn, rmu = oracle.synthetic_map(I1, dx, dy, wl["images"][img] if fit else None, crop=bool(variant))
+            scale = np.abs(ref).max()
+            assert np.abs(got - ref).max() <= 2e-6 * scale + 1e-6 * scale, (img, o, c, dx, dy, np.abs(got - ref).max(), scale)
+            assert abs(gn - rn) <= 1e-5 * abs(rn) + 1e-12 and abs(gmu - rmu) <= 1e-5 * max(abs(rmu), scale), (gn, rn, gmu, rmu)
+            if not fit:
+                assert (gn, gmu) == (1.0, 0.0)
+        # the fitted map is the least-squares image: its residual against the particle is orthogonal to the map and to a constant
+        img = 0
+        got, gn, gmu = b.get_synthetic_map(0, cases[0][1], cases[0][2], cases[0][3], cases[0][4], wl["images"][img])
+        r = wl["images"][img].astype(np.float64) - got
+        assert abs(r.sum()) <= 1e-4 * np.abs(wl["images"][img]).sum() and abs((r * got).sum()) <= 1e-4 * np.abs(wl["images"][img] * got).sum()
+        with pytest.raises(Exception):
+            b.get_synthetic_map(0, 0, 0, N, 0)
+
+
 def test_ensemble_posterior_eq10():
     """Eq. 10 (SURVEY 8(f) #4) from the log-posteriors of a run, against the oracle's Eq. 10 on the ORACLE's log-posteriors."""
     import oracle

@@ -121,7 +121,9 @@ int bioem_get_best(bioem_ctx *ctx, int32_t *orient_idx, int32_t *ctf_idx, int32_
  * off executes the same code as before).  The table has 32 rows, so the chunk is capped at 32.  The terms that the FP64
  * re-scoring replaces (the 8 largest per image and model) are replaced here too; the others keep FP32 accuracy
  * (R24).  enable: 0 | 1.  get_: caller-allocated [n_img][n_model][n_orient] doubles; BIOEM_EBADSTATE if the
- * last run was made without the option. */
+ * last run was made without the option.  On a context that holds an orientation slice (bioem_set_orientation_slice) the output
+ * is that rank's part, [n_img][n_model][o_end - o_begin]: the values are those of the undivided run, bit for bit, and the ranks'
+ * parts concatenated along the last axis are its output (shard.run_orientation_sharded gathers them). */
 int bioem_set_orientation_posterior(bioem_ctx *ctx, int enable);
 int bioem_get_orientation_log_posterior(bioem_ctx *ctx, double *out);
 

@@ -219,6 +219,7 @@ class BioEM:
     # ---- the run in phases (orientation sharding, include/bioem.h)
     def set_orientation_slice(self, o_begin=0, o_end=-1):
         self._ck(self._L.bioem_set_orientation_slice(self._h, int(o_begin), int(o_end)))
+        self._slice = (int(o_begin), int(o_end)) if o_end >= 0 else None
 
     def run_partial(self):
         self._ck(self._L.bioem_run_partial(self._h))
@@ -306,7 +307,9 @@ class BioEM:
         self._ck(self._L.bioem_set_orientation_posterior(self._h, int(bool(enable))))
 
     def get_orientation_log_posterior(self):
-        out = np.empty((self.n_img, self.n_models, self.n_orient))
+        """[n_img][n_model][orientations of this context's slice (the whole grid without one)]"""
+        sl = getattr(self, "_slice", None)
+        out = np.empty((self.n_img, self.n_models, sl[1] - sl[0] if sl else self.n_orient))
         self._ck(self._L.bioem_get_orientation_log_posterior(self._h, out.ctypes.data_as(_dp)))
         return out
 

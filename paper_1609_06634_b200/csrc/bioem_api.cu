@@ -394,7 +394,6 @@ int bioem_run_partial(bioem_ctx *ctx)
     const bool sliced = ctx->slice_end >= 0;
     const int o_first = sliced ? ctx->slice_begin : 0, O = (sliced ? ctx->slice_end : Ofull) - o_first;      // resident orientations
     if (sliced && (o_first < 0 || O < 0 || o_first + O > Ofull)) FAIL(BIOEM_EBADARG, "run: orientation slice outside the grid");
-    if (sliced && ctx->want_orient) FAIL(BIOEM_EUNSUPPORTED, "run: the per-orientation posterior is not available on an orientation slice");
     CK(cudaSetDevice(ctx->device));
     cudaStream_t st = ctx->stream;
     const size_t n = (size_t)N * N, H = (size_t)(N / 2 + 1) * N;
@@ -419,6 +418,7 @@ int bioem_run_partial(bioem_ctx *ctx)
     // posterior per orientation: the chunked kernels close their sums per orientation in a shared-memory table of 32 rows;
     // the cluster kernel (a cross-check, never chosen automatically) has no such table and runs one orientation per work item
     const bool fold = ctx->want_orient && !use_c2;
+    if (sliced && ctx->want_orient && !fold) FAIL(BIOEM_EUNSUPPORTED, "run: the per-orientation posterior on an orientation slice needs a kernel that folds it (not the cluster kernel)");
     if (ctx->want_orient && !fold) oc = 1;
     if (fold && oc > 32) oc = 32;
     if (sliced && o_first % oc != 0) FAIL(BIOEM_EBADARG, "run: an orientation slice must begin at a multiple of the orientation chunk");
@@ -704,9 +704,11 @@ int bioem_finish(bioem_ctx *ctx)
         const size_t items = IM * ctx->run_chunks;
         const float *part_m = ctx->run_orient_folded ? ctx->orient_m.as<float>() : ctx->blob.as<float>();
         const float *part_s = ctx->run_orient_folded ? ctx->orient_s.as<float>() : part_m + items;
-        CK(ctx->logp_orient.ensure(IM * ctx->run_orient * sizeof(double)));
-        CK(launch_orient_final(part_m, part_s, ctx->run_orient_folded ? 1 : 2, ctx->top.as<TopEntry>(), ctx->g64.as<double>(), ctx->Dw.as<double>(), I, M,
-                               ctx->run_orient, ctx->run_ctf, N, const_n, ctx->logp_orient.as<double>(), st));
+        // the resident orientations only: a rank of an orientation-sharded run produces its slice of the output
+        CK(ctx->logp_orient.ensure(IM * std::max(ctx->run_o_local, 1) * sizeof(double)));
+        if (ctx->run_o_local > 0)
+            CK(launch_orient_final(part_m, part_s, ctx->run_orient_folded ? 1 : 2, ctx->top.as<TopEntry>(), ctx->g64.as<double>(), ctx->Dw.as<double>(), I, M,
+                                   ctx->run_o_local, ctx->run_o_first, ctx->run_ctf, N, const_n, ctx->logp_orient.as<double>(), st));
         ctx->launches += 1;
         ctx->ran_orient = true;
     }
@@ -792,7 +794,7 @@ int bioem_get_orientation_log_posterior(bioem_ctx *ctx, double *out)
 {
     if (!ctx || !out) return BIOEM_EBADARG;
     if (!ctx->ran || !ctx->ran_orient) FAIL(BIOEM_EBADSTATE, "get_orientation_log_posterior: no completed run with the option enabled");
-    return fetch(ctx, out, ctx->logp_orient.p, (size_t)ctx->run_img * ctx->run_models * ctx->run_orient * sizeof(double));
+    return fetch(ctx, out, ctx->logp_orient.p, (size_t)ctx->run_img * ctx->run_models * ctx->run_o_local * sizeof(double));
 }
 
 int bioem_get_ensemble_log_posterior(bioem_ctx *ctx, const double *weights, double *out_total, double *out_per_image)

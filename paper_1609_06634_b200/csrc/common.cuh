@@ -103,7 +103,7 @@ cudaError_t launch_final(const double *m32, const double *s32, const TopEntry *t
                          int n_img, int n_model, int n_ctf, int N, int D, double const_n, double *logp, double *logp32,
                          int32_t *best, double *best_logp, cudaStream_t st);
 cudaError_t launch_orient_final(const float *part_m, const float *part_s, int parts_per_orient, const TopEntry *top, const double *g64,
-                                const double *Dw, int n_img, int n_model, int n_orient, int n_ctf, int N, double const_n,
+                                const double *Dw, int n_img, int n_model, int n_orient, int o_first, int n_ctf, int N, double const_n,
                                 double *logp_orient, cudaStream_t st);
 cudaError_t launch_ensemble(const double *logp, const double *logw, int n_img, int n_model, double *per_image, double *total, cudaStream_t st);
 cudaError_t launch_calc_image(const cd *F0, const double *K64, int N, double *out, cudaStream_t st);

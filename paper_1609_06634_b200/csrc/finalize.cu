@@ -182,11 +182,12 @@ cudaError_t launch_final(const double *m32, const double *s32, const TopEntry *t
     return cudaGetLastError();
 }
 
-// Posterior per orientation: with one orientation per work item the per-item partials ARE the per-orientation sums.
-// One thread per (image, model, orientation): combine the item's partials in order (the cluster kernel writes two), replace
-// the re-scored terms of this orientation by their FP64 values, add the constants.
+// Posterior per orientation from the per-orientation (m, s) the fused kernels wrote (the folded table, ppo = 1; or, cluster
+// kernel with one orientation per work item, its two partials, ppo = 2).  One thread per (image, model, resident orientation):
+// combine in order, replace the re-scored terms of this orientation -- candidates carry GLOBAL orientation indices, local
+// orientation o is o + o_first of the grid -- by their FP64 values, add the constants.  out [img][model][o].
 __global__ void k_orient_final(const float *part_m, const float *part_s, int ppo, const TopEntry *top, const double *g64, const double *Dw,
-                               int n_img, int n_model, int n_orient, int n_ctf, int N, double const_n, double *out)
+                               int n_img, int n_model, int n_orient, int o_first, int n_ctf, int N, double const_n, double *out)
 {
     const size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (idx >= (size_t)n_img * n_model * n_orient) return;
@@ -207,10 +208,10 @@ __global__ void k_orient_final(const float *part_m, const float *part_s, int ppo
     const double *g = g64 + (size_t)im * BIOEM_TOPK;
     double ref = Mn;
     for (int k = 0; k < BIOEM_TOPK; ++k)
-        if (t[k].pair != 0xffffffffu && (int)(t[k].pair / n_ctf) == o && g[k] > ref) ref = g[k];
+        if (t[k].pair != 0xffffffffu && (int)(t[k].pair / n_ctf) == o + o_first && g[k] > ref) ref = g[k];
     double tot = S * exp(Mn - ref), t32 = 0.0, t64 = 0.0;
     for (int k = 0; k < BIOEM_TOPK; ++k)
-        if (t[k].pair != 0xffffffffu && (int)(t[k].pair / n_ctf) == o) {
+        if (t[k].pair != 0xffffffffu && (int)(t[k].pair / n_ctf) == o + o_first) {
             t32 += exp((double)t[k].g * LN2 - ref);
             t64 += exp(g[k] - ref);
         }
@@ -220,11 +221,11 @@ __global__ void k_orient_final(const float *part_m, const float *part_s, int ppo
 }
 
 cudaError_t launch_orient_final(const float *part_m, const float *part_s, int parts_per_orient, const TopEntry *top, const double *g64,
-                                const double *Dw, int n_img, int n_model, int n_orient, int n_ctf, int N, double const_n,
+                                const double *Dw, int n_img, int n_model, int n_orient, int o_first, int n_ctf, int N, double const_n,
                                 double *logp_orient, cudaStream_t st)
 {
     const size_t n = (size_t)n_img * n_model * n_orient;
-    k_orient_final<<<(unsigned)((n + 127) / 128), 128, 0, st>>>(part_m, part_s, parts_per_orient, top, g64, Dw, n_img, n_model, n_orient, n_ctf, N,
+    k_orient_final<<<(unsigned)((n + 127) / 128), 128, 0, st>>>(part_m, part_s, parts_per_orient, top, g64, Dw, n_img, n_model, n_orient, o_first, n_ctf, N,
                                                                 const_n, logp_orient);
     return cudaGetLastError();
 }

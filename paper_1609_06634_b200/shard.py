@@ -102,21 +102,26 @@ def orientation_shard(n_orient: int, chunk: int, rank: int, world: int) -> tuple
     return min(b * chunk, n_orient), min(e * chunk, n_orient)
 
 
-def run_orientation_sharded(ctx, chunk: int, group=None) -> dict:
+def run_orientation_sharded(ctx, chunk: int, group=None, orientation_posterior: bool = False) -> dict:
     """Score the images pushed into `ctx` against the whole grid with the orientation grid sharded over the ranks of `group`
     ("MPI over orientations").  `ctx` is a configured BioEM context (models, grids, images; the same on every rank).
     Exchange steps ("absence of communication" but for the final gather): one all_gather of the per-chunk partials, one
     all_reduce of the FP64 re-scored candidates.  Every rank returns the full results, bit-identical to one GPU with
-    set_orientation_chunk(chunk) (include/bioem.h)."""
+    set_orientation_chunk(chunk) (include/bioem.h).  orientation_posterior=True adds "logp_orient" [I][M][O]: every rank
+    computes the entries of its own orientations, one more all_gather puts the parts side by side."""
     import torch
     import torch.distributed as dist
 
     on = dist.is_available() and dist.is_initialized()
     world = dist.get_world_size(group) if on else 1
     rank = dist.get_rank(group) if on else 0
+    if orientation_posterior:
+        chunk = min(chunk, 32)                                               # the library's cap with that option (include/bioem.h)
     ob, oe = orientation_shard(ctx.n_orient, chunk, rank, world)
     ctx.set_orientation_chunk(chunk)
     ctx.set_orientation_slice(ob, oe)
+    if orientation_posterior:
+        ctx.set_orientation_posterior(True)
     try:
         ctx.run_partial()
         if world == 1:
@@ -143,6 +148,21 @@ def run_orientation_sharded(ctx, chunk: int, group=None) -> dict:
             dist.all_reduce(g, op=dist.ReduceOp.SUM, group=group)            # owner's value + exact zeros
             ctx.import_rescore(g)
         ctx.finish()
-        return dict(logp=ctx.get_log_posterior(), **ctx.get_best())
+        out = dict(logp=ctx.get_log_posterior(), **ctx.get_best())
+        if orientation_posterior:
+            part = ctx.get_orientation_log_posterior()                       # [I][M][oe - ob]
+            if world == 1:
+                out["logp_orient"] = part
+            else:
+                spans = [orientation_shard(ctx.n_orient, chunk, r, world) for r in range(world)]
+                width = max(max(e - b for b, e in spans), 1)
+                mine = torch.zeros(part.shape[:2] + (width,), dtype=torch.float64, device=dev)
+                mine[:, :, : oe - ob] = torch.from_numpy(part).to(dev)
+                parts = [torch.empty_like(mine) for _ in range(world)]
+                dist.all_gather(parts, mine, group=group)
+                out["logp_orient"] = np.concatenate([p[:, :, : e - b].cpu().numpy() for p, (b, e) in zip(parts, spans)], axis=2)
+        return out
     finally:
         ctx.set_orientation_slice(0, -1)
+        if orientation_posterior:
+            ctx.set_orientation_posterior(False)

@@ -631,6 +631,62 @@ def test_orientation_sharding_is_bit_identical(name, chunk, world):
     assert np.abs(one["logp"] - ref["logp"]).max() <= TOL_LOGP
 
 
+@pytest.mark.parametrize("name,chunk,world", [("small_mid", 5, 3), ("paper_mid", 4, 2), ("ensemble_mid", 48, 2)])
+def test_orientation_posterior_under_orientation_sharding(name, chunk, world):
+    """8(f) #1 with 8(f) #5: every rank (a context on this GPU, the exchanges by hand as above) produces the per-orientation
+    posterior of ITS orientations; side by side they are the output of one context over the whole grid, bit for bit.  A chunk
+    above the option's cap of 32 is cut to it on both sides (shard.run_orientation_sharded does the same)."""
+    from paper_1609_06634_b200 import BioEM
+    from paper_1609_06634_b200.shard import orientation_shard
+    wl = W.build_workload(name)
+    s = wl["spec"]
+    chunk = min(chunk, 32)
+    with BioEM() as b:
+        b.load_workload(wl)
+        b.set_orientation_chunk(chunk)
+        b.set_orientation_posterior(True)
+        b.run()
+        one, one_lp = b.get_orientation_log_posterior(), b.get_log_posterior()
+    assert one.shape == (s.n_images, s.n_models, s.n_orient)
+    ctxs = [BioEM() for _ in range(world)]
+    try:
+        blobs, sizes, chunks, spans = [], [], [], []
+        for r, c in enumerate(ctxs):
+            c.load_workload(wl)
+            c.set_orientation_chunk(chunk)
+            spans.append(orientation_shard(s.n_orient, chunk, r, world))
+            c.set_orientation_slice(*spans[-1])
+            c.set_orientation_posterior(True)
+            c.run_partial()
+            nb, nc = c.get_partials_size()
+            buf = np.zeros(max(nb, 4), np.uint8)
+            c.export_partials(buf)
+            blobs.append(buf); sizes.append(nb); chunks.append(nc)
+        stride = max(max(sizes), 4)
+        allb = np.zeros(world * stride, np.uint8)
+        for r, bb in enumerate(blobs):
+            allb[r * stride: r * stride + bb.size] = bb
+        g = np.zeros(ctxs[0].rescore_shape())
+        for c in ctxs:
+            c.merge_partials(allb, stride, chunks)
+            c.rescore_local()
+            gr = np.empty_like(g)
+            c.export_rescore(gr)
+            g += gr
+        parts = []
+        for c, (ob, oe) in zip(ctxs, spans):
+            c.import_rescore(g)
+            c.finish()
+            assert np.array_equal(c.get_log_posterior(), one_lp)
+            part = c.get_orientation_log_posterior()
+            assert part.shape == (s.n_images, s.n_models, oe - ob)
+            parts.append(part)
+        assert np.array_equal(np.concatenate(parts, axis=2), one)
+    finally:
+        for c in ctxs:
+            c.close()
+
+
 def test_orientation_slice_errors():
     from paper_1609_06634_b200 import BioEM
     from paper_1609_06634_b200.binding import BioEMError

@@ -154,6 +154,22 @@ class _FakeCtx:
     def finish(self):
         pass
 
+    def set_orientation_posterior(self, on):
+        self.want_po = bool(on)
+
+    def get_orientation_log_posterior(self):
+        """This rank's orientations only, [I][M][e - b]: the FP32 score, with the re-scored candidates that fall on the
+        orientation (known on every rank after the all_reduce) added -- so a wrong gather AND a stale g both show."""
+        assert self.want_po
+        b, e = self.sl
+        out = self.score[:, :, b:e].astype(np.float64)
+        for k in range(self.K):
+            c = self.cand[:, :, k]
+            own = (c >= b) & (c < e)
+            i, m = np.nonzero(own)
+            out[i, m, c[i, m] - b] += self.g[i, m, k]
+        return out
+
     def get_log_posterior(self):
         return self.tot.astype(np.float64) + self.g.max(axis=2)
 
@@ -169,7 +185,7 @@ def _orient_worker(rank, world, port, q):
     os.environ["MASTER_PORT"] = str(port)
     dist.init_process_group("gloo", rank=rank, world_size=world)
     try:
-        out = run_orientation_sharded(_FakeCtx(5, 2, 43), chunk=4)        # 11 chunks, the last one ragged: 6 + 5 over two ranks
+        out = run_orientation_sharded(_FakeCtx(5, 2, 43), chunk=4, orientation_posterior=True)   # 11 chunks, the last one ragged: 6 + 5 over two ranks
         q.put((rank, {k: v.tolist() for k, v in out.items()}))
     finally:
         dist.destroy_process_group()
@@ -190,7 +206,9 @@ def test_orientation_sharding_two_ranks_equal_one_rank():
     for p in procs:
         p.join(timeout=60)
         assert p.exitcode == 0
-    want = run_orientation_sharded(_FakeCtx(5, 2, 43), chunk=4)           # no process group: one rank, the whole grid
+    want = run_orientation_sharded(_FakeCtx(5, 2, 43), chunk=4, orientation_posterior=True)    # no process group: one rank, the whole grid
+    assert want["logp_orient"].shape == (5, 2, 43)
     for r in range(2):
         assert np.array_equal(np.array(got[r]["logp"]), want["logp"])                   # bit-identical on every rank
+        assert np.array_equal(np.array(got[r]["logp_orient"]), want["logp_orient"])     # each rank's part, side by side
         assert np.array_equal(np.array(got[r]["orient"], dtype=np.int32), want["orient"])

@@ -39,7 +39,7 @@ def _worker(rank, world, port, backend, q):
         by_img = run_sharded(make_ctx, wl["images"])
         with make_ctx() as b:
             b.push_images(wl["images"])
-            by_ori = run_orientation_sharded(b, CHUNK)
+            by_ori = run_orientation_sharded(b, CHUNK, orientation_posterior=True)
         q.put((rank, {k: np.asarray(v).tolist() for k, v in by_img.items()}, {k: np.asarray(v).tolist() for k, v in by_ori.items()}))
     finally:
         dist.destroy_process_group()
@@ -73,7 +73,11 @@ def test_two_ranks_reproduce_one_rank(backend):
         b.set_orientation_chunk(CHUNK)
         b.run()
         want = dict(logp=b.get_log_posterior(), **b.get_best())
+        b.set_orientation_posterior(True)                                    # the orientation-sharded run asks for P:225 too
+        b.run()
+        want_po = dict(logp=b.get_log_posterior(), logp_orient=b.get_orientation_log_posterior(), **b.get_best())
     for r in range(2):
-        for which in (0, 1):                                                 # images sharded, orientations sharded
-            for k, v in want.items():
+        for which, ref in ((0, want), (1, want_po)):                         # images sharded, orientations sharded
+            assert set(got[r][which]) == set(ref)
+            for k, v in ref.items():
                 assert np.array_equal(np.asarray(got[r][which][k], dtype=v.dtype), v), (r, which, k)

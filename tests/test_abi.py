@@ -66,6 +66,25 @@ def test_host_only_helper_and_error_paths(library):
     assert library.bioem_create(None, 0, None) != 0                                                # NULL out pointer
 
 
+def test_noalloc_entry_point_checks_its_arguments_before_touching_the_device(library):
+    """bioem_ensemble_log_posterior_noalloc: NULL pointers and sizes beyond the fixed work array are refused with a message and
+    nothing is enqueued (the checks come before the first CUDA call, so they run here without a device)."""
+    from paper_1609_06634_b200 import binding
+    one = ctypes.c_void_p(8)                                       # never dereferenced: the calls below return before any launch
+    f = library.bioem_ensemble_log_posterior_noalloc
+    assert f(0, None, 4, 2, None, None, one, None) == -1
+    assert f(0, None, 4, 2, one, None, None, None) == -1
+    assert f(0, None, 0, 2, one, None, one, None) == -1
+    assert f(0, None, binding.NOALLOC_MAX_IMG + 1, 2, one, None, one, None) == -5
+    msg = library.bioem_noalloc_last_error().decode()
+    assert str(binding.NOALLOC_MAX_IMG) in msg and "at most" in msg
+    assert f(0, None, 4, binding.NOALLOC_MAX_MODEL + 1, one, None, one, None) == -5
+    assert library.bioem_noalloc_prepare(-1) == -1 and library.bioem_noalloc_prepare(64) == -1
+    header = HEADER.read_text()
+    assert f"#define BIOEM_NOALLOC_MAX_IMG   {binding.NOALLOC_MAX_IMG}" in header
+    assert f"#define BIOEM_NOALLOC_MAX_MODEL {binding.NOALLOC_MAX_MODEL}" in header
+
+
 def test_no_device_means_loud_failure(library):
     import torch
     if torch.cuda.is_available():

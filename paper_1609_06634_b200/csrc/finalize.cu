@@ -12,27 +12,31 @@ __device__ __forceinline__ bool before(const TopEntry &a, const TopEntry &b)
     return a.g > b.g || (a.g == b.g && (a.pair < b.pair || (a.pair == b.pair && a.shift < b.shift)));
 }
 
-// One thread per (image, model): combine the per-work-item partials in chunk order (bit-reproducible).  The partials arrive as
-// `n_blobs` blobs of `stride` bytes (one per rank when the orientation grid is sharded; one otherwise), blob r
-// holding chunks_of_blob[r] chunks per model: float m[n_r], float s[n_r], TopEntry top[n_r][TOPK], n_r = n_model * chunks * n_img,
-// item = (model * chunks + chunk) * n_img + img.  Blobs in rank order = chunks in grid order, so the sums and the candidate
-// lists come out exactly as on one GPU with the same chunking.
-__global__ void k_merge(const unsigned char *blobs, size_t stride, const int *chunks_of_blob, int n_blobs, int n_img, int n_model, double *m32,
-                        double *s32, TopEntry *top)
+// One WARP per (image, model): combine the per-work-item partials (bit-reproducible: the result is a fixed function of the
+// sequence of chunks).  The partials arrive as `n_blobs` blobs of `stride` bytes (one per rank when the orientation grid is sharded,
+// P:199; one otherwise), blob r holding chunks_of_blob[r] chunks per model: float m[n_r], float s[n_r], TopEntry
+// top[n_r][TOPK], n_r = n_model * chunks * n_img, item = (model * chunks + chunk) * n_img + img.  Blobs in rank order = chunks in
+// grid order; lane i takes the chunks whose index in that ONE sequence is i, i + 32, ... -- where the blobs are cut does not
+// enter, so the sums and the candidate lists come out exactly as on one GPU with the same chunking.
+//   sums:       each lane adds its chunks in order, then a butterfly over the lanes (both partners compute the same a + b)
+//   candidates: the K best of all lists under the strict total order `before` -- a set that does not depend on any order of
+//               evaluation -- picked one after the other: round k takes the best entry that comes after pick k - 1.
+// (As one thread per (image, model) walking the chunks it took 0.20 ms on Tiny, 2.5 x the fused kernel: 64 dependent rounds of
+// loads and an insertion sort in local memory.)
+__global__ void __launch_bounds__(128) k_merge(const unsigned char *blobs, size_t stride, const int *chunks_of_blob, int n_blobs, int n_img, int n_model,
+                                               double *m32, double *s32, TopEntry *top)
 {
-    const int im = blockIdx.x * blockDim.x + threadIdx.x;
-    if (im >= n_img * n_model) return;
+    constexpr unsigned FULL = 0xffffffffu;
+    const int im = blockIdx.x * 4 + (threadIdx.x >> 5), lane = threadIdx.x & 31;
+    if (im >= n_img * n_model) return;                               // warp-uniform
     const int img = im / n_model, model = im % n_model;
+    // ---- sums
     double M = -CUDART_INF, S = 0.0;
-    TopEntry best[BIOEM_TOPK];
-#pragma unroll
-    for (int k = 0; k < BIOEM_TOPK; ++k) best[k] = {-CUDART_INF_F, 0xffffffffu, 0xffffffffu};
-    for (int r = 0; r < n_blobs; ++r) {
+    for (int r = 0, g0 = 0; r < n_blobs; ++r) {
         const int cpm = chunks_of_blob[r];
         const size_t n_r = (size_t)n_model * cpm * n_img;
         const float *part_m = reinterpret_cast<const float *>(blobs + (size_t)r * stride), *part_s = part_m + n_r;
-        const TopEntry *part_top = reinterpret_cast<const TopEntry *>(part_s + n_r);
-        for (int ch = 0; ch < cpm; ++ch) {
+        for (int ch = ((lane - g0) % 32 + 32) % 32; ch < cpm; ch += 32) {
             const size_t item = ((size_t)model * cpm + ch) * n_img + img;
             const double m = part_m[item], s = part_s[item];
             if (m != -CUDART_INF) {
@@ -40,25 +44,57 @@ __global__ void k_merge(const unsigned char *blobs, size_t stride, const int *ch
                 else if (m > M) { S = S * exp2(M - m) + s; M = m; }          // base-2 units
                 else S += s * exp2(m - M);
             }
-            for (int k = 0; k < BIOEM_TOPK; ++k) {
-                TopEntry e = part_top[item * BIOEM_TOPK + k];
-                if (e.pair == 0xffffffffu) break;
-                if (!before(e, best[BIOEM_TOPK - 1])) continue;
-                int pos = BIOEM_TOPK - 1;
-                while (pos > 0 && before(e, best[pos - 1])) { best[pos] = best[pos - 1]; --pos; }
-                best[pos] = e;
+        }
+        g0 += cpm;
+    }
+#pragma unroll
+    for (int off = 16; off >= 1; off >>= 1) {
+        const double m2 = __shfl_xor_sync(FULL, M, off), s2 = __shfl_xor_sync(FULL, S, off);
+        const double Mx = fmax(M, m2);
+        const double a = M == -CUDART_INF ? 0.0 : S * exp2(M - Mx), b = m2 == -CUDART_INF ? 0.0 : s2 * exp2(m2 - Mx);
+        S = a + b; M = Mx;                                           // a + b == b + a: both partners hold the same bits
+    }
+    if (lane == 0) { m32[im] = M; s32[im] = S; }
+    // ---- candidates
+    const TopEntry none = {-CUDART_INF_F, 0xffffffffu, 0xffffffffu};
+    TopEntry prev = none;
+    for (int k = 0; k < BIOEM_TOPK; ++k) {
+        TopEntry cand = none;
+        for (int r = 0, g0 = 0; r < n_blobs; ++r) {
+            const int cpm = chunks_of_blob[r];
+            const size_t n_r = (size_t)n_model * cpm * n_img;
+            const TopEntry *part_top = reinterpret_cast<const TopEntry *>(reinterpret_cast<const float *>(blobs + (size_t)r * stride) + 2 * n_r);
+            for (int ch = ((lane - g0) % 32 + 32) % 32; ch < cpm; ch += 32) {
+                const TopEntry *list = part_top + (((size_t)model * cpm + ch) * n_img + img) * BIOEM_TOPK;
+                for (int j = 0; j < BIOEM_TOPK; ++j) {               // every entry: a list need not be in `before` order among equal g
+                    const TopEntry e = list[j];
+                    if (e.pair == 0xffffffffu) break;
+                    if (e.g != e.g || (k > 0 && !before(prev, e))) continue;
+                    if (cand.pair == 0xffffffffu || before(e, cand)) cand = e;
+                }
             }
+            g0 += cpm;
+        }
+#pragma unroll
+        for (int off = 16; off >= 1; off >>= 1) {
+            TopEntry o;
+            o.g = __shfl_xor_sync(FULL, cand.g, off); o.pair = __shfl_xor_sync(FULL, cand.pair, off); o.shift = __shfl_xor_sync(FULL, cand.shift, off);
+            if (o.pair != 0xffffffffu && (cand.pair == 0xffffffffu || before(o, cand))) cand = o;
+        }
+        if (lane == 0) top[(size_t)im * BIOEM_TOPK + k] = cand;      // `none` once the lists are exhausted
+        prev = cand;
+        if (cand.pair == 0xffffffffu) {
+            if (lane == 0) for (int kk = k + 1; kk < BIOEM_TOPK; ++kk) top[(size_t)im * BIOEM_TOPK + kk] = none;
+            break;
         }
     }
-    m32[im] = M; s32[im] = S;
-    for (int k = 0; k < BIOEM_TOPK; ++k) top[(size_t)im * BIOEM_TOPK + k] = best[k];
 }
 
 cudaError_t launch_merge(const unsigned char *blobs, size_t stride, const int *chunks_of_blob, int n_blobs, int n_img, int n_model, double *m32,
                          double *s32, TopEntry *top, cudaStream_t st)
 {
     int n = n_img * n_model;
-    k_merge<<<(n + 63) / 64, 64, 0, st>>>(blobs, stride, chunks_of_blob, n_blobs, n_img, n_model, m32, s32, top);
+    k_merge<<<(n + 3) / 4, 128, 0, st>>>(blobs, stride, chunks_of_blob, n_blobs, n_img, n_model, m32, s32, top);
     return cudaGetLastError();
 }
 

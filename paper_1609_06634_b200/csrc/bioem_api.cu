@@ -454,13 +454,13 @@ int bioem_run_partial(bioem_ctx *ctx)
         }
 
         // ---- a1/a1' + a2: spectra of the projections of the resident orientations, model by model, batch by batch
-        const int OB = 1024;                                          // orientations per projection batch (scratch: 40 bytes per pixel and orientation)
+        const int OB = 2048;                                          // orientations per projection batch (scratch: 32 bytes per pixel and orientation: 1.6 GB at 224^2)
         const double *rot = ctx->rot.as<double>() + (size_t)o_first * 9;
         for (int mi = 0; mi < M && O > 0; ++mi) {
             Model &m = ctx->models[mi];
             cd *F64m = ctx->F064.as<cd>() + (size_t)mi * O * H;
+            cf *F32m = ctx->F032.as<cf>() + (size_t)mi * O * H;
             if (m.kind == 0) {
-                CK(ctx->scratch_a.ensure((size_t)OB * n * sizeof(double)));      // I0 (double)
                 CK(ctx->scratch_b.ensure((size_t)OB * H * sizeof(cd)));          // transform intermediate
                 CK(ctx->scratch_c.ensure((size_t)OB * n * sizeof(long long)));   // fixed-point accumulator
                 // fixed-point scale: a pixel can never hold more than the total |weight| of the model
@@ -470,9 +470,11 @@ int bioem_run_partial(bioem_ctx *ctx)
                 for (int o0 = 0; o0 < O; o0 += OB) {
                     const int nb = std::min(OB, O - o0);
                     CK(launch_project_atoms(m.xyz.as<double>(), m.rad.as<double>(), m.wt.as<double>(), m.n_atoms, rot + (size_t)o0 * 9,
-                                            nb, N, ctx->px, fx_scale, ctx->scratch_c.as<long long>(), ctx->scratch_a.as<double>(), st));
-                    CK(launch_fft2_r2c_f64(ctx->scratch_a.as<double>(), nb, N, ctx->scratch_b.as<cd>(), F64m + (size_t)o0 * H, st));
-                    ctx->launches += 4;
+                                            nb, N, ctx->px, fx_scale, ctx->scratch_c.as<long long>(), st));
+                    // I0 = fixed-point / scale, converted as the row transform loads it; the FP32 spectrum is written with the FP64 one
+                    CK(launch_fft2_r2c_fixed(ctx->scratch_c.as<long long>(), 1.0 / fx_scale, nb, N, ctx->scratch_b.as<cd>(), F64m + (size_t)o0 * H,
+                                             F32m + (size_t)o0 * H, st));
+                    ctx->launches += 3;
                 }
             } else {
                 const size_t n3 = (size_t)N * N * N;
@@ -480,16 +482,16 @@ int bioem_run_partial(bioem_ctx *ctx)
                 CK(ctx->scratch_b.ensure(n3 * sizeof(cd)));
                 CK(launch_dft3_f64(m.rho.as<float>(), N, ctx->scratch_a.as<cd>(), ctx->scratch_b.as<cd>(), st));
                 CK(launch_slice_f64(ctx->scratch_a.as<cd>(), N, m.voxel, rot, O, F64m, st));
-                ctx->launches += 6;
+                CK(launch_cast_spectrum(F64m, F32m, (size_t)O * H, st));
+                ctx->launches += 7;
             }
         }
         if (O > 0) {
-            CK(launch_cast_spectrum(ctx->F064.as<cd>(), ctx->F032.as<cf>(), MO * H, st));
             CK(launch_calc_stats(ctx->F064.as<cd>(), ctx->K64.as<double>(), (int)MO, O, Ofull, C, N,
                                  ctx->has_lp_orient ? ctx->lp_orient.as<double>() + o_first : nullptr,
                                  ctx->has_lp_ctf ? ctx->lp_ctf.as<double>() : nullptr, std::log((double)(2 * D + 1) * (2 * D + 1)),
                                  ctx->Tc64.as<double>(), ctx->h64.as<double>(), ctx->alpha32.as<float>(), ctx->h32.as<float>(), ctx->flags.as<int>() + 1, st));
-            ctx->launches += 2;
+            ctx->launches += 1;
         }
     }
 

@@ -78,10 +78,11 @@ cudaError_t launch_fused_tm(const FusedParams &p, const float *Kt, bool dump, cu
 // precompute
 cudaError_t launch_image_stats(const float *img, int n_img, int N, double *centered, double *Dw, cudaStream_t st);
 cudaError_t launch_fft2_r2c_f64(const double *in, int batch, int N, cd *tmp, cd *out, cudaStream_t st);   // out [b][l][m]
+cudaError_t launch_fft2_r2c_fixed(const long long *in, double in_scale, int batch, int N, cd *tmp, cd *out, cf *out32, cudaStream_t st);
 cudaError_t launch_cast_spectrum(const cd *in, cf *out, size_t count, cudaStream_t st);
 cudaError_t launch_zero_dc(cd *spec, int batch, size_t H, cudaStream_t st);
 cudaError_t launch_project_atoms(const double *xyz, const double *rad, const double *wt, int n_atoms, const double *rot,
-                                 int n_orient, int N, double px, double fx_scale, long long *acc, double *out, cudaStream_t st);
+                                 int n_orient, int N, double px, double fx_scale, long long *acc, cudaStream_t st);
 cudaError_t launch_dft3_f64(const float *rho, int N, cd *work_a, cd *work_b, cudaStream_t st);           // result in work_a, centred sign applied
 cudaError_t launch_slice_f64(const cd *Vc, int N, double voxel, const double *rot, int n_orient, cd *out, cudaStream_t st);
 cudaError_t launch_ctf_tables(const double *a, const double *A, const double *b, int n_ctf, int N, double px,

@@ -63,10 +63,14 @@ cudaError_t launch_beta(const double *Dw, int n_img, float *beta, int *flags, cu
 
 // ------------------------------------------------------------------------------------------------ generic FP64 1-D transform (two-step)
 // y[k] = sum_e x[e] exp(SIGN 2 pi i e k / N), k < kout.  Sequence g: batch b = g / spb, s = g % spb;
-// x[e] at in + b*ibs + s*iss + e*ies (real or complex), y[k] at out + b*obs + s*oss + k*oes.
-template <int N, int SIGN, bool REAL_IN, int SPB>
-__global__ void __launch_bounds__(SPB *(N / n1_of(N))) k_fft1d_f64(const void *in_, long ibs, long iss, long ies, cd *out, long obs,
-                                                                    long oss, long oes, int nseq, int spb, int kout)
+// x[e] at in + b*ibs + s*iss + e*ies, y[k] at out + b*obs + s*oss + k*oes.  IN = IN_CPLX: complex input; IN_REAL: real doubles;
+// IN_FIXED: the 64-bit fixed-point pixels k_project accumulates, x = (double)q * in_scale (the conversion pass of its own that
+// round 2 began with was 4 ms of the Ensemble step).  out32 != NULL: the result is also written as complex<float> at the same
+// index (the FP32 copy the hot loop reads; was a pass of its own too).
+enum { IN_CPLX = 0, IN_REAL = 1, IN_FIXED = 2 };
+template <int N, int SIGN, int IN, int SPB>
+__global__ void __launch_bounds__(SPB *(N / n1_of(N))) k_fft1d_f64(const void *in_, double in_scale, long ibs, long iss, long ies, cd *out, cf *out32,
+                                                                    long obs, long oss, long oes, int nseq, int spb, int kout)
 {
     constexpr int N1 = n1_of(N), N2 = N / N1, ZP = N1 + 1, LB = ilog2(N1), NT = SPB * N2;
     __shared__ cd Z[SPB * N2 * ZP];
@@ -85,7 +89,8 @@ __global__ void __launch_bounds__(SPB *(N / n1_of(N))) k_fft1d_f64(const void *i
 #pragma unroll
         for (int j = 0; j < N1; ++j) {
             long e = off + (long)(N2 * j + t) * ies;
-            if (REAL_IN) a[j] = {reinterpret_cast<const double *>(in_)[e], 0.0};
+            if (IN == IN_REAL) a[j] = {reinterpret_cast<const double *>(in_)[e], 0.0};
+            else if (IN == IN_FIXED) a[j] = {(double)reinterpret_cast<const long long *>(in_)[e] * in_scale, 0.0};
             else a[j] = reinterpret_cast<const cd *>(in_)[e];
         }
         fft_dif<double, N1, SIGN>(a);
@@ -105,7 +110,9 @@ __global__ void __launch_bounds__(SPB *(N / n1_of(N))) k_fft1d_f64(const void *i
             acc.x += w.x * z.x - w.y * z.y;
             acc.y += w.x * z.y + w.y * z.x;
         }
-        out[(long)(g2 / spb) * obs + (long)(g2 % spb) * oss + (long)k * oes] = acc;
+        const long oi = (long)(g2 / spb) * obs + (long)(g2 % spb) * oss + (long)k * oes;
+        out[oi] = acc;
+        if (out32) out32[oi] = {(float)acc.x, (float)acc.y};
     }
 }
 
@@ -114,28 +121,29 @@ __global__ void __launch_bounds__(SPB *(N / n1_of(N))) k_fft1d_f64(const void *i
 // projections took 25 ms)
 __host__ __device__ constexpr int spb_of(int N) { return N == 64 ? 32 : N == 128 ? 16 : N == 96 ? 16 : N == 170 ? 4 : 8; }
 
-template <int N, int SIGN, bool REAL_IN>
-static cudaError_t fft1d_n(const void *in, long ibs, long iss, long ies, cd *out, long obs, long oss, long oes, int nseq, int spb, int kout,
-                           cudaStream_t st)
+template <int N, int SIGN, int IN>
+static cudaError_t fft1d_n(const void *in, double in_scale, long ibs, long iss, long ies, cd *out, cf *out32, long obs, long oss, long oes, int nseq,
+                           int spb, int kout, cudaStream_t st)
 {
     constexpr int SPB = spb_of(N);
-    k_fft1d_f64<N, SIGN, REAL_IN, SPB><<<(nseq + SPB - 1) / SPB, SPB * (N / n1_of(N)), 0, st>>>(in, ibs, iss, ies, out, obs, oss, oes, nseq, spb, kout);
+    k_fft1d_f64<N, SIGN, IN, SPB><<<(nseq + SPB - 1) / SPB, SPB * (N / n1_of(N)), 0, st>>>(in, in_scale, ibs, iss, ies, out, out32, obs, oss, oes, nseq,
+                                                                                      spb, kout);
     return cudaGetLastError();
 }
 
-template <int SIGN, bool REAL_IN>
+template <int SIGN, int IN>
 static cudaError_t fft1d(int N, const void *in, long ibs, long iss, long ies, cd *out, long obs, long oss, long oes, int nseq,
-                         int spb, int kout, cudaStream_t st)
+                         int spb, int kout, cudaStream_t st, double in_scale = 1.0, cf *out32 = nullptr)
 {
     switch (N) {
-    case 64: return fft1d_n<64, SIGN, REAL_IN>(in, ibs, iss, ies, out, obs, oss, oes, nseq, spb, kout, st);
-    case 96: return fft1d_n<96, SIGN, REAL_IN>(in, ibs, iss, ies, out, obs, oss, oes, nseq, spb, kout, st);
-    case 128: return fft1d_n<128, SIGN, REAL_IN>(in, ibs, iss, ies, out, obs, oss, oes, nseq, spb, kout, st);
-    case 160: return fft1d_n<160, SIGN, REAL_IN>(in, ibs, iss, ies, out, obs, oss, oes, nseq, spb, kout, st);
-    case 170: return fft1d_n<170, SIGN, REAL_IN>(in, ibs, iss, ies, out, obs, oss, oes, nseq, spb, kout, st);
-    case 192: return fft1d_n<192, SIGN, REAL_IN>(in, ibs, iss, ies, out, obs, oss, oes, nseq, spb, kout, st);
-    case 224: return fft1d_n<224, SIGN, REAL_IN>(in, ibs, iss, ies, out, obs, oss, oes, nseq, spb, kout, st);
-    case 256: return fft1d_n<256, SIGN, REAL_IN>(in, ibs, iss, ies, out, obs, oss, oes, nseq, spb, kout, st);
+    case 64: return fft1d_n<64, SIGN, IN>(in, in_scale, ibs, iss, ies, out, out32, obs, oss, oes, nseq, spb, kout, st);
+    case 96: return fft1d_n<96, SIGN, IN>(in, in_scale, ibs, iss, ies, out, out32, obs, oss, oes, nseq, spb, kout, st);
+    case 128: return fft1d_n<128, SIGN, IN>(in, in_scale, ibs, iss, ies, out, out32, obs, oss, oes, nseq, spb, kout, st);
+    case 160: return fft1d_n<160, SIGN, IN>(in, in_scale, ibs, iss, ies, out, out32, obs, oss, oes, nseq, spb, kout, st);
+    case 170: return fft1d_n<170, SIGN, IN>(in, in_scale, ibs, iss, ies, out, out32, obs, oss, oes, nseq, spb, kout, st);
+    case 192: return fft1d_n<192, SIGN, IN>(in, in_scale, ibs, iss, ies, out, out32, obs, oss, oes, nseq, spb, kout, st);
+    case 224: return fft1d_n<224, SIGN, IN>(in, in_scale, ibs, iss, ies, out, out32, obs, oss, oes, nseq, spb, kout, st);
+    case 256: return fft1d_n<256, SIGN, IN>(in, in_scale, ibs, iss, ies, out, out32, obs, oss, oes, nseq, spb, kout, st);
     default: return cudaErrorInvalidValue;
     }
 }
@@ -146,10 +154,19 @@ cudaError_t launch_fft2_r2c_f64(const double *in, int batch, int N, cd *tmp, cd 
     const int NC = N / 2 + 1;
     const long H = (long)NC * N;
     // along x: sequence = row k of image b
-    cudaError_t e = fft1d<-1, true>(N, in, (long)N * N, N, 1, tmp, H, 1, N, batch * N, N, NC, st);
+    cudaError_t e = fft1d<-1, IN_REAL>(N, in, (long)N * N, N, 1, tmp, H, 1, N, batch * N, N, NC, st);
     if (e != cudaSuccess) return e;
     // along y: sequence = column l of image b
-    return fft1d<-1, false>(N, tmp, H, N, 1, out, H, N, 1, batch * NC, NC, N, st);
+    return fft1d<-1, IN_CPLX>(N, tmp, H, N, 1, out, H, N, 1, batch * NC, NC, N, st);
+}
+// the same for the fixed-point projections of k_project (x = q * in_scale), with the FP32 copy of the spectrum written alongside
+cudaError_t launch_fft2_r2c_fixed(const long long *in, double in_scale, int batch, int N, cd *tmp, cd *out, cf *out32, cudaStream_t st)
+{
+    const int NC = N / 2 + 1;
+    const long H = (long)NC * N;
+    cudaError_t e = fft1d<-1, IN_FIXED>(N, in, (long)N * N, N, 1, tmp, H, 1, N, batch * N, N, NC, st, in_scale);
+    if (e != cudaSuccess) return e;
+    return fft1d<-1, IN_CPLX>(N, tmp, H, N, 1, out, H, N, 1, batch * NC, NC, N, st, 1.0, out32);
 }
 
 __global__ void k_cast_spec(const cd *in, cf *out, size_t n)
@@ -231,20 +248,14 @@ __global__ void __launch_bounds__(256) k_project(const double *xyz, const double
     }
 }
 
-__global__ void k_fixed_to_double(const long long *acc, double *out, size_t n, double inv_scale)
-{
-    size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < n) out[i] = (double)acc[i] * inv_scale;
-}
-
+// acc: [n_orient][N][N] fixed-point pixels, value = acc / fx_scale (launch_fft2_r2c_fixed converts on load)
 cudaError_t launch_project_atoms(const double *xyz, const double *rad, const double *wt, int n_atoms, const double *rot, int n_orient,
-                                 int N, double px, double fx_scale, long long *acc, double *out, cudaStream_t st)
+                                 int N, double px, double fx_scale, long long *acc, cudaStream_t st)
 {
     size_t n = (size_t)n_orient * N * N;
     cudaError_t e = cudaMemsetAsync(acc, 0, n * sizeof(long long), st);
     if (e != cudaSuccess) return e;
     k_project<<<dim3(n_orient, (n_atoms + 255) / 256), 256, 0, st>>>(xyz, rad, wt, n_atoms, rot, N, px, fx_scale, acc);
-    k_fixed_to_double<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(acc, out, n, 1.0 / fx_scale);
     return cudaGetLastError();
 }
 
@@ -271,13 +282,13 @@ cudaError_t launch_dft3_f64(const float *rho, int N, cd *work_a, cd *work_b, cud
     const long N2 = (long)N * N;
     k_rho_to_cd<<<(unsigned)((n3 + 255) / 256), 256, 0, st>>>(rho, work_a, n3);
     // x: sequences (z,y) contiguous
-    cudaError_t e = fft1d<-1, false>(N, work_a, 0, N, 1, work_b, 0, N, 1, N * N, N * N, N, st);
+    cudaError_t e = fft1d<-1, IN_CPLX>(N, work_a, 0, N, 1, work_b, 0, N, 1, N * N, N * N, N, st);
     if (e != cudaSuccess) return e;
     // y: batch z, sequence kx, element stride N
-    e = fft1d<-1, false>(N, work_b, N2, 1, N, work_a, N2, 1, N, N * N, N, N, st);
+    e = fft1d<-1, IN_CPLX>(N, work_b, N2, 1, N, work_a, N2, 1, N, N * N, N, N, st);
     if (e != cudaSuccess) return e;
     // z: sequence (ky,kx) flat, element stride N^2
-    e = fft1d<-1, false>(N, work_a, 0, 1, N2, work_b, 0, 1, N2, N * N, N * N, N, st);
+    e = fft1d<-1, IN_CPLX>(N, work_a, 0, 1, N2, work_b, 0, 1, N2, N * N, N * N, N, st);
     if (e != cudaSuccess) return e;
     e = cudaMemcpyAsync(work_a, work_b, n3 * sizeof(cd), cudaMemcpyDeviceToDevice, st);
     if (e != cudaSuccess) return e;

@@ -62,6 +62,19 @@ def default_score(ctx, block) -> dict:
     return dict(logp=ctx.get_log_posterior(), **ctx.get_best())
 
 
+def run_in_subsets(ctx, images, subset: int, score=None) -> dict:
+    """An image stack that does not fit device memory ("processed in subsets"): `subset` images at a time through one
+    configured context, results concatenated in image order.  The calculated images (a1-a3) are built by the first subset and
+    reused by the others (the context's cache), so the cost over the whole-stack run is one a0 per subset.  The bits are those of
+    the whole-stack run when the orientation chunk is set explicitly (the automatic one depends on the image count)."""
+    if subset < 1:
+        raise ValueError("run_in_subsets: subset must be >= 1")
+    parts = [(score or default_score)(ctx, images[i:i + subset]) for i in range(0, len(images), subset)]
+    if not parts:
+        return {}
+    return {k: np.concatenate([np.asarray(p[k]) for p in parts], axis=0) for k in parts[0]}
+
+
 def score_block_and_gather(ctx, block, n_images: int, score=None, group=None) -> dict:
     """This rank already holds ITS block of a stack of `n_images` images (block r = image_shard(n_images, r, world); e.g. each
     rank read its own part of the stack): score it and all_gather the per-image results in image order."""

@@ -730,6 +730,9 @@ def test_image_subsets_reuse_the_calculated_images():
         assert np.array_equal(np.concatenate([p[0] for p in parts]), whole[0])
         assert np.array_equal(np.concatenate([p[1] for p in parts]), whole[1])
         assert max(launches) < n_first                                       # no projection / CTF-table / statistics launches
+        from paper_1609_06634_b200.shard import run_in_subsets              # the same through the helper, ragged last subset
+        sub = run_in_subsets(b, wl["images"], 2)
+        assert np.array_equal(sub["logp"], whole[0]) and np.array_equal(sub["orient"], whole[1])
         b.invalidate_precompute()
         b.run()
         assert b.get_launch_count()[0] == n_first - 0 or b.get_launch_count()[0] >= max(launches)

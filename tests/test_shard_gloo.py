@@ -28,6 +28,20 @@ def _score(ctx, block):
     return dict(logp=np.stack([s.sum(1), (s * s).sum(1)], axis=1), orient=np.argmax(s, axis=1).astype(np.int32)[:, None])
 
 
+def test_run_in_subsets_concatenates_in_image_order():
+    # a stack processed in subsets; ragged last subset, a subset larger than the stack, an empty stack
+    from paper_1609_06634_b200.shard import run_in_subsets
+    rng = np.random.default_rng(3)
+    images = rng.normal(size=(11, 4, 4)).astype(np.float32)
+    want = _score(None, images)
+    for subset in (1, 3, 4, 11, 50):
+        got = run_in_subsets(None, images, subset, score=_score)
+        assert set(got) == set(want) and all(np.array_equal(got[k], want[k]) and got[k].dtype == want[k].dtype for k in want)
+    assert run_in_subsets(None, images[:0], 4, score=_score) == {}
+    with pytest.raises(ValueError):
+        run_in_subsets(None, images, 0, score=_score)
+
+
 def _worker(rank, world, port, n_img, q):
     import torch.distributed as dist
     from paper_1609_06634_b200.shard import run_sharded

@@ -42,8 +42,10 @@ def test_noalloc_ensemble_matches_existing_path_twice_in_a_row():
     # warm call (loads the two kernels), then the calls that are checked: back to back on one stream, no sync in between
     BioEM.ensemble_log_posterior_noalloc(d_logp, None, d_tot[0:1], d_per[0], device=0, stream=stream)
     torch.cuda.synchronize()
-    free_before, _ = torch.cuda.mem_get_info(dev)
-    for rep in range(2):
+    free_before = None
+    for rep in range(3):
+        if rep == 1:                                                  # everything below has run once: torch's kernels are loaded too
+            free_before, _ = torch.cuda.mem_get_info(dev)
         d_tot.fill_(float("nan"))
         d_per.fill_(float("nan"))
         for k in range(len(weight_sets)):
@@ -54,7 +56,7 @@ def test_noalloc_ensemble_matches_existing_path_twice_in_a_row():
             assert abs(tot[k] - rtot) <= RTOL * abs(rtot), (rep, k, tot[k], rtot)
             assert np.abs(per[k] - rper).max() <= RTOL * np.abs(rper).max(), (rep, k)
     free_after, _ = torch.cuda.mem_get_info(dev)
-    assert free_after >= free_before, (free_before, free_after)      # nothing was allocated on the device by the six calls
+    assert free_after >= free_before, (free_before, free_after)      # nothing was allocated on the device by the last six calls
 
 
 def test_noalloc_stale_contents_and_optional_output():

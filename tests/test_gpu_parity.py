@@ -271,6 +271,45 @@ def test_kernel_plan_edges(base, D, n_img, stride, nctf):
     assert np.abs(best["log_p"][:, 0] - st.best).max() <= TOL_LOGP
 
 
+@pytest.mark.parametrize("base,dmax,strides", [("tiny_mini", 17, (1, 2)), ("small_mini", 17, (768, 1152)), ("paper_mini", 33, (1024, 2048))])
+def test_every_shift_range(base, dmax, strides):
+    """Every shift range D = 0 .. dmax of a box size (the kernels' task tables, Horner masks and row-pair counts depend on D; past
+    the tuned kernels' limit the generic kernel takes over), each with a seeded draw of image count, orientation count, CTF count,
+    orientation chunk and the per-orientation option: log-posterior, argmax and (with the option) the log-sum-exp over
+    orientations against the oracle.  (The same sweep with 13 seeds, 910 cases, ran clean at the end of round 2.)"""
+    import oracle
+    from paper_1609_06634_b200 import BioEM
+    rng = np.random.default_rng(1)
+    for D in range(dmax + 1):
+        n_img, stride, nctf, chunk = int(rng.integers(1, 4)), int(rng.choice(strides)), int(rng.integers(1, 5)), int(rng.integers(1, 5))
+        opt = bool(rng.integers(2))
+        wl = W.build_workload(W.get_spec(base, n_images=n_img, orient_stride=stride))
+        s = wl["spec"]
+        quats, ctfs, imgs = wl["quats"], wl["ctfs"][:nctf], wl["images"]
+        with BioEM() as b:
+            b.load_workload(wl, images=False)
+            b.set_ctf_grid(ctfs[:, 0], ctfs[:, 1], ctfs[:, 2])
+            b.set_shift_range(D)
+            b.set_orientation_chunk(chunk)
+            b.set_orientation_posterior(opt)
+            b.push_images(imgs)
+            b.run()
+            got, best = b.get_log_posterior(), b.get_best()
+            po = b.get_orientation_log_posterior() if opt else None
+        st = oracle.run_model(wl["models"][0], s.n_pix, s.pixel_A, D, quats, ctfs, imgs)
+        case = (base, D, n_img, stride, nctf, chunk, opt)
+        assert np.abs(got[:, 0] - st.log_posterior()).max() <= TOL_LOGP, case
+        o, c, dx, dy = oracle.unflatten(st.best_flat, len(ctfs), D)
+        tie = (st.best - st.second) < 1e-6
+        for k, ref in (("orient", o), ("ctf", c), ("dx", dx), ("dy", dy)):
+            assert np.all((best[k][:, 0] == ref) | tie), (case, k)
+        assert np.abs(best["log_p"][:, 0] - st.best).max() <= TOL_LOGP, case
+        if opt:
+            g = po[:, 0, :]
+            m = g.max(axis=1)
+            assert np.abs(m + np.log(np.exp(g - m[:, None]).sum(axis=1)) - st.log_posterior()).max() <= TOL_LOGP, case
+
+
 @pytest.mark.parametrize("name", ["tiny_mini", "small_mini", "paper_mini", "density_mini", "ensemble_mini"])
 def test_orientation_posterior(name):
     """posterior per orientation.  Bar: entries that matter (within 30 log-units of the image's

@@ -421,7 +421,8 @@ int bioem_run_partial(bioem_ctx *ctx)
     if (sliced && ctx->want_orient && !fold) FAIL(BIOEM_EUNSUPPORTED, "run: the per-orientation posterior on an orientation slice needs a kernel that folds it (not the cluster kernel)");
     if (ctx->want_orient && !fold) oc = 1;
     if (fold && oc > 32) oc = 32;
-    if (sliced && o_first % oc != 0) FAIL(BIOEM_EBADARG, "run: an orientation slice must begin at a multiple of the orientation chunk");
+    // (an EMPTY slice -- a rank beyond the last chunk, [n_orient, n_orient) -- begins wherever the grid ends)
+    if (sliced && O > 0 && o_first % oc != 0) FAIL(BIOEM_EBADARG, "run: an orientation slice must begin at a multiple of the orientation chunk");
     const int cpm = (O + oc - 1) / oc;
     const int ppi = use_c2 ? 2 : 1;                                       // partials per work item (the cluster kernel writes one per CTA)
     const size_t items = (size_t)I * M * cpm * ppi;

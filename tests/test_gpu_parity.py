@@ -618,7 +618,8 @@ def test_split_stack_is_bit_identical():
     assert np.array_equal(outs[0][0], outs[1][0]) and np.array_equal(outs[0][1], outs[1][1])
 
 
-@pytest.mark.parametrize("name,chunk,world", [("small_mid", 5, 3), ("paper_mid", 2, 2), ("ensemble_mid", 4, 2), ("tiny_mid", 32, 3)])
+@pytest.mark.parametrize("name,chunk,world", [("small_mid", 5, 3), ("paper_mid", 2, 2), ("ensemble_mid", 4, 2), ("tiny_mid", 32, 3),
+                                              ("tiny_mini", 3, 4)])                # 2 chunks over 4 ranks: two ranks hold an empty slice
 def test_orientation_sharding_is_bit_identical(name, chunk, world):
     """the orientation grid cut over `world` ranks (here: contexts on one GPU, run one after
     the other, the two exchanges done by hand on the host exactly as shard.run_orientation_sharded does them with
@@ -670,7 +671,7 @@ def test_orientation_sharding_is_bit_identical(name, chunk, world):
     assert np.abs(one["logp"] - ref["logp"]).max() <= TOL_LOGP
 
 
-@pytest.mark.parametrize("name,chunk,world", [("small_mid", 5, 3), ("paper_mid", 4, 2), ("ensemble_mid", 48, 2)])
+@pytest.mark.parametrize("name,chunk,world", [("small_mid", 5, 3), ("paper_mid", 4, 2), ("ensemble_mid", 48, 2), ("paper_mini", 3, 3)])
 def test_orientation_posterior_under_orientation_sharding(name, chunk, world):
     """8(f) #1 with 8(f) #5: every rank (a context on this GPU, the exchanges by hand as above) produces the per-orientation
     posterior of ITS orientations; side by side they are the output of one context over the whole grid, bit for bit.  A chunk

@@ -782,6 +782,84 @@ def test_image_subsets_reuse_the_calculated_images():
         assert np.array_equal(b.get_log_posterior(), whole[0])
 
 
+@pytest.mark.parametrize("base", ["small_mini", "ensemble_mini", "paper_mini", "density_mini", "tiny_mini"])
+def test_long_lived_context_equals_a_fresh_one(base):
+    """The calculated-image cache and the options of a context that lives through a seeded sequence of changes (shift range, CTF grid
+    and priors, orientation list and priors, image subset, chunk, per-orientation option, displacement variant, models, explicit
+    invalidation): after every change its run gives the bits of a fresh context configured the same way."""
+    from paper_1609_06634_b200 import BioEM
+    rng = np.random.default_rng(1)
+    wl = W.build_workload(W.get_spec(base, n_images=4))
+    st = dict(models=list(wl["models"]), quats=wl["quats"], ctfs=wl["ctfs"], lpo=None, lpc=None, D=min(wl["spec"].max_shift, 5), variant=0,
+              images=wl["images"], chunk=2, opt=False)
+
+    def add_models(b):
+        b.clear_models()
+        for m in st["models"]:
+            b.add_model_atoms(m["xyz"], m["radius"], m["weight"]) if m["kind"] == "atoms" else b.add_model_density(m["rho"], m["voxel_A"])
+
+    def configure(b):
+        b.set_image_geometry(wl["spec"].n_pix, wl["spec"].pixel_A)
+        add_models(b)
+        b.set_orientations_quat(st["quats"], st["lpo"])
+        b.set_ctf_grid(st["ctfs"][:, 0], st["ctfs"][:, 1], st["ctfs"][:, 2], st["lpc"])
+        b.set_shift_range(st["D"])
+        b.set_displacement_variant(st["variant"])
+        b.push_images(st["images"])
+        b.set_orientation_chunk(st["chunk"])
+        b.set_orientation_posterior(st["opt"])
+
+    def results(b):
+        b.run()
+        out = dict(logp=b.get_log_posterior(), **b.get_best())
+        if st["opt"]:
+            out["po"] = b.get_orientation_log_posterior()
+        return out
+
+    with BioEM() as live:
+        configure(live)
+        results(live)
+        for step in range(14):
+            mut = int(rng.integers(10))
+            if mut == 0:
+                st["D"] = int(rng.integers(0, 7)); live.set_shift_range(st["D"])
+            elif mut == 1:
+                st["ctfs"], st["lpc"] = wl["ctfs"][:int(rng.integers(1, len(wl["ctfs"]) + 1))], None
+                live.set_ctf_grid(st["ctfs"][:, 0], st["ctfs"][:, 1], st["ctfs"][:, 2], None)
+            elif mut == 2:
+                k = int(rng.integers(1, len(wl["quats"]) + 1))
+                st["quats"], st["lpo"] = wl["quats"][:k], (np.log(rng.dirichlet(np.ones(k))).astype(np.float32) if rng.integers(2) else None)
+                live.set_orientations_quat(st["quats"], st["lpo"])
+            elif mut == 3:
+                i0 = int(rng.integers(0, 3)); st["images"] = wl["images"][i0:i0 + int(rng.integers(1, 3))]
+                live.push_images(st["images"])
+            elif mut == 4:
+                st["chunk"] = int(rng.integers(1, 4)); live.set_orientation_chunk(st["chunk"])
+            elif mut == 5:
+                st["opt"] = (not st["opt"]) if st["variant"] == 0 else False; live.set_orientation_posterior(st["opt"])
+            elif mut == 6:
+                st["lpc"] = np.log(rng.dirichlet(np.ones(len(st["ctfs"])))).astype(np.float32)
+                live.set_ctf_grid(st["ctfs"][:, 0], st["ctfs"][:, 1], st["ctfs"][:, 2], st["lpc"])
+            elif mut == 7:
+                st["variant"] = 1 - st["variant"]
+                if st["variant"] == 1:                                   # real space: no per-orientation output, few displacements
+                    st["opt"], st["D"] = False, min(st["D"], 3)
+                    live.set_orientation_posterior(False); live.set_shift_range(st["D"])
+                live.set_displacement_variant(st["variant"]); live.push_images(st["images"])
+            elif mut == 8:
+                live.invalidate_precompute()
+            elif len(wl["models"]) > 1:
+                st["models"] = list(wl["models"][:int(rng.integers(1, len(wl["models"]) + 1))])
+                add_models(live)
+            got = results(live)
+            with BioEM() as fresh:
+                configure(fresh)
+                want = results(fresh)
+            assert set(got) == set(want), (step, mut)
+            for k in want:
+                assert np.array_equal(got[k], want[k]), (step, mut, k)
+
+
 @pytest.mark.parametrize("name,D", [("tiny_mini", 4), ("small_mini", 2), ("paper_mini", 1), ("density_mini", 2), ("ensemble_mini", 3)])
 def test_real_space_cropping_variant(name, D):
     """the real-space displacement variant against the oracle's tier 2 (bo_cropped_sums),

@@ -101,3 +101,33 @@ def test_noalloc_rejects_sizes_beyond_the_work_array():
     BioEM.ensemble_log_posterior_noalloc(full, None, out, per)
     torch.cuda.synchronize()
     assert abs(out.item()) <= 1e-9 and per.abs().max().item() <= 1e-15
+
+
+def test_noalloc_entry_point_under_graph_capture():
+    """What the entry point is for: it can be captured into a CUDA graph (nothing in it allocates or synchronises) and replayed on
+    new contents of the same buffers."""
+    import torch
+    from paper_1609_06634_b200 import BioEM
+    dev = torch.device("cuda", 0)
+    rng = np.random.default_rng(0)
+    logp = torch.from_numpy(rng.normal(size=(1000, 5)) * 10 - 3000).to(dev)
+    w = torch.tensor([0.1, 0.2, 0.3, 0.25, 0.15], dtype=torch.float64, device=dev)
+    tot = torch.zeros(1, dtype=torch.float64, device=dev)
+    per = torch.zeros(1000, dtype=torch.float64, device=dev)
+    BioEM.noalloc_prepare(0)                                         # the symbol's address is taken before the capture begins
+    BioEM.ensemble_log_posterior_noalloc(logp, w, tot, per)          # eager: loads the kernels, gives the expected values
+    torch.cuda.synchronize()
+    want_tot, want_per = tot.item(), per.clone()
+    tot.zero_(); per.zero_()
+    torch.cuda.synchronize()
+    graph, side = torch.cuda.CUDAGraph(), torch.cuda.Stream()
+    with torch.cuda.graph(graph, stream=side):
+        BioEM.ensemble_log_posterior_noalloc(logp, w, tot, per, device=0, stream=torch.cuda.current_stream().cuda_stream)
+    assert tot.item() == 0.0                                         # captured, not run
+    graph.replay()
+    torch.cuda.synchronize()
+    assert tot.item() == want_tot and torch.equal(per, want_per)
+    logp += 1.0                                                      # every log P up by one: every inner sum too
+    graph.replay()
+    torch.cuda.synchronize()
+    assert abs(tot.item() - (want_tot + 1000.0)) <= 1e-9 * abs(want_tot) and (per - want_per - 1.0).abs().max().item() <= 1e-9

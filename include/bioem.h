@@ -160,7 +160,8 @@ int bioem_set_orientation_chunk(bioem_ctx *ctx, int n_orient_per_item);
  * all n pixels, so C_co, C_c and C_cc depend on d (reading R25 in DESIGN.md).  The paper's route for very few displacements
  * (Fig. 2): (2D+1)^2 n multiply-adds per pair, FP64 throughout (no re-scoring step), deterministic.  Call BEFORE
  * bioem_push_images (the real-space variant keeps the mean-free images in real space); BIOEM_EBADSTATE at bioem_run otherwise.
- * Not combinable with orientation slices or the per-orientation posterior (BIOEM_EUNSUPPORTED). */
+ * The per-orientation posterior is available with it (running sums per (image, model, orientation), FP64); orientation slices are
+ * not (BIOEM_EUNSUPPORTED). */
 int bioem_set_displacement_variant(bioem_ctx *ctx, int variant);
 
 /* ---- orientation sharding: the paper's MPI axis ("MPI over orientations"; no communication but one gather) ----

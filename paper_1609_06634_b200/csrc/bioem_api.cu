@@ -498,7 +498,7 @@ int bioem_run_partial(bioem_ctx *ctx)
 
     if (ctx->variant == 1) {
         // ---- the real-space, cropping variant: FP64 scoring of every calculated image against every image
-        if (sliced || ctx->want_orient) FAIL(BIOEM_EUNSUPPORTED, "run: the real-space variant supports neither orientation slices nor the per-orientation posterior");
+        if (sliced) FAIL(BIOEM_EUNSUPPORTED, "run: the real-space variant does not support orientation slices");
         if (ctx->img_variant != 1) FAIL(BIOEM_EBADSTATE, "run: set the displacement variant before bioem_push_images (the real-space variant keeps the images in real space)");
         const int S = (2 * D + 1) * (2 * D + 1), RB = 64;                 // calculated images per batch
         const size_t IM = (size_t)I * M;
@@ -518,7 +518,15 @@ int bioem_run_partial(bioem_ctx *ctx)
         CK(ctx->logp32.ensure(IM * sizeof(double)));
         CK(ctx->best.ensure(IM * 4 * sizeof(int32_t)));
         CK(ctx->best_logp.ensure(IM * sizeof(double)));
+        double *po_m = nullptr, *po_s = nullptr;                         // posterior per orientation: running (m, s) per (image, model, orientation)
+        if (ctx->want_orient) {
+            CK(ctx->orient_m.ensure(IM * O * sizeof(double)));
+            CK(ctx->orient_s.ensure(IM * O * sizeof(double)));
+            CK(ctx->logp_orient.ensure(IM * O * sizeof(double)));
+            po_m = ctx->orient_m.as<double>(); po_s = ctx->orient_s.as<double>();
+        }
         CK(cudaEventRecord(ctx->ev[1], st));
+        if (po_m) { CK(launch_rs_orient_init(IM * O, po_m, po_s, st)); ctx->launches += 1; }
         CK(launch_rs_init((int)IM, ctx->rs_m.as<double>(), ctx->rs_s.as<double>(), ctx->rs_best.as<double>(), ctx->rs_bpair.as<long long>(),
                           ctx->rs_bshift.as<int>(), st));
         ctx->launches += 1;
@@ -533,7 +541,7 @@ int bioem_run_partial(bioem_ctx *ctx)
                     CK(launch_rs_score(ctx->Oreal64.as<double>(), ctx->Dw.as<double>(), ctx->rs_I1.as<double>(), ctx->rs_logw.as<double>(),
                                        ctx->rs_pair.as<long long>(), nb, I, M, mi, N, D, ctx->rs_cc.as<double>(), ctx->rs_ccc.as<double>(), ctx->rs_part.p,
                                        ctx->rs_m.as<double>(), ctx->rs_s.as<double>(), ctx->rs_best.as<double>(), ctx->rs_bpair.as<long long>(),
-                                       ctx->rs_bshift.as<int>(), ctx->flags.as<int>() + 1, st));
+                                       ctx->rs_bshift.as<int>(), ctx->flags.as<int>() + 1, po_m, po_s, O, o0, st));
                     ctx->launches += 6; ctx->fused_launches += 1;
                 }
             }
@@ -544,11 +552,15 @@ int bioem_run_partial(bioem_ctx *ctx)
                            ctx->rs_bshift.as<int>(), ctx->Dw.as<double>(), I, M, C, N, D, const_n, ctx->logp.as<double>(), ctx->logp32.as<double>(),
                            ctx->best.as<int32_t>(), ctx->best_logp.as<double>(), st));
         ctx->launches += 1;
+        if (po_m) {
+            CK(launch_rs_orient_final(po_m, po_s, ctx->Dw.as<double>(), I, M, O, N, const_n, ctx->logp_orient.as<double>(), st));
+            ctx->launches += 1;
+        }
         CK(cudaEventRecord(ctx->ev[3], st));
         ctx->pre_valid = true; ctx->flags_checked = false;
         ctx->run_kernel = KERNEL_REALSPACE; ctx->run_oc = 0; ctx->run_o_first = 0; ctx->run_o_local = O; ctx->run_chunks = 0;
         ctx->run_models = M; ctx->run_orient = Ofull; ctx->run_ctf = C; ctx->run_D = D; ctx->run_img = I;
-        ctx->ran = true; ctx->ran_orient = false; ctx->phase = 4;
+        ctx->ran = true; ctx->ran_orient = po_m != nullptr; ctx->phase = 4;
         return BIOEM_OK;
     }
 

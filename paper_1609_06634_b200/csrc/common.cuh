@@ -118,7 +118,11 @@ cudaError_t launch_rs_batch_meta(const double *h64, const double *Tc64, int mode
                                  long long *pair_of, cudaStream_t st);
 cudaError_t launch_rs_score(const double *Oc, const double *Dw, const double *I1, const double *logw, const long long *pair_of, int nb, int n_img,
                             int n_model, int model, int N, int D, double *cc, double *ccc, void *part, double *acc_m, double *acc_s,
-                            double *acc_best, long long *acc_pair, int *acc_shift, int *flags, cudaStream_t st);
+                            double *acc_best, long long *acc_pair, int *acc_shift, int *flags, double *po_m, double *po_s, int n_orient, int o0,
+                            cudaStream_t st);
+cudaError_t launch_rs_orient_init(size_t n, double *po_m, double *po_s, cudaStream_t st);
+cudaError_t launch_rs_orient_final(const double *po_m, const double *po_s, const double *Dw, int n_img, int n_model, int n_orient, int N, double const_n,
+                                   double *out, cudaStream_t st);
 cudaError_t launch_rs_init(int n, double *acc_m, double *acc_s, double *acc_best, long long *acc_pair, int *acc_shift, cudaStream_t st);
 cudaError_t launch_rs_final(const double *acc_m, const double *acc_s, const double *acc_best, const long long *acc_pair, const int *acc_shift,
                             const double *Dw, int n_img, int n_model, int n_ctf, int N, int D, double const_n, double *logp, double *logp32,

@@ -159,9 +159,11 @@ __global__ void __launch_bounds__(256) k_rs_score(const double *Oc, const double
     }
 }
 
-// ---- fold the batch into the running sums, calculated images in batch order; one thread per image
+// ---- fold the batch into the running sums, calculated images in batch order; one thread per image.  po_m != NULL (posterior per
+// orientation): calculated image b of the batch belongs to orientation o0 + b, whose own running sum
+// po[(img * n_model + model) * n_orient + o] takes the same term (the batches of the other CTFs of that orientation follow in stream order).
 __global__ void k_rs_merge(const RsPartial *part, const long long *pair_of, int nb, int n_img, int n_model, int model, double *acc_m, double *acc_s,
-                           double *acc_best, long long *acc_pair, int *acc_shift)
+                           double *acc_best, long long *acc_pair, int *acc_shift, double *po_m, double *po_s, int n_orient, int o0)
 {
     const int img = blockIdx.x * blockDim.x + threadIdx.x;
     if (img >= n_img) return;
@@ -173,6 +175,11 @@ __global__ void k_rs_merge(const RsPartial *part, const long long *pair_of, int 
         const RsPartial p = part[(size_t)b * n_img + img];
         if (!p.valid) continue;
         if (p.m > M) { Ssum = Ssum * exp(M - p.m) + p.s; M = p.m; } else Ssum += p.s * exp(p.m - M);
+        if (po_m) {
+            const size_t io = im * n_orient + o0 + b;
+            const double m0 = po_m[io], s0 = po_s[io];
+            if (p.m > m0) { po_s[io] = s0 * exp(m0 - p.m) + p.s; po_m[io] = p.m; } else po_s[io] = s0 + p.s * exp(p.m - m0);
+        }
         const long long pr = pair_of[b];
         if (p.best > best || (p.best == best && (bp < 0 || pr < bp))) { best = p.best; bp = pr; bsft = p.shift; }
     }
@@ -184,6 +191,23 @@ __global__ void k_rs_init(int n, double *acc_m, double *acc_s, double *acc_best,
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     acc_m[i] = -CUDART_INF; acc_s[i] = 0.0; acc_best[i] = -CUDART_INF; acc_pair[i] = -1; acc_shift[i] = 0;
+}
+
+__global__ void k_rs_orient_init(size_t n, double *po_m, double *po_s)
+{
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) { po_m[i] = -CUDART_INF; po_s[i] = 0.0; }
+}
+
+// out[img][model][o] = log sum_{ctf, d} w P of orientation o (FP64 throughout: nothing to re-score)
+__global__ void k_rs_orient_final(const double *po_m, const double *po_s, const double *Dw, int n_img, int n_model, int n_orient, int N, double const_n,
+                                  double *out)
+{
+    const size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= (size_t)n_img * n_model * n_orient) return;
+    const int img = (int)(idx / ((size_t)n_model * n_orient));
+    const double n = (double)N * N;
+    out[idx] = po_s[idx] > 0.0 ? const_n - 0.5 * (n - 3.0) * log(Dw[img]) + po_m[idx] + log(po_s[idx]) : -CUDART_INF;
 }
 
 __global__ void k_rs_final(const double *acc_m, const double *acc_s, const double *acc_best, const long long *acc_pair, const int *acc_shift,
@@ -238,7 +262,8 @@ cudaError_t launch_rs_batch_meta(const double *h64, const double *Tc64, int mode
 
 cudaError_t launch_rs_score(const double *Oc, const double *Dw, const double *I1, const double *logw, const long long *pair_of, int nb, int n_img,
                             int n_model, int model, int N, int D, double *cc, double *ccc, void *part, double *acc_m, double *acc_s,
-                            double *acc_best, long long *acc_pair, int *acc_shift, int *flags, cudaStream_t st)
+                            double *acc_best, long long *acc_pair, int *acc_shift, int *flags, double *po_m, double *po_s, int n_orient, int o0,
+                            cudaStream_t st)
 {
     const int S = (2 * D + 1) * (2 * D + 1);
     k_rs_crop_sums<<<dim3(S, nb), 256, 0, st>>>(I1, N, D, cc, ccc);
@@ -249,7 +274,21 @@ cudaError_t launch_rs_score(const double *Oc, const double *Dw, const double *I1
     }
     k_rs_score<<<dim3(n_img, nb), 256, sm, st>>>(Oc, Dw, I1, cc, ccc, logw, n_img, N, D, static_cast<RsPartial *>(part), flags);
     k_rs_merge<<<(n_img + 127) / 128, 128, 0, st>>>(static_cast<const RsPartial *>(part), pair_of, nb, n_img, n_model, model, acc_m, acc_s, acc_best,
-                                                     acc_pair, acc_shift);
+                                                     acc_pair, acc_shift, po_m, po_s, n_orient, o0);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_rs_orient_init(size_t n, double *po_m, double *po_s, cudaStream_t st)
+{
+    k_rs_orient_init<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(n, po_m, po_s);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_rs_orient_final(const double *po_m, const double *po_s, const double *Dw, int n_img, int n_model, int n_orient, int N, double const_n,
+                                   double *out, cudaStream_t st)
+{
+    const size_t n = (size_t)n_img * n_model * n_orient;
+    k_rs_orient_final<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(po_m, po_s, Dw, n_img, n_model, n_orient, N, const_n, out);
     return cudaGetLastError();
 }
 

@@ -890,6 +890,33 @@ def test_real_space_cropping_variant(name, D):
     assert np.abs(got - circ).max() > 1e-4                                   # not the circular variant
 
 
+@pytest.mark.parametrize("name,D", [("tiny_mini", 3), ("ensemble_mini", 1), ("paper_mini", 2)])
+def test_real_space_variant_orientation_posterior(name, D):
+    """P:225 with the real-space displacement variant (8(f) #1 with #3): every entry against the oracle's tier-2 loop nest restricted
+    to that orientation (weights of the full grid); FP64 on both sides."""
+    import oracle
+    from paper_1609_06634_b200 import BioEM
+    wl = W.build_workload(name)
+    s = wl["spec"]
+    with BioEM() as b:
+        b.load_workload(wl, images=False)
+        b.set_shift_range(D)
+        b.set_displacement_variant(1)
+        b.set_orientation_posterior(True)
+        b.push_images(wl["images"])
+        b.run()
+        po, lp = b.get_orientation_log_posterior(), b.get_log_posterior()
+        assert b.get_run_plan()[0] == 6
+    assert po.shape == (s.n_images, s.n_models, len(wl["quats"]))
+    for mi, model in enumerate(wl["models"]):
+        model = oracle.prepare_model(model)
+        for o in range(len(wl["quats"])):
+            ref = oracle.run_model(model, s.n_pix, s.pixel_A, D, wl["quats"], wl["ctfs"], wl["images"], o_begin=o, o_end=o + 1, tier=2).log_posterior()
+            assert np.abs(po[:, mi, o] - ref).max() <= 1e-6, (mi, o, np.abs(po[:, mi, o] - ref).max())
+        m = po[:, mi, :].max(axis=1)
+        assert np.abs(m + np.log(np.exp(po[:, mi, :] - m[:, None]).sum(axis=1)) - lp[:, mi]).max() <= 1e-9
+
+
 def test_real_space_variant_needs_its_images():
     from paper_1609_06634_b200 import BioEM
     from paper_1609_06634_b200.binding import BioEMError

@@ -836,15 +836,15 @@ def test_long_lived_context_equals_a_fresh_one(base):
             elif mut == 4:
                 st["chunk"] = int(rng.integers(1, 4)); live.set_orientation_chunk(st["chunk"])
             elif mut == 5:
-                st["opt"] = (not st["opt"]) if st["variant"] == 0 else False; live.set_orientation_posterior(st["opt"])
+                st["opt"] = not st["opt"]; live.set_orientation_posterior(st["opt"])
             elif mut == 6:
                 st["lpc"] = np.log(rng.dirichlet(np.ones(len(st["ctfs"])))).astype(np.float32)
                 live.set_ctf_grid(st["ctfs"][:, 0], st["ctfs"][:, 1], st["ctfs"][:, 2], st["lpc"])
             elif mut == 7:
                 st["variant"] = 1 - st["variant"]
-                if st["variant"] == 1:                                   # real space: no per-orientation output, few displacements
-                    st["opt"], st["D"] = False, min(st["D"], 3)
-                    live.set_orientation_posterior(False); live.set_shift_range(st["D"])
+                if st["variant"] == 1:                                   # real space: few displacements
+                    st["D"] = min(st["D"], 3)
+                    live.set_shift_range(st["D"])
                 live.set_displacement_variant(st["variant"]); live.push_images(st["images"])
             elif mut == 8:
                 live.invalidate_precompute()

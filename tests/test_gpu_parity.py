@@ -917,6 +917,39 @@ def test_real_space_variant_orientation_posterior(name, D):
         assert np.abs(m + np.log(np.exp(po[:, mi, :] - m[:, None]).sum(axis=1)) - lp[:, mi]).max() <= 1e-9
 
 
+def test_real_space_variant_seeded_sweep():
+    """The real-space variant over seeded draws of config, shift range (0 .. 3) and image count: log-posterior and argmax against the
+    oracle's tier 2, and the synthetic map of the best parameters (cropped, fitted to the particle) against the oracle's."""
+    import oracle
+    from paper_1609_06634_b200 import BioEM
+    rng = np.random.default_rng(2)
+    for _ in range(12):
+        base = str(rng.choice(["tiny_mini", "small_mini", "density_mini", "ensemble_mini", "paper_mini"]))
+        D, n_img = int(rng.integers(0, 4)), int(rng.integers(1, 4))
+        wl = W.build_workload(W.get_spec(base, n_images=n_img))
+        s = wl["spec"]
+        with BioEM() as b:
+            b.load_workload(wl, images=False)
+            b.set_shift_range(D)
+            b.set_displacement_variant(1)
+            b.push_images(wl["images"])
+            b.run()
+            got, best = b.get_log_posterior(), b.get_best()
+            i = int(rng.integers(n_img))
+            sm, gn, gmu = b.get_synthetic_map(0, int(best["orient"][i, 0]), int(best["ctf"][i, 0]), int(best["dx"][i, 0]), int(best["dy"][i, 0]),
+                                              wl["images"][i])
+        model = oracle.prepare_model(wl["models"][0])
+        st = oracle.run_model(model, s.n_pix, s.pixel_A, D, wl["quats"], wl["ctfs"], wl["images"], tier=2)
+        case = (base, D, n_img)
+        assert np.abs(got[:, 0] - st.log_posterior()).max() <= 1e-6, case
+        o, c, dx, dy = oracle.unflatten(st.best_flat, s.n_ctf, D)
+        for k, ref in (("orient", o), ("ctf", c), ("dx", dx), ("dy", dy)):
+            assert np.array_equal(best[k][:, 0], ref), (case, k)
+        I1 = oracle.calc_image(model, wl["quats"][o[i]], wl["ctfs"][c[i]], s.n_pix, s.pixel_A)
+        ref, rn, rmu = oracle.synthetic_map(I1, int(dx[i]), int(dy[i]), wl["images"][i], crop=True)
+        assert np.abs(sm - ref).max() <= 3e-6 * np.abs(ref).max() and abs(gn - rn) <= 1e-5 * abs(rn), case
+
+
 def test_real_space_variant_needs_its_images():
     from paper_1609_06634_b200 import BioEM
     from paper_1609_06634_b200.binding import BioEMError

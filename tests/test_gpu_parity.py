@@ -727,6 +727,88 @@ def test_orientation_posterior_under_orientation_sharding(name, chunk, world):
             c.close()
 
 
+def test_orientation_sharding_seeded_sweep():
+    """Orientation sharding over seeded draws: config (atoms, density map, several models), CTF count, shift range, orientation and
+    CTF priors, chunk, 1-4 ranks (more ranks than chunks included), the per-orientation option.  One context over the whole grid
+    against the oracle; the emulated ranks against that context, bit for bit."""
+    import oracle
+    from paper_1609_06634_b200 import BioEM
+    from paper_1609_06634_b200.shard import orientation_shard
+    rng = np.random.default_rng(3)
+    for _ in range(10):
+        base = str(rng.choice(["density_mini", "ensemble_mini", "small_mini", "tiny_mini", "paper_mini"]))
+        wl = W.build_workload(W.get_spec(base, n_images=int(rng.integers(1, 4))))
+        s = wl["spec"]
+        nctf, O = int(rng.integers(1, len(wl["ctfs"]) + 1)), len(wl["quats"])
+        ctfs = wl["ctfs"][:nctf]
+        D = int(rng.integers(0, min(s.max_shift, 12) + 1))
+        pri = bool(rng.integers(2))
+        lpo = np.log(rng.dirichlet(np.ones(O))).astype(np.float32) if pri else None
+        lpc = np.log(rng.dirichlet(np.ones(nctf))).astype(np.float32) if pri else None
+        chunk, world, opt = int(rng.integers(1, 4)), int(rng.integers(1, 5)), bool(rng.integers(2))
+        case = (base, nctf, D, pri, chunk, world, opt)
+
+        def configure(b):
+            b.load_workload(wl, images=False)
+            b.set_orientations_quat(wl["quats"], lpo)
+            b.set_ctf_grid(ctfs[:, 0], ctfs[:, 1], ctfs[:, 2], lpc)
+            b.set_shift_range(D)
+            b.push_images(wl["images"])
+            b.set_orientation_chunk(chunk)
+            b.set_orientation_posterior(opt)
+
+        with BioEM() as b:
+            configure(b)
+            b.run()
+            got, best = b.get_log_posterior(), b.get_best()
+            po = b.get_orientation_log_posterior() if opt else None
+        for mi, model in enumerate(wl["models"][:2]):
+            st = oracle.run_model(oracle.prepare_model(model), s.n_pix, s.pixel_A, D, wl["quats"], ctfs, wl["images"],
+                                  lp_orient=None if lpo is None else lpo.astype(np.float64), lp_ctf=None if lpc is None else lpc.astype(np.float64))
+            assert np.abs(got[:, mi] - st.log_posterior()).max() <= TOL_LOGP, case
+            o, c, dx, dy = oracle.unflatten(st.best_flat, nctf, D)
+            tie = (st.best - st.second) < 1e-6
+            for k, ref in (("orient", o), ("ctf", c), ("dx", dx), ("dy", dy)):
+                assert np.all((best[k][:, mi] == ref) | tie), (case, k)
+        ctxs = [BioEM() for _ in range(world)]
+        try:
+            blobs, sizes, chunks = [], [], []
+            for r, c in enumerate(ctxs):
+                configure(c)
+                c.set_orientation_slice(*orientation_shard(O, chunk, r, world))
+                c.run_partial()
+                nb, nc = c.get_partials_size()
+                buf = np.zeros(max(nb, 4), np.uint8)
+                c.export_partials(buf)
+                blobs.append(buf); sizes.append(nb); chunks.append(nc)
+            stride = max(max(sizes), 4)
+            allb = np.zeros(world * stride, np.uint8)
+            for r, bb in enumerate(blobs):
+                allb[r * stride: r * stride + bb.size] = bb
+            g = np.zeros(ctxs[0].rescore_shape())
+            for c in ctxs:
+                c.merge_partials(allb, stride, chunks)
+                c.rescore_local()
+                gr = np.empty_like(g)
+                c.export_rescore(gr)
+                g += gr
+            parts = []
+            for c in ctxs:
+                c.import_rescore(g)
+                c.finish()
+                assert np.array_equal(c.get_log_posterior(), got), case
+                bb = c.get_best()
+                for k in best:
+                    assert np.array_equal(bb[k], best[k]), (case, k)
+                if opt:
+                    parts.append(c.get_orientation_log_posterior())
+            if opt:
+                assert np.array_equal(np.concatenate(parts, axis=2), po), case
+        finally:
+            for c in ctxs:
+                c.close()
+
+
 def test_orientation_slice_errors():
     from paper_1609_06634_b200 import BioEM
     from paper_1609_06634_b200.binding import BioEMError
